@@ -1,0 +1,48 @@
+/* oracle/oracle.h — C interface of the CPU test oracle (TEST INFRASTRUCTURE, NOT THE PRODUCT).
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may load
+ * liboracle.so.  The product library (include/mhd.h, libmhd.so) neither includes this file nor links it.
+ * All pointers are HOST pointers; all field arrays are N^3 doubles laid out [z][y][x] (x fastest).
+ * Functions return 0 on success, a negative number on error (orc_last_error() gives the text).
+ */
+#ifndef ORACLE_H
+#define ORACLE_H
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct orc_ctx orc_ctx;
+
+typedef struct {
+    double t;
+    long long step;
+    double ke, me, ie, mass, mom[3], etot, max_divb, rho_min, p_min;
+} orc_diag;
+
+/* precision: 0 = double arithmetic, 1 = long double arithmetic (inputs/outputs stay double). */
+int orc_create(orc_ctx **out, int N, double L, double gamma, double mu, double eta, double dt, int precision);
+int orc_destroy(orc_ctx *c);
+const char *orc_last_error(void);
+void orc_set_threads(int n);               /* OpenMP threads used by the pencil loops (0 = default)  */
+int orc_get_threads(void);
+int orc_use_direct_dft(orc_ctx *c, int on); /* substitute the O(N^6) DFT for the FFT (pin P13)        */
+
+int orc_set_fields(orc_ctx *c, int kind, const double *const f[8]);  /* 0 conservative, 1 primitive  */
+int orc_get_fields(orc_ctx *c, int kind, double *const out[8]);
+int orc_rhs(orc_ctx *c, double *const out[8]);                       /* dU/dt of the current state    */
+int orc_rhs_scales(orc_ctx *c, double *const out[8], double phi[8], double dsc[8]);
+int orc_step(orc_ctx *c, int nsteps);
+int orc_nspec(orc_ctx *c);
+int orc_diagnostics(orc_ctx *c, orc_diag *d, double *spec_kin, double *spec_mag, int nspec);
+
+/* operator family O1 on one field: op 0,1,2 = d/dx,d/dy,d/dz; 3 = Laplacian; 4 = dealias projection */
+int orc_apply(orc_ctx *c, int op, const double *in, double *out);
+
+/* transforms O0 on interleaved (re,im) complex N^3 arrays; sign -1 forward (unnormalised), +1 inverse (1/N^3) */
+int orc_fft3(int N, int sign, int precision, const double *in, double *out);
+int orc_dft3_direct(int N, int sign, int precision, const double *in, double *out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,122 @@
+// oracle/oracle_capi.cpp — C interface of the CPU test oracle (TEST INFRASTRUCTURE, NOT THE PRODUCT).
+// See oracle/oracle.h and oracle/mhd_oracle.hpp.  Build: oracle/build_oracle.py (g++ -O2 -fopenmp -shared).
+#include "oracle.h"
+#include "mhd_oracle.hpp"
+
+#include <memory>
+#include <string>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+struct orc_ctx {
+    int precision;
+    std::unique_ptr<orc::Solver<double>> d;
+    std::unique_ptr<orc::Solver<long double>> ld;
+};
+
+static thread_local std::string g_err;
+
+template <class F> static int guarded(F&& f) {
+    try { f(); return 0; }
+    catch (const std::exception& e) { g_err = e.what(); return -1; }
+    catch (...) { g_err = "unknown exception"; return -1; }
+}
+
+#define DISPATCH(c, expr) do { if ((c)->precision == 0) { auto& S = *(c)->d; expr; } else { auto& S = *(c)->ld; expr; } } while (0)
+
+template <class T> static void rhs_out(orc::Solver<T>& S, double* const out[8], double* phi, double* dsc) {
+    if (!S.have_fields) throw std::runtime_error("no fields set");
+    orc::rfield<T> R[8];
+    S.rhs(S.U, R, phi, dsc);
+    for (int c = 0; c < 8; ++c)
+        for (std::int64_t i = 0; i < S.N3; ++i) out[c][i] = double(R[c][i]);
+}
+
+template <class T> static void apply_out(orc::Solver<T>& S, int op, const double* in, double* out) {
+    orc::rfield<T> f(S.N3), o;
+    for (std::int64_t i = 0; i < S.N3; ++i) f[i] = T(in[i]);
+    S.apply(f, op, o);
+    for (std::int64_t i = 0; i < S.N3; ++i) out[i] = double(o[i]);
+}
+
+template <class T> static void transform(int N, int sign, bool direct, const double* in, double* out) {
+    const std::int64_t N3 = std::int64_t(N) * N * N;
+    orc::cfield<T> a(N3), o;
+    for (std::int64_t i = 0; i < N3; ++i) a[i] = orc::cplx<T>(T(in[2 * i]), T(in[2 * i + 1]));
+    if (direct) { orc::dft3_direct(a, o, N, sign); a.swap(o); } else orc::fft3(a, N, sign);
+    for (std::int64_t i = 0; i < N3; ++i) { out[2 * i] = double(a[i].real()); out[2 * i + 1] = double(a[i].imag()); }
+}
+
+extern "C" {
+
+int orc_create(orc_ctx** out, int N, double L, double gamma, double mu, double eta, double dt, int precision) {
+    return guarded([&] {
+        if (!out) throw std::invalid_argument("null out");
+        if (!(L > 0) || !(gamma > 1) || mu < 0 || eta < 0 || !(dt > 0)) throw std::invalid_argument("bad parameter");
+        auto c = std::make_unique<orc_ctx>();
+        c->precision = precision ? 1 : 0;
+        if (c->precision == 0) c->d = std::make_unique<orc::Solver<double>>(N, L, gamma, mu, eta, dt);
+        else c->ld = std::make_unique<orc::Solver<long double>>(N, L, gamma, mu, eta, dt);
+        *out = c.release();
+    });
+}
+
+int orc_destroy(orc_ctx* c) { delete c; return 0; }
+const char* orc_last_error(void) { return g_err.c_str(); }
+
+void orc_set_threads(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+int orc_get_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+int orc_use_direct_dft(orc_ctx* c, int on) { return guarded([&] { DISPATCH(c, S.use_direct_dft = (on != 0)); }); }
+
+int orc_set_fields(orc_ctx* c, int kind, const double* const f[8]) {
+    return guarded([&] { if (kind != 0 && kind != 1) throw std::invalid_argument("kind"); DISPATCH(c, S.set_fields(kind, f)); });
+}
+int orc_get_fields(orc_ctx* c, int kind, double* const out[8]) {
+    return guarded([&] { if (kind != 0 && kind != 1) throw std::invalid_argument("kind"); DISPATCH(c, S.get_fields(kind, out)); });
+}
+int orc_rhs(orc_ctx* c, double* const out[8]) { return guarded([&] { DISPATCH(c, rhs_out(S, out, nullptr, nullptr)); }); }
+int orc_rhs_scales(orc_ctx* c, double* const out[8], double phi[8], double dsc[8]) {
+    return guarded([&] { DISPATCH(c, rhs_out(S, out, phi, dsc)); });
+}
+int orc_step(orc_ctx* c, int nsteps) {
+    return guarded([&] { DISPATCH(c, { if (!S.have_fields) throw std::runtime_error("no fields set"); S.step(nsteps); }); });
+}
+int orc_nspec(orc_ctx* c) { int n = 0; DISPATCH(c, n = S.nspec()); return n; }
+int orc_diagnostics(orc_ctx* c, orc_diag* d, double* spec_kin, double* spec_mag, int nspec) {
+    return guarded([&] {
+        DISPATCH(c, {
+            if (!S.have_fields) throw std::runtime_error("no fields set");
+            if ((spec_kin || spec_mag) && nspec != S.nspec()) throw std::invalid_argument("nspec");
+            orc::Diag g;
+            S.diagnostics(g, spec_kin, spec_mag);
+            d->t = g.t; d->step = g.step; d->ke = g.ke; d->me = g.me; d->ie = g.ie; d->mass = g.mass;
+            for (int k = 0; k < 3; ++k) d->mom[k] = g.mom[k];
+            d->etot = g.etot; d->max_divb = g.max_divb; d->rho_min = g.rho_min; d->p_min = g.p_min;
+        });
+    });
+}
+int orc_apply(orc_ctx* c, int op, const double* in, double* out) {
+    return guarded([&] { if (op < 0 || op > 4) throw std::invalid_argument("op"); DISPATCH(c, apply_out(S, op, in, out)); });
+}
+int orc_fft3(int N, int sign, int precision, const double* in, double* out) {
+    return guarded([&] { if (precision) transform<long double>(N, sign, false, in, out); else transform<double>(N, sign, false, in, out); });
+}
+int orc_dft3_direct(int N, int sign, int precision, const double* in, double* out) {
+    return guarded([&] { if (precision) transform<long double>(N, sign, true, in, out); else transform<double>(N, sign, true, in, out); });
+}
+
+}  // extern "C"
