@@ -1,0 +1,140 @@
+/* include/mhd.h — C ABI of libmhd: the B200-native (sm_100a) hot path of the pseudo-spectral compressible
+ * MHD solver of arXiv 1810.12707 ("G-MHD3D").
+ *
+ * What the library computes (citations: PAPER.md = the paper text; DESIGN.md = this repo's readings R1-R10):
+ *   the right-hand side and explicit Adams-Bashforth step of the 3-D compressible, viscous, resistive MHD
+ *   equations on a triply periodic N^3 box of side L (Sec. V Eq. 17-19; energy equation
+ *   Eq. 12, in normalised units), discretised pseudo-spectrally: 3-D real FFTs, derivatives by
+ *   multiplication with i*k, 2/3-rule dealiasing (L27; R5), real-space flux
+ *   products, mu*lap(u) and eta*lap(B) diffusion, all in fp64 (Table I).
+ *
+ * Conventions
+ *   - every field array is N^3 doubles laid out [z][y][x], x fastest, x_i = i*L/N (plan (Nz,Ny,Nx));
+ *   - field order, conservative (kind 0): rho, mx, my, mz, E, Bx, By, Bz   with m = rho*u and
+ *     E = P/(gamma-1) + rho|u|^2/2 + |B|^2/2 (1/8pi -> 1/2);
+ *     primitive (kind 1): rho, ux, uy, uz, P, Bx, By, Bz;
+ *   - `where` says what the caller's pointers are: MHD_HOST (0) = host memory (pageable or pinned),
+ *     MHD_DEVICE (1) = device memory of the current CUDA device;
+ *   - ownership: the caller owns every buffer it passes; the library copies in / out and never frees them.
+ *     The context owns only small host metadata; all device storage lives inside the workspace handed to
+ *     mhd_bind(), which the caller allocates (e.g. with torch) and must keep alive until mhd_destroy();
+ *   - ordering: every call enqueues its work on the stream given to mhd_bind(); calls that return data to
+ *     host memory (where = MHD_HOST, mhd_diagnostics) synchronise that stream before returning, calls with
+ *     device pointers return as soon as the work is enqueued;
+ *   - errors: every function returns MHD_OK (0) or a negative code and never throws, aborts or prints;
+ *     mhd_last_error() returns a description of the last failure on that context;
+ *   - threads: one context per host thread; contexts are independent.
+ *   There is no CPU fallback: without a CUDA device every compute entry point returns MHD_ERR_CUDA.
+ */
+#ifndef MHD_H
+#define MHD_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MHD_OK 0
+#define MHD_ERR_INVALID_ARG (-1)
+#define MHD_ERR_NOT_BOUND (-2)
+#define MHD_ERR_NO_FIELDS (-3)
+#define MHD_ERR_CUDA (-4)
+#define MHD_ERR_NOMEM (-5)
+
+#define MHD_HOST 0
+#define MHD_DEVICE 1
+
+#define MHD_CONSERVATIVE 0
+#define MHD_PRIMITIVE 1
+
+/* workspace flags */
+#define MHD_FLAG_DEFAULT 0u
+#define MHD_FLAG_OUT_OF_CORE 1u /* field storage in pinned host memory, slabs streamed (Sec. VII-C) */
+
+/* options for mhd_set_option() */
+#define MHD_OPT_FUSED 1      /* 1 (default): fused kernels; 0: one kernel per step of the path (debug/bisect)  */
+#define MHD_OPT_PRUNE 2      /* 1 (default): skip pencils the 2/3 mask makes identically zero; 0: full sweeps  */
+#define MHD_OPT_INTEGRATOR 3 /* 0 (default): Adams-Bashforth 2 with Euler start; 1: RK4; 2: predictor-corrector
+                                (Table I; R6)                                 */
+
+typedef struct mhd_ctx mhd_ctx; /* opaque, owned by the library */
+
+/* Diagnostics record ("per grid" = volume means; L71 Eq. 9; R8). */
+typedef struct {
+    double t;          /* time = step * dt                                                     */
+    long long step;    /* steps taken since the last mhd_set_fields                            */
+    double ke;         /* <rho |u|^2 / 2>                                                      */
+    double me;         /* <|B|^2 / 2>                                                          */
+    double ie;         /* <P> / (gamma - 1)                                                    */
+    double mass;       /* <rho>                                                                */
+    double mom[3];     /* <m>                                                                  */
+    double etot;       /* <E>                                                                  */
+    double max_divb;   /* max over grid points of |d~x Bx + d~y By + d~z Bz| (dealiased spectral derivative) */
+    double rho_min;    /* min rho                                                              */
+    double p_min;      /* min P                                                                */
+} mhd_diag;
+
+/* Create a context.  N: power of two, 16 <= N <= 1024; L > 0; gamma > 1; mu, eta >= 0; dt > 0.
+ * (mu, eta are the normalised 1/Re, 1/Rm of PAPER.md L140-152.)  Does not touch the GPU. */
+int mhd_init(mhd_ctx **out, int N, double L, double gamma, double mu, double eta, double dt);
+
+/* Device bytes the caller must provide to mhd_bind() for grid size N and the given flags. */
+size_t mhd_workspace_bytes(int N, unsigned flags);
+/* Pinned host bytes needed by the out-of-core path (0 for the in-core path). */
+size_t mhd_pinned_bytes(int N, unsigned flags);
+
+/* Attach storage.  dev_workspace: device pointer, 256-byte aligned, >= mhd_workspace_bytes(N, flags);
+ * cuda_stream: a cudaStream_t (NULL = legacy default stream); pinned_host/pinned_bytes: page-locked host
+ * memory for the out-of-core path (NULL/0 otherwise).  Builds the twiddle tables (device work). */
+int mhd_bind(mhd_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream, unsigned flags,
+             void *pinned_host, size_t pinned_bytes);
+
+int mhd_set_option(mhd_ctx *ctx, int option, int value);
+
+/* Load a state.  f[i]: N^3 doubles each.  Primitive input is converted point-wise to conservative; each of the
+ * 8 conservative fields is then dealias-projected, U <- IFFT(M FFT U) (R5).  Resets t = 0, step = 0
+ * and the Adams-Bashforth history (the next step is a forward-Euler step, R6). */
+int mhd_set_fields(mhd_ctx *ctx, int kind, int where, const double *const f[8]);
+
+/* dU/dt of the current state in real space, 8 x N^3 doubles, conservative order.  Does not change the state,
+ * the time or the integrator history. */
+int mhd_rhs(mhd_ctx *ctx, int where, double *const out[8]);
+
+/* Advance nsteps explicit steps of size dt.  mhd_step(a); mhd_step(b) is identical to mhd_step(a+b).
+ * Only kernel launches; no host round trip. */
+int mhd_step(mhd_ctx *ctx, int nsteps);
+
+/* Current state in real space (kind as in mhd_set_fields). */
+int mhd_get_fields(mhd_ctx *ctx, int kind, int where, double *const out[8]);
+
+/* Diagnostics of the current state.  spec_kin / spec_mag (host pointers, may be NULL): shell spectra of
+ * sqrt(rho)*u and of B, S(K) = sum over the full mode cube with floor(|n|+1/2) = K of 1/2 |w^(n)|^2 / N^6,
+ * K = 0 .. nspec-1, nspec must equal mhd_nspec(N) = ceil(sqrt(3) N / 2) + 1; sum_K S(K) = ke resp. me. */
+int mhd_diagnostics(mhd_ctx *ctx, mhd_diag *d, double *spec_kin, double *spec_mag, int nspec);
+int mhd_nspec(int N);
+
+/* Stand-alone batched 3-D real FFT on DEVICE buffers (the FFT metric of BASELINE.json).
+ *   r2c: real[i] (N^3 doubles) -> spec[i]: N*N*(N/2) complex doubles [kz][ky][kx], kx = 0..N/2-1, unnormalised
+ *        forward transform F(n) = sum_x f(x) exp(-i k.x); the Nyquist column kx = N/2 goes to nyq[i]
+ *        (N*N*8 complex, column 0 of each 8-wide row holds the value; may be NULL to drop it).
+ *   c2r: the inverse with 1/N^3, Nyquist column taken as zero.  spec is destroyed (used as scratch).
+ * prune != 0 restricts both to modes inside the 2/3 mask (others are not written / are read as zero). */
+int mhd_fft3d_r2c(mhd_ctx *ctx, int nfields, const double *const real[], double *const spec[],
+                  double *const nyq[], int prune);
+int mhd_fft3d_c2r(mhd_ctx *ctx, int nfields, double *const spec[], double *const real[], int prune);
+
+/* Number of kernels this context has launched so far (for the bench's gpu_launches claim). */
+long long mhd_launch_count(const mhd_ctx *ctx);
+/* Milliseconds and launches accumulated per kernel family since the last reset; names[i] are static strings.
+ * Timing uses CUDA events on the bound stream and is only collected while enabled (adds synchronisation). */
+int mhd_profile_enable(mhd_ctx *ctx, int on);
+int mhd_profile_get(mhd_ctx *ctx, int max_entries, const char **names, double *ms, long long *launches);
+
+const char *mhd_last_error(const mhd_ctx *ctx);
+int mhd_destroy(mhd_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MHD_H */

@@ -1,0 +1,219 @@
+"""Thin ctypes binding of libmhd.so (include/mhd.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of `csrc/`; this module only loads the shared library,
+declares the C signatures under the same names, and offers `MHD`, a convenience class that lets torch own
+the device workspace and the stream (plumbing, not arithmetic).  There is no CPU fallback: if the library
+is missing or no CUDA device is present, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import math
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmhd.so")
+
+MHD_OK = 0
+MHD_HOST, MHD_DEVICE = 0, 1
+MHD_CONSERVATIVE, MHD_PRIMITIVE = 0, 1
+MHD_OPT_FUSED, MHD_OPT_PRUNE, MHD_OPT_INTEGRATOR = 1, 2, 3
+ERRORS = {-1: "MHD_ERR_INVALID_ARG", -2: "MHD_ERR_NOT_BOUND", -3: "MHD_ERR_NO_FIELDS", -4: "MHD_ERR_CUDA",
+          -5: "MHD_ERR_NOMEM"}
+
+# every symbol include/mhd.h declares (checked by tests/test_abi.py)
+SYMBOLS = ["mhd_init", "mhd_workspace_bytes", "mhd_pinned_bytes", "mhd_bind", "mhd_set_option", "mhd_set_fields",
+           "mhd_rhs", "mhd_step", "mhd_get_fields", "mhd_diagnostics", "mhd_nspec", "mhd_fft3d_r2c",
+           "mhd_fft3d_c2r", "mhd_launch_count", "mhd_profile_enable", "mhd_profile_get", "mhd_last_error",
+           "mhd_destroy"]
+
+
+class MhdDiag(C.Structure):
+    _fields_ = [("t", C.c_double), ("step", C.c_longlong), ("ke", C.c_double), ("me", C.c_double),
+                ("ie", C.c_double), ("mass", C.c_double), ("mom", C.c_double * 3), ("etot", C.c_double),
+                ("max_divb", C.c_double), ("rho_min", C.c_double), ("p_min", C.c_double)]
+
+
+_lib = None
+
+
+def lib():
+    """Load libmhd.so (fails loudly if it has not been built: there is no fallback path)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError("libmhd.so is missing (%s): run `python -m paper_1810_12707_b200.build` "
+                           "(or __graft_entry__.build()); the product path has no CPU fallback" % LIB_PATH)
+    L = C.CDLL(LIB_PATH)
+    P8 = C.POINTER(C.c_void_p)
+    L.mhd_init.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, C.c_double]
+    L.mhd_workspace_bytes.argtypes = [C.c_int, C.c_uint]
+    L.mhd_workspace_bytes.restype = C.c_size_t
+    L.mhd_pinned_bytes.argtypes = [C.c_int, C.c_uint]
+    L.mhd_pinned_bytes.restype = C.c_size_t
+    L.mhd_bind.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p, C.c_uint, C.c_void_p, C.c_size_t]
+    L.mhd_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int]
+    L.mhd_set_fields.argtypes = [C.c_void_p, C.c_int, C.c_int, P8]
+    L.mhd_rhs.argtypes = [C.c_void_p, C.c_int, P8]
+    L.mhd_step.argtypes = [C.c_void_p, C.c_int]
+    L.mhd_get_fields.argtypes = [C.c_void_p, C.c_int, C.c_int, P8]
+    L.mhd_diagnostics.argtypes = [C.c_void_p, C.POINTER(MhdDiag), C.c_void_p, C.c_void_p, C.c_int]
+    L.mhd_nspec.argtypes = [C.c_int]
+    L.mhd_fft3d_r2c.argtypes = [C.c_void_p, C.c_int, P8, P8, P8, C.c_int]
+    L.mhd_fft3d_c2r.argtypes = [C.c_void_p, C.c_int, P8, P8, C.c_int]
+    L.mhd_launch_count.argtypes = [C.c_void_p]
+    L.mhd_launch_count.restype = C.c_longlong
+    L.mhd_profile_enable.argtypes = [C.c_void_p, C.c_int]
+    L.mhd_profile_get.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_char_p), C.POINTER(C.c_double),
+                                  C.POINTER(C.c_longlong)]
+    L.mhd_last_error.argtypes = [C.c_void_p]
+    L.mhd_last_error.restype = C.c_char_p
+    L.mhd_destroy.argtypes = [C.c_void_p]
+    _lib = L
+    return L
+
+
+def _ptr_array(ptrs):
+    a = (C.c_void_p * len(ptrs))()
+    for i, p in enumerate(ptrs):
+        a[i] = p
+    return a
+
+
+class MHD:
+    """One solver context on the current CUDA device; torch owns the workspace and the stream."""
+
+    def __init__(self, N, L=2 * math.pi, gamma=5.0 / 3.0, mu=0.0, eta=0.0, dt=1e-3, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: the product path has no CPU fallback")
+        self._L = lib()
+        self.N = int(N)
+        self.torch = torch
+        self.device = torch.device(device)
+        self._h = C.c_void_p()
+        rc = self._L.mhd_init(C.byref(self._h), self.N, L, gamma, mu, eta, dt)
+        if rc != MHD_OK:
+            raise ValueError("mhd_init: %s" % ERRORS.get(rc, rc))
+        nbytes = int(self._L.mhd_workspace_bytes(self.N, 0))
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = self.workspace.data_ptr()
+            self._base = (base + 255) // 256 * 256
+            self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            self._check(self._L.mhd_bind(self._h, self._base, nbytes, self.stream.cuda_stream, 0, None, 0))
+
+    # -- helpers ----------------------------------------------------------------------------------------
+    def _check(self, rc):
+        if rc != MHD_OK:
+            raise RuntimeError("libmhd: %s: %s" % (ERRORS.get(rc, rc), self._L.mhd_last_error(self._h).decode()))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.mhd_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _marshal(self, fields):
+        """-> (where, pointer array, keep-alive list) for 8 numpy (host) or torch cuda (device) arrays."""
+        torch = self.torch
+        n3 = self.N ** 3
+        if all(isinstance(f, np.ndarray) for f in fields):
+            keep = [np.ascontiguousarray(f, dtype=np.float64) for f in fields]
+            assert all(k.size == n3 for k in keep)
+            return MHD_HOST, _ptr_array([k.ctypes.data for k in keep]), keep
+        assert all(isinstance(f, torch.Tensor) for f in fields)
+        keep = [f.contiguous() for f in fields]
+        assert all(k.dtype == torch.float64 and k.numel() == n3 for k in keep)
+        if all(k.is_cuda for k in keep):
+            return MHD_DEVICE, _ptr_array([k.data_ptr() for k in keep]), keep
+        assert all(not k.is_cuda for k in keep)      # host tensors (e.g. pinned)
+        return MHD_HOST, _ptr_array([k.data_ptr() for k in keep]), keep
+
+    def _new_out(self, where, out):
+        torch = self.torch
+        shape = (self.N,) * 3
+        if out is not None:
+            return self._marshal(out)[1], out
+        if where == MHD_HOST:
+            arrs = [np.empty(shape, dtype=np.float64) for _ in range(8)]
+            return _ptr_array([a.ctypes.data for a in arrs]), arrs
+        arrs = [torch.empty(shape, dtype=torch.float64, device=self.device) for _ in range(8)]
+        return _ptr_array([a.data_ptr() for a in arrs]), arrs
+
+    # -- the ABI calls ------------------------------------------------------------------------------------
+    def set_option(self, option, value):
+        self._check(self._L.mhd_set_option(self._h, int(option), int(value)))
+
+    def set_fields(self, fields, kind="primitive"):
+        where, ptrs, keep = self._marshal(fields)
+        self._check(self._L.mhd_set_fields(self._h, MHD_PRIMITIVE if kind == "primitive" else MHD_CONSERVATIVE, where, ptrs))
+
+    def rhs(self, where="host", out=None):
+        w = MHD_HOST if where == "host" else MHD_DEVICE
+        ptrs, arrs = self._new_out(w, out)
+        self._check(self._L.mhd_rhs(self._h, w, ptrs))
+        return arrs
+
+    def step(self, n=1):
+        self._check(self._L.mhd_step(self._h, int(n)))
+
+    def get_fields(self, kind="conservative", where="host", out=None):
+        w = MHD_HOST if where == "host" else MHD_DEVICE
+        ptrs, arrs = self._new_out(w, out)
+        self._check(self._L.mhd_get_fields(self._h, MHD_PRIMITIVE if kind == "primitive" else MHD_CONSERVATIVE, w, ptrs))
+        return arrs
+
+    def nspec(self):
+        return int(self._L.mhd_nspec(self.N))
+
+    def diagnostics(self, spectra=False):
+        d = MhdDiag()
+        if spectra:
+            ns = self.nspec()
+            sk, sm = np.zeros(ns), np.zeros(ns)
+            self._check(self._L.mhd_diagnostics(self._h, C.byref(d), sk.ctypes.data, sm.ctypes.data, ns))
+        else:
+            sk = sm = None
+            self._check(self._L.mhd_diagnostics(self._h, C.byref(d), None, None, 0))
+        out = {k: getattr(d, k) for k in ("t", "step", "ke", "me", "ie", "mass", "etot", "max_divb", "rho_min", "p_min")}
+        out["mom"] = [d.mom[0], d.mom[1], d.mom[2]]
+        if spectra:
+            out["spec_kin"], out["spec_mag"] = sk, sm
+        return out
+
+    def fft3d_r2c(self, real, spec, nyq=None, prune=False):
+        """real/spec/nyq: lists of torch cuda float64 tensors (N^3 / N*N*(N/2)*2 / N*N*8*2 doubles)."""
+        n = len(real)
+        r = _ptr_array([t.data_ptr() for t in real])
+        s = _ptr_array([t.data_ptr() for t in spec])
+        q = _ptr_array([t.data_ptr() for t in nyq]) if nyq is not None else None
+        self._check(self._L.mhd_fft3d_r2c(self._h, n, r, s, q, int(prune)))
+
+    def fft3d_c2r(self, spec, real, prune=False):
+        n = len(real)
+        r = _ptr_array([t.data_ptr() for t in real])
+        s = _ptr_array([t.data_ptr() for t in spec])
+        self._check(self._L.mhd_fft3d_c2r(self._h, n, s, r, int(prune)))
+
+    def launch_count(self):
+        return int(self._L.mhd_launch_count(self._h))
+
+    def profile_enable(self, on=True):
+        self._check(self._L.mhd_profile_enable(self._h, int(on)))
+
+    def profile_get(self):
+        n = 32
+        names = (C.c_char_p * n)()
+        ms = (C.c_double * n)()
+        cnt = (C.c_longlong * n)()
+        k = self._L.mhd_profile_get(self._h, n, names, ms, cnt)
+        return {names[i].decode(): {"ms": ms[i], "launches": int(cnt[i])} for i in range(k)}

@@ -1,0 +1,179 @@
+// fft_core.cuh — register-resident fp64 Stockham FFT engine for sm_100a (device templates only).
+//
+// One "line" of NL complex points is transformed by T = NL/E threads, each holding E points in registers
+// (v[m] <-> element t + T*m, the same ownership at entry and exit, so the first stage reads straight from
+// global memory and the last stage writes straight to it).  Between stages the points are exchanged through
+// a shared-memory tile whose fastest index is the line ("column"): 8 lanes with 8 different lines touch one
+// 128-byte row, so every access pattern of the autosort exchange is bank-conflict free by construction.
+// Stage s with radix R performs E/R butterflies per thread:
+//     j = t + b*T,  k = j mod Ns,  u[r] = in[j + r*NL/R] * w^(r*k*NL/(Ns*R)),  u = DFT_R(u),
+//     out[(j-k)*R + k + q*Ns] = u[q]                        (Ns = product of the radices already applied)
+// which is the Stockham autosort formulation: natural order in, natural order out, no bit reversal.
+// Twiddles come from an exactly rounded table w[m] = exp(-2*pi*i*m/NT) built once with sincospi (no
+// recurrences: the fp64 error bound of the transform depends on it).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace mhd {
+
+typedef double2 cd;
+
+__device__ __forceinline__ cd mk(double x, double y) { return make_double2(x, y); }
+__device__ __forceinline__ cd operator+(cd a, cd b) { return mk(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ cd operator-(cd a, cd b) { return mk(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ cd operator*(double s, cd a) { return mk(s * a.x, s * a.y); }
+__device__ __forceinline__ cd cconj(cd a) { return mk(a.x, -a.y); }
+__device__ __forceinline__ cd cmul(cd a, cd b) { return mk(fma(a.x, b.x, -(a.y * b.y)), fma(a.x, b.y, a.y * b.x)); }
+// a * w for the forward transform (DIR < 0), a * conj(w) for the inverse (DIR > 0); w = forward table entry
+template <int DIR> __device__ __forceinline__ cd twmul(cd a, cd w) {
+    if (DIR < 0) return mk(fma(a.x, w.x, -(a.y * w.y)), fma(a.x, w.y, a.y * w.x));
+    return mk(fma(a.x, w.x, a.y * w.y), fma(a.y, w.x, -(a.x * w.y)));
+}
+// a * (-i) forward, a * (+i) inverse
+template <int DIR> __device__ __forceinline__ cd mul_mi(cd a) {
+    if (DIR < 0) return mk(a.y, -a.x);
+    return mk(-a.y, a.x);
+}
+
+// a * exp(DIR * 2*pi*i * K/R), 0 <= K < R/2, R in {2,4,8,16}: constants of the in-register butterflies
+template <int R, int K, int DIR> __device__ __forceinline__ cd mul_root(cd a) {
+    constexpr int K16 = K * (16 / R);
+    constexpr double SQH = 0.70710678118654752440;   // sqrt(1/2)
+    constexpr double C8 = 0.92387953251128675613;    // cos(pi/8)
+    constexpr double S8 = 0.38268343236508977173;    // sin(pi/8)
+    constexpr double sg = (DIR < 0) ? -1.0 : 1.0;    // sign of the imaginary part of the root
+    if constexpr (K16 == 0) return a;
+    else if constexpr (K16 == 4) return mul_mi<DIR>(a);
+    else if constexpr (K16 == 2) return mk(SQH * (a.x - sg * a.y), SQH * (a.y + sg * a.x));
+    else if constexpr (K16 == 6) return mk(-SQH * (a.x + sg * a.y), SQH * (sg * a.x - a.y));
+    else {
+        constexpr double wr = (K16 == 1) ? C8 : (K16 == 3) ? S8 : (K16 == 5) ? -S8 : -C8;
+        constexpr double wi = sg * ((K16 == 1 || K16 == 7) ? S8 : C8);
+        return mk(fma(a.x, wr, -(a.y * wi)), fma(a.x, wi, a.y * wr));
+    }
+}
+
+// In-register DFT of R points, natural order in and out:  v[q] <- sum_r v[r] exp(DIR*2*pi*i*r*q/R)
+template <int R, int DIR> struct Dft;
+template <int DIR> struct Dft<1, DIR> {
+    __device__ __forceinline__ static void run(cd*) {}
+};
+template <int DIR> struct Dft<2, DIR> {
+    __device__ __forceinline__ static void run(cd* v) {
+        const cd a = v[0], b = v[1];
+        v[0] = a + b; v[1] = a - b;
+    }
+};
+template <int DIR> struct Dft<4, DIR> {
+    __device__ __forceinline__ static void run(cd* v) {
+        const cd a0 = v[0] + v[2], a1 = v[0] - v[2], a2 = v[1] + v[3], a3 = mul_mi<DIR>(v[1] - v[3]);
+        v[0] = a0 + a2; v[2] = a0 - a2; v[1] = a1 + a3; v[3] = a1 - a3;
+    }
+};
+template <int R, int K, int DIR> struct Combine {   // v[k] = e[k] + W^k o[k], v[k+R/2] = e[k] - W^k o[k]
+    __device__ __forceinline__ static void run(cd* v, const cd* e, const cd* o) {
+        const cd t = mul_root<R, K, DIR>(o[K]);
+        v[K] = e[K] + t; v[K + R / 2] = e[K] - t;
+        if constexpr (K + 1 < R / 2) Combine<R, K + 1, DIR>::run(v, e, o);
+    }
+};
+template <int R, int DIR> struct Dft {
+    __device__ __forceinline__ static void run(cd* v) {
+        cd e[R / 2], o[R / 2];
+#pragma unroll
+        for (int i = 0; i < R / 2; ++i) { e[i] = v[2 * i]; o[i] = v[2 * i + 1]; }
+        Dft<R / 2, DIR>::run(e);
+        Dft<R / 2, DIR>::run(o);
+        Combine<R, 0, DIR>::run(v, e, o);
+    }
+};
+
+// ---------------------------------------------------------------------------------------------------
+// line plans: radices per stage and points per thread
+// ---------------------------------------------------------------------------------------------------
+template <int NL> struct Plan;
+template <> struct Plan<4>    { static constexpr int NS = 1, R0 = 4,  R1 = 1,  R2 = 1, E = 4;  };
+template <> struct Plan<8>    { static constexpr int NS = 1, R0 = 8,  R1 = 1,  R2 = 1, E = 8;  };
+template <> struct Plan<16>   { static constexpr int NS = 2, R0 = 4,  R1 = 4,  R2 = 1, E = 4;  };
+template <> struct Plan<32>   { static constexpr int NS = 2, R0 = 8,  R1 = 4,  R2 = 1, E = 8;  };
+template <> struct Plan<64>   { static constexpr int NS = 2, R0 = 8,  R1 = 8,  R2 = 1, E = 8;  };
+template <> struct Plan<128>  { static constexpr int NS = 2, R0 = 16, R1 = 8,  R2 = 1, E = 16; };
+template <> struct Plan<256>  { static constexpr int NS = 2, R0 = 16, R1 = 16, R2 = 1, E = 16; };
+template <> struct Plan<512>  { static constexpr int NS = 3, R0 = 8,  R1 = 8,  R2 = 8, E = 16; };
+template <> struct Plan<1024> { static constexpr int NS = 3, R0 = 16, R1 = 8,  R2 = 8, E = 16; };
+
+template <int NL> struct PlanInfo {
+    typedef Plan<NL> P;
+    static constexpr int E = P::E;
+    static constexpr int T = NL / E;    // threads per line
+};
+
+// shared-memory tile layouts: element index of (row n, this thread's line)
+struct LayoutPlain {        // tile[n][C], thread's column c fixed
+    int C, c;
+    __device__ __forceinline__ int operator()(int n) const { return n * C + c; }
+};
+struct LayoutSwz {          // tile[n][SL] with the low 3 slot bits XOR-swizzled by the row (SL >= 8)
+    int SL, slot;
+    __device__ __forceinline__ int operator()(int n) const { return n * SL + (slot ^ (n & 7)); }
+};
+
+// one stage: butterflies on registers; non-final stages scatter to shared memory and gather back
+template <int NL, int R, int NSTRIDE /*Ns*/, bool LAST, bool FIRST, int DIR, int TWS, class Layout>
+__device__ __forceinline__ void fft_stage(cd (&v)[PlanInfo<NL>::E], int t, const cd* __restrict__ tw, cd* sm,
+                                          const Layout& L) {
+    constexpr int E = PlanInfo<NL>::E, T = PlanInfo<NL>::T, B = E / R;
+    static_assert(E % R == 0, "radix must divide the points per thread");
+    if constexpr (!LAST && !FIRST) __syncthreads();   // every thread has gathered the previous exchange
+#pragma unroll
+    for (int b = 0; b < B; ++b) {
+        const int j = t + b * T;
+        const int k = j & (NSTRIDE - 1);
+        cd u[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) u[r] = v[b + r * B];
+        if constexpr (NSTRIDE > 1) {
+#pragma unroll
+            for (int r = 1; r < R; ++r) {
+                const cd w = __ldg(&tw[(r * k * (NL / (NSTRIDE * R))) * TWS]);
+                u[r] = twmul<DIR>(u[r], w);
+            }
+        }
+        Dft<R, DIR>::run(u);
+        if constexpr (LAST) {
+#pragma unroll
+            for (int q = 0; q < R; ++q) v[b + q * B] = u[q];
+        } else {
+            const int j0 = (j - k) * R + k;
+#pragma unroll
+            for (int q = 0; q < R; ++q) sm[L(j0 + q * NSTRIDE)] = u[q];
+        }
+    }
+    if constexpr (!LAST) {
+        __syncthreads();
+#pragma unroll
+        for (int m = 0; m < E; ++m) v[m] = sm[L(t + T * m)];
+    }
+}
+
+// Whole line transform on registers.  On entry v[m] = x[t + T*m]; on exit v[m] = X[t + T*m] with
+// X[q] = sum_n x[n] exp(DIR*2*pi*i*n*q/NL) (unnormalised).  `sm` is the exchange tile (must be free on entry;
+// all threads of the block must call).  tw[m*TWS] = exp(-2*pi*i*m/NL).
+template <int NL, int DIR, int TWS, class Layout>
+__device__ __forceinline__ void fft_line(cd (&v)[PlanInfo<NL>::E], int t, const cd* __restrict__ tw, cd* sm,
+                                         const Layout& L) {
+    typedef Plan<NL> P;
+    if constexpr (P::NS == 1) {
+        fft_stage<NL, P::R0, 1, true, true, DIR, TWS>(v, t, tw, sm, L);
+    } else if constexpr (P::NS == 2) {
+        fft_stage<NL, P::R0, 1, false, true, DIR, TWS>(v, t, tw, sm, L);
+        fft_stage<NL, P::R1, P::R0, true, false, DIR, TWS>(v, t, tw, sm, L);
+    } else {
+        fft_stage<NL, P::R0, 1, false, true, DIR, TWS>(v, t, tw, sm, L);
+        fft_stage<NL, P::R1, P::R0, false, false, DIR, TWS>(v, t, tw, sm, L);
+        fft_stage<NL, P::R2, P::R0 * P::R1, true, false, DIR, TWS>(v, t, tw, sm, L);
+    }
+}
+
+}  // namespace mhd

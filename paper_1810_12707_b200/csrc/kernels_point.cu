@@ -1,0 +1,398 @@
+// kernels_point.cu — point-wise kernels in k-space and real space, reductions for the diagnostics, twiddles.
+//
+// k-space kernels run over the half-spectrum arrays [kz][ky][kx] (row pitch hx = N/2 complex; the Nyquist
+// column is not stored).  In pruned mode only the modes inside the 2/3 mask are visited — (2kc+1)^2 (kc+1) of
+// N^2 N/2, i.e. 30 % — everything outside is identically zero by construction and is never read.
+#include "fft_core.cuh"
+#include "kernels.h"
+#include "physics.cuh"
+
+namespace mhd {
+
+// ---- mode geometry -----------------------------------------------------------------------------------------
+struct ModeIt {
+    int ix, iy, iz;          // array indices
+    int nx, ny, nz;          // integer modes
+    bool inside;             // inside the 2/3 mask
+    long long idx;           // linear index
+};
+// grid: x over kx (blockDim.x threads), y over the (possibly pruned) ky count, z over the kz count
+__device__ __forceinline__ bool mode_of_thread(const SpecGeom& g, ModeIt& m) {
+    const int N = g.N, kc = g.kc;
+    m.ix = blockIdx.x * blockDim.x + threadIdx.x;
+    int oy = blockIdx.y, oz = blockIdx.z;
+    if (g.pruned) {
+        if (m.ix > kc) return false;
+        m.iy = oy <= kc ? oy : N - (2 * kc + 1) + oy;
+        m.iz = oz <= kc ? oz : N - (2 * kc + 1) + oz;
+    } else {
+        if (m.ix >= g.hx) return false;
+        m.iy = oy; m.iz = oz;
+    }
+    m.nx = m.ix;
+    m.ny = m.iy <= N / 2 ? m.iy : m.iy - N;
+    m.nz = m.iz <= N / 2 ? m.iz : m.iz - N;
+    m.inside = m.nx <= kc && abs(m.ny) <= kc && abs(m.nz) <= kc;
+    m.idx = ((long long)m.iz * N + m.iy) * g.hx + m.ix;
+    return true;
+}
+static dim3 mode_grid(const SpecGeom& g, int threads) {
+    const int nxv = g.pruned ? g.kc + 1 : g.hx;
+    const int nyv = g.pruned ? 2 * g.kc + 1 : g.N;
+    return dim3((nxv + threads - 1) / threads, nyv, nyv);
+}
+constexpr int KT = 64;   // threads along kx for the k-space kernels
+
+struct Ptr3 { const cd* p[3]; };
+struct PtrW3 { cd* p[3]; };
+struct Ptr8 { cd* p[8]; };
+struct PtrC16 { const cd* p[16]; };
+struct PtrN { cd* p[MAXF]; };
+struct PtrCN { const cd* p[MAXF]; };
+
+// ---- J^ = M i k x B^ -----------------------------------------------------------------------------------
+__global__ void build_current_kernel(SpecGeom g, Ptr3 B, PtrW3 J, Phys ph) {
+    ModeIt m;
+    if (!mode_of_thread(g, m)) return;
+    cd jx = mk(0, 0), jy = jx, jz = jx;
+    if (m.inside) {
+        const double kx = ph.k0 * m.nx, ky = ph.k0 * m.ny, kz = ph.k0 * m.nz;
+        const cd bx = B.p[0][m.idx], by = B.p[1][m.idx], bz = B.p[2][m.idx];
+        jx = imul(ky, bz) - imul(kz, by);
+        jy = imul(kz, bx) - imul(kx, bz);
+        jz = imul(kx, by) - imul(ky, bx);
+    }
+    J.p[0][m.idx] = jx; J.p[1][m.idx] = jy; J.p[2][m.idx] = jz;
+}
+void launch_build_current(const SpecGeom& g, const cd* const B[3], cd* const J[3], Phys ph, cudaStream_t st) {
+    Ptr3 b; PtrW3 j;
+    for (int c = 0; c < 3; ++c) { b.p[c] = B[c]; j.p[c] = J[c]; }
+    build_current_kernel<<<mode_grid(g, KT), KT, 0, st>>>(g, b, j, ph);
+}
+
+// ---- div^ = M i k . B^ ---------------------------------------------------------------------------------
+__global__ void divergence_kernel(SpecGeom g, Ptr3 B, cd* out, Phys ph) {
+    ModeIt m;
+    if (!mode_of_thread(g, m)) return;
+    cd d = mk(0, 0);
+    if (m.inside) {
+        const double kx = ph.k0 * m.nx, ky = ph.k0 * m.ny, kz = ph.k0 * m.nz;
+        d = imul(kx, B.p[0][m.idx]) + imul(ky, B.p[1][m.idx]) + imul(kz, B.p[2][m.idx]);
+    }
+    out[m.idx] = d;
+}
+void launch_divergence(const SpecGeom& g, const cd* const B[3], cd* out, Phys ph, cudaStream_t st) {
+    Ptr3 b;
+    for (int c = 0; c < 3; ++c) b.p[c] = B[c];
+    divergence_kernel<<<mode_grid(g, KT), KT, 0, st>>>(g, b, out, ph);
+}
+
+// ---- R^ assembly (+ explicit update) -------------------------------------------------------------------
+// mode 0: rout = R ; 1: U += dt R, Rold = R ; 2: U += dt (1.5 R - 0.5 Rold), Rold = R
+__global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 rout, int mode, double dt, Phys ph) {
+    ModeIt m;
+    if (!mode_of_thread(g, m)) return;
+    const long long i = m.idx;
+    cd R[8];
+    if (m.inside) {
+        const double kx = ph.k0 * m.nx, ky = ph.k0 * m.ny, kz = ph.k0 * m.nz;
+        const double k2 = kx * kx + ky * ky + kz * kz;
+        cd u[8];
+#pragma unroll
+        for (int f = 0; f < 8; ++f) u[f] = U.p[f][i];
+        const cd txx = pr.p[P_TXX][i], txy = pr.p[P_TXY][i], txz = pr.p[P_TXZ][i];
+        const cd tyy = pr.p[P_TYY][i], tyz = pr.p[P_TYZ][i], tzz = pr.p[P_TZZ][i];
+        const cd ex = pr.p[P_EX][i], ey = pr.p[P_EY][i], ez = pr.p[P_EZ][i];
+        // -i k.F = -(i kx Fx + i ky Fy + i kz Fz)
+        R[0] = mk(0, 0) - (imul(kx, u[1]) + imul(ky, u[2]) + imul(kz, u[3]));
+        R[1] = mk(0, 0) - (imul(kx, txx) + imul(ky, txy) + imul(kz, txz)) - (ph.mu * k2) * pr.p[P_UX][i];
+        R[2] = mk(0, 0) - (imul(kx, txy) + imul(ky, tyy) + imul(kz, tyz)) - (ph.mu * k2) * pr.p[P_UY][i];
+        R[3] = mk(0, 0) - (imul(kx, txz) + imul(ky, tyz) + imul(kz, tzz)) - (ph.mu * k2) * pr.p[P_UZ][i];
+        R[4] = mk(0, 0) - (imul(kx, pr.p[P_FEX][i]) + imul(ky, pr.p[P_FEY][i]) + imul(kz, pr.p[P_FEZ][i]))
+               - (ph.mu * k2) * pr.p[P_Q][i];
+        R[5] = imul(ky, ez) - imul(kz, ey) - (ph.eta * k2) * u[5];
+        R[6] = imul(kz, ex) - imul(kx, ez) - (ph.eta * k2) * u[6];
+        R[7] = imul(kx, ey) - imul(ky, ex) - (ph.eta * k2) * u[7];
+        if (mode == 0) {
+#pragma unroll
+            for (int f = 0; f < 8; ++f) rout.p[f][i] = R[f];
+        } else {
+#pragma unroll
+            for (int f = 0; f < 8; ++f) {
+                cd inc;
+                if (mode == 1) inc = R[f];
+                else { const cd ro = Rold.p[f][i]; inc = mk(1.5 * R[f].x - 0.5 * ro.x, 1.5 * R[f].y - 0.5 * ro.y); }
+                U.p[f][i] = mk(u[f].x + dt * inc.x, u[f].y + dt * inc.y);
+                Rold.p[f][i] = R[f];
+            }
+        }
+    } else if (mode == 0) {      // unpruned sweep: make the masked-out modes explicit zeros
+#pragma unroll
+        for (int f = 0; f < 8; ++f) rout.p[f][i] = mk(0, 0);
+    }
+}
+void launch_assemble(const SpecGeom& g, const cd* const prod[16], cd* const U[8], cd* const Rold[8],
+                     cd* const rout[8], int mode, double dt, Phys ph, cudaStream_t st) {
+    PtrC16 p; Ptr8 u, ro, rr;
+    for (int f = 0; f < 16; ++f) p.p[f] = prod[f];
+    for (int f = 0; f < 8; ++f) { u.p[f] = U[f]; ro.p[f] = Rold ? Rold[f] : nullptr; rr.p[f] = rout ? rout[f] : nullptr; }
+    assemble_kernel<<<mode_grid(g, KT), KT, 0, st>>>(g, p, u, ro, rr, mode, dt, ph);
+}
+
+// ---- y = a y + b x on the masked modes (integrator stages) -----------------------------------------------
+__global__ void axpby_kernel(SpecGeom g, int nf, double a, PtrN y, double b, PtrCN x) {
+    ModeIt m;
+    if (!mode_of_thread(g, m) || !m.inside) return;
+    for (int f = 0; f < nf; ++f) {
+        const cd xv = x.p[f][m.idx];
+        cd yv = mk(0, 0);
+        if (a != 0.0) { yv = y.p[f][m.idx]; yv = mk(a * yv.x, a * yv.y); }
+        y.p[f][m.idx] = mk(yv.x + b * xv.x, yv.y + b * xv.y);
+    }
+}
+void launch_axpby(const SpecGeom& g, int nf, double a, cd* const y[], double b, const cd* const x[], cudaStream_t st) {
+    PtrN yy; PtrCN xx;
+    for (int f = 0; f < nf; ++f) { yy.p[f] = y[f]; xx.p[f] = x[f]; }
+    axpby_kernel<<<mode_grid(g, KT), KT, 0, st>>>(g, nf, a, yy, b, xx);
+}
+void launch_copy_masked(const SpecGeom& g, int nf, cd* const dst[], const cd* const src[], cudaStream_t st) {
+    launch_axpby(g, nf, 0.0, dst, 1.0, src, st);
+}
+
+// ---- zero the modes outside the mask (unpruned sweep over everything stored) -----------------------------
+__global__ void zero_outside_kernel(SpecGeom g, int nf, PtrN f) {
+    ModeIt m;
+    if (!mode_of_thread(g, m) || m.inside) return;
+    for (int c = 0; c < nf; ++c) f.p[c][m.idx] = mk(0, 0);
+}
+void launch_zero_outside_mask(const SpecGeom& g0, int nf, cd* const f[], cudaStream_t st) {
+    SpecGeom g = g0; g.pruned = 0;
+    PtrN p;
+    for (int c = 0; c < nf; ++c) p.p[c] = f[c];
+    zero_outside_kernel<<<mode_grid(g, KT), KT, 0, st>>>(g, nf, p);
+}
+
+// ---- real-space point-wise kernels -----------------------------------------------------------------------
+struct PtrR11 { const double* p[11]; };
+struct PtrR16 { double* p[16]; };
+struct PtrR8 { double* p[8]; };
+struct PtrRC8 { const double* p[8]; };
+struct PtrRW3 { double* p[3]; };
+
+__global__ void flux_real_kernel(long long n, PtrR11 in, PtrR16 out, Phys ph) {
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        double s[S_NIN], o[P_NOUT];
+#pragma unroll
+        for (int f = 0; f < S_NIN; ++f) s[f] = in.p[f][i];
+        flux_point(s, o, ph);
+#pragma unroll
+        for (int f = 0; f < P_NOUT; ++f) out.p[f][i] = o[f];
+    }
+}
+static int ew_blocks(long long n, int threads) {
+    long long b = (n + threads - 1) / threads;
+    const long long cap = 148LL * 16;
+    return (int)(b < cap ? b : cap);
+}
+void launch_flux_real(long long n, const double* const in[11], double* const out[16], Phys ph, cudaStream_t st) {
+    PtrR11 a; PtrR16 b;
+    for (int f = 0; f < 11; ++f) a.p[f] = in[f];
+    for (int f = 0; f < 16; ++f) b.p[f] = out[f];
+    flux_real_kernel<<<ew_blocks(n, 256), 256, 0, st>>>(n, a, b, ph);
+}
+
+__global__ void prim_to_cons_kernel(long long n, PtrR8 f, double gamma) {
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const double rho = f.p[0][i], ux = f.p[1][i], uy = f.p[2][i], uz = f.p[3][i], P = f.p[4][i];
+        const double bx = f.p[5][i], by = f.p[6][i], bz = f.p[7][i];
+        f.p[1][i] = rho * ux; f.p[2][i] = rho * uy; f.p[3][i] = rho * uz;
+        f.p[4][i] = P / (gamma - 1.0) + 0.5 * rho * (ux * ux + uy * uy + uz * uz) + 0.5 * (bx * bx + by * by + bz * bz);
+    }
+}
+void launch_prim_to_cons(long long n, double* const f[8], double gamma, cudaStream_t st) {
+    PtrR8 a;
+    for (int c = 0; c < 8; ++c) a.p[c] = f[c];
+    prim_to_cons_kernel<<<ew_blocks(n, 256), 256, 0, st>>>(n, a, gamma);
+}
+__global__ void cons_to_prim_kernel(long long n, PtrR8 f, double gamma) {
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const double rho = f.p[0][i], mx = f.p[1][i], my = f.p[2][i], mz = f.p[3][i], E = f.p[4][i];
+        const double bx = f.p[5][i], by = f.p[6][i], bz = f.p[7][i];
+        const double ux = mx / rho, uy = my / rho, uz = mz / rho;
+        f.p[1][i] = ux; f.p[2][i] = uy; f.p[3][i] = uz;
+        f.p[4][i] = (gamma - 1.0) * (E - 0.5 * (mx * ux + my * uy + mz * uz) - 0.5 * (bx * bx + by * by + bz * bz));
+    }
+}
+void launch_cons_to_prim(long long n, double* const f[8], double gamma, cudaStream_t st) {
+    PtrR8 a;
+    for (int c = 0; c < 8; ++c) a.p[c] = f[c];
+    cons_to_prim_kernel<<<ew_blocks(n, 256), 256, 0, st>>>(n, a, gamma);
+}
+
+__global__ void sqrt_rho_u_kernel(long long n, PtrRC8 U, PtrRW3 w) {
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const double s = 1.0 / sqrt(U.p[0][i]);
+        w.p[0][i] = U.p[1][i] * s; w.p[1][i] = U.p[2][i] * s; w.p[2][i] = U.p[3][i] * s;
+    }
+}
+void launch_sqrt_rho_u(long long n, const double* const U[8], double* const w[3], cudaStream_t st) {
+    PtrRC8 a; PtrRW3 b;
+    for (int c = 0; c < 8; ++c) a.p[c] = U[c];
+    for (int c = 0; c < 3; ++c) b.p[c] = w[c];
+    sqrt_rho_u_kernel<<<ew_blocks(n, 256), 256, 0, st>>>(n, a, b);
+}
+
+// ---- reductions: fixed grid, fixed tree order -> bitwise reproducible -------------------------------------
+constexpr int RB = 1024;     // blocks of the first stage
+constexpr int RT = 256;      // threads per block
+constexpr int NRED = 10;     // ke, me, ie, mass, momx, momy, momz, etot (sums); rho_min, p_min
+
+__device__ __forceinline__ void block_reduce(double (&v)[NRED], double* sh /*[NRED][RT]*/) {
+    const int t = threadIdx.x;
+#pragma unroll
+    for (int q = 0; q < NRED; ++q) sh[q * RT + t] = v[q];
+    __syncthreads();
+    for (int s = RT / 2; s > 0; s >>= 1) {
+        if (t < s) {
+#pragma unroll
+            for (int q = 0; q < NRED; ++q) {
+                const double a = sh[q * RT + t], b = sh[q * RT + t + s];
+                sh[q * RT + t] = (q < 8) ? a + b : fmin(a, b);
+            }
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int q = 0; q < NRED; ++q) v[q] = sh[q * RT];
+}
+
+__global__ void __launch_bounds__(RT) diag_stage1(long long n, PtrRC8 U, double gamma, double* part /*[RB][NRED]*/) {
+    __shared__ double sh[NRED * RT];
+    double v[NRED];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) v[q] = 0.0;
+    v[8] = v[9] = 1e300;
+    for (long long i = blockIdx.x * (long long)RT + threadIdx.x; i < n; i += (long long)RB * RT) {
+        const double rho = U.p[0][i], mx = U.p[1][i], my = U.p[2][i], mz = U.p[3][i], E = U.p[4][i];
+        const double bx = U.p[5][i], by = U.p[6][i], bz = U.p[7][i];
+        const double ux = mx / rho, uy = my / rho, uz = mz / rho;
+        const double k = 0.5 * (mx * ux + my * uy + mz * uz), hb = 0.5 * (bx * bx + by * by + bz * bz);
+        const double P = (gamma - 1.0) * (E - k - hb);
+        v[0] += k; v[1] += hb; v[2] += P / (gamma - 1.0); v[3] += rho; v[4] += mx; v[5] += my; v[6] += mz; v[7] += E;
+        v[8] = fmin(v[8], rho); v[9] = fmin(v[9], P);
+    }
+    block_reduce(v, sh);
+    if (threadIdx.x == 0)
+        for (int q = 0; q < NRED; ++q) part[blockIdx.x * NRED + q] = v[q];
+}
+__global__ void __launch_bounds__(RT) diag_stage2(const double* part, double* out, double inv_n) {
+    __shared__ double sh[NRED * RT];
+    double v[NRED];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) v[q] = 0.0;
+    v[8] = v[9] = 1e300;
+    for (int b = threadIdx.x; b < RB; b += RT)
+        for (int q = 0; q < NRED; ++q) {
+            const double x = part[b * NRED + q];
+            v[q] = (q < 8) ? v[q] + x : fmin(v[q], x);
+        }
+    block_reduce(v, sh);
+    if (threadIdx.x == 0)
+        for (int q = 0; q < NRED; ++q) out[q] = (q < 8) ? v[q] * inv_n : v[q];
+}
+void launch_diag_reduce(long long n, const double* const U[8], double gamma, double* scratch, double* out,
+                        cudaStream_t st) {
+    PtrRC8 a;
+    for (int c = 0; c < 8; ++c) a.p[c] = U[c];
+    diag_stage1<<<RB, RT, 0, st>>>(n, a, gamma, scratch);
+    diag_stage2<<<1, RT, 0, st>>>(scratch, out, 1.0 / (double)n);
+}
+
+__global__ void __launch_bounds__(RT) absmax_stage1(long long n, const double* f, double* part) {
+    __shared__ double sh[RT];
+    double v = 0.0;
+    for (long long i = blockIdx.x * (long long)RT + threadIdx.x; i < n; i += (long long)RB * RT) v = fmax(v, fabs(f[i]));
+    sh[threadIdx.x] = v;
+    __syncthreads();
+    for (int s = RT / 2; s > 0; s >>= 1) {
+        if (threadIdx.x < s) sh[threadIdx.x] = fmax(sh[threadIdx.x], sh[threadIdx.x + s]);
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) part[blockIdx.x] = sh[0];
+}
+__global__ void __launch_bounds__(RT) absmax_stage2(const double* part, double* out) {
+    __shared__ double sh[RT];
+    double v = 0.0;
+    for (int b = threadIdx.x; b < RB; b += RT) v = fmax(v, part[b]);
+    sh[threadIdx.x] = v;
+    __syncthreads();
+    for (int s = RT / 2; s > 0; s >>= 1) {
+        if (threadIdx.x < s) sh[threadIdx.x] = fmax(sh[threadIdx.x], sh[threadIdx.x + s]);
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) out[0] = sh[0];
+}
+void launch_absmax(long long n, const double* f, double* scratch, double* out, cudaStream_t st) {
+    absmax_stage1<<<RB, RT, 0, st>>>(n, f, scratch);
+    absmax_stage2<<<1, RT, 0, st>>>(scratch, out);
+}
+
+// ---- shell spectra ---------------------------------------------------------------------------------------
+// S(K) = sum over the FULL mode cube with floor(|n|+1/2) = K of 1/2 sum_c |w^_c(n)|^2 / N^6.  The stored half
+// spectrum counts kx = 1..N/2-1 twice (the conjugate half), kx = 0 and the Nyquist plane once.
+constexpr int SB = 512;      // blocks of the first stage
+constexpr int MAXSPEC = 1024;
+int diag_scratch_doubles(int nspec) { int a = SB * nspec, b = RB * NRED; return a > b ? a : b; }
+
+__global__ void __launch_bounds__(256) spectrum_stage1(int N, Ptr3 spec, Ptr3 nyq, double* part /*[SB][nspec]*/, int nspec) {
+    __shared__ double hist[MAXSPEC];
+    for (int k = threadIdx.x; k < nspec; k += blockDim.x) hist[k] = 0.0;
+    __syncthreads();
+    const int hx = N / 2;
+    const long long nmain = (long long)N * N * hx, nny = (long long)N * N;
+    const double n3 = (double)N * N * N, norm = 0.5 / (n3 * n3);
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < nmain + nny; i += (long long)SB * blockDim.x) {
+        int ix, iy, iz; double e = 0.0, wgt;
+        if (i < nmain) {
+            ix = (int)(i % hx); iy = (int)((i / hx) % N); iz = (int)(i / ((long long)hx * N));
+            for (int c = 0; c < 3; ++c) { const cd a = spec.p[c][i]; e += a.x * a.x + a.y * a.y; }
+            wgt = ix == 0 ? 1.0 : 2.0;
+        } else {
+            const long long r = i - nmain;
+            ix = hx; iy = (int)(r % N); iz = (int)(r / N);
+            if (nyq.p[0]) for (int c = 0; c < 3; ++c) { const cd a = nyq.p[c][r * 8]; e += a.x * a.x + a.y * a.y; }
+            wgt = 1.0;
+        }
+        const int ny = iy <= N / 2 ? iy : iy - N, nz = iz <= N / 2 ? iz : iz - N;
+        const int K = (int)floor(sqrt((double)(ix * ix + ny * ny + nz * nz)) + 0.5);
+        if (e != 0.0) atomicAdd(&hist[K], wgt * norm * e);
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < nspec; k += blockDim.x) part[(long long)blockIdx.x * nspec + k] = hist[k];
+}
+__global__ void spectrum_stage2(const double* part, double* out, int nspec) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nspec) return;
+    double s = 0.0;
+    for (int b = 0; b < SB; ++b) s += part[(long long)b * nspec + k];
+    out[k] = s;
+}
+void launch_shell_spectrum(int N, const cd* const spec[3], const cd* const nyq[3], double* scratch, double* out,
+                           int nspec, cudaStream_t st) {
+    Ptr3 a, b;
+    for (int c = 0; c < 3; ++c) { a.p[c] = spec[c]; b.p[c] = nyq ? nyq[c] : nullptr; }
+    spectrum_stage1<<<SB, 256, 0, st>>>(N, a, b, scratch, nspec);
+    spectrum_stage2<<<(nspec + 127) / 128, 128, 0, st>>>(scratch, out, nspec);
+}
+
+// ---- twiddle table: w[m] = exp(-2 pi i m / N), exactly rounded sincospi, no recurrences -------------------
+__global__ void twiddle_kernel(int N, cd* tw) {
+    const int m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= N) return;
+    double s, c;
+    sincospi(2.0 * (double)m / (double)N, &s, &c);
+    tw[m] = mk(c, -s);
+}
+void launch_twiddle_table(int N, cd* tw, cudaStream_t st) { twiddle_kernel<<<(N + 127) / 128, 128, 0, st>>>(N, tw); }
+
+}  // namespace mhd

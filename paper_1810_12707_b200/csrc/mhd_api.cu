@@ -1,0 +1,538 @@
+// mhd_api.cu — context, workspace layout, sweep orchestration and the C ABI of include/mhd.h.
+//
+// State lives in k-space: U^ (8 half-spectrum arrays, zero outside the 2/3 mask) and the Adams-Bashforth history
+// R^old.  One right-hand side is five sweeps over HBM:
+//   S1  build J^ = i k x B^ ; inverse z pass of (U^, J^) -> W[0..10]          (pruned: only modes inside the mask)
+//   S2  inverse y pass, in place
+//   S3  x_fused: C2R of 11 fields, flux products, R2C of 16 products, in place on W[0..15]
+//   S4  forward y pass, in place
+//   S5  forward z pass ; assembly of R^ (i k, -k^2, mask) and the explicit update
+// No host round trip inside mhd_step: only kernel launches on the bound stream.
+#include "../../include/mhd.h"
+#include "kernels.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace mhd;
+
+namespace {
+
+enum Family { F_STRIDED_INV = 0, F_STRIDED_FWD, F_X_FUSED, F_X_C2R, F_X_R2C, F_FLUX, F_CURRENT, F_ASSEMBLE, F_AXPBY,
+              F_POINT, F_DIAG, F_COUNT };
+const char* kFamilyNames[F_COUNT] = {"strided_inverse", "strided_forward", "x_fused", "x_c2r", "x_r2c", "flux_real",
+                                     "build_current", "assemble", "axpby", "pointwise_misc", "diagnostics"};
+
+size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+constexpr int NFIELD_BUFS = 48;   // U 8, Rold 8, W 16, X 8, Y 8
+
+struct Layout {
+    size_t field_bytes, tw_off, field_off, nyq_off, nyq_bytes, scratch_off, scratch_bytes, res_off, total;
+};
+int nspec_of(int N) { return (int)std::ceil(std::sqrt(3.0) * N / 2.0) + 1; }
+Layout make_layout(int N) {
+    Layout l;
+    l.field_bytes = (size_t)N * N * N * sizeof(double);
+    size_t off = 0;
+    l.tw_off = off; off += align_up((size_t)N * sizeof(cd));
+    l.field_off = off; off += (size_t)NFIELD_BUFS * align_up(l.field_bytes);
+    l.nyq_bytes = align_up((size_t)N * N * 8 * sizeof(cd));
+    l.nyq_off = off; off += 3 * l.nyq_bytes;
+    l.scratch_bytes = align_up((size_t)diag_scratch_doubles(nspec_of(N)) * sizeof(double));
+    l.scratch_off = off; off += l.scratch_bytes;
+    l.res_off = off; off += align_up((size_t)(64 + 2 * nspec_of(N)) * sizeof(double));
+    l.total = off;
+    return l;
+}
+bool valid_N(int N) { return N >= 16 && N <= 1024 && (N & (N - 1)) == 0; }
+
+}  // namespace
+
+struct mhd_ctx {
+    int N = 0;
+    double L = 0, gamma = 0, mu = 0, eta = 0, dt = 0;
+    bool bound = false, have_fields = false, have_old = false;
+    cudaStream_t st = nullptr;
+    unsigned flags = 0;
+    int opt_fused = 1, opt_prune = 1, integrator = 0;
+    long long step = 0;
+    long long launches = 0;
+    std::string err;
+    // device storage (inside the caller's workspace)
+    cd* tw = nullptr;
+    cd *U[8], *Rold[8], *W[16], *X[8], *Y[8], *nyq[3];
+    double *scratch = nullptr, *res = nullptr;
+    // profiling
+    bool prof = false;
+    struct Rec { int fam; cudaEvent_t a, b; };
+    std::vector<Rec> recs;
+    std::vector<cudaEvent_t> pool;
+    double fam_ms[F_COUNT] = {0};
+    long long fam_n[F_COUNT] = {0};
+
+    int fail(int code, const std::string& m) { err = m; return code; }
+    int hx() const { return N / 2; }
+    int kc() const { return N / 3; }
+    long long n3() const { return (long long)N * N * N; }
+    Phys phys() const { return Phys{2.0 * M_PI / L, gamma, mu, eta}; }
+    SpecGeom geom() const { return SpecGeom{N, N / 2, N / 3, opt_prune}; }
+
+    cudaEvent_t get_event() {
+        if (!pool.empty()) { cudaEvent_t e = pool.back(); pool.pop_back(); return e; }
+        cudaEvent_t e; cudaEventCreate(&e); return e;
+    }
+    struct Scope {
+        mhd_ctx* c; int fam; cudaEvent_t a = nullptr;
+        Scope(mhd_ctx* c_, int fam_, int nlaunch = 1) : c(c_), fam(fam_) {
+            c->launches += nlaunch; c->fam_n[fam] += nlaunch;
+            if (c->prof) { a = c->get_event(); cudaEventRecord(a, c->st); }
+        }
+        ~Scope() {
+            if (a) { cudaEvent_t b = c->get_event(); cudaEventRecord(b, c->st); c->recs.push_back({fam, a, b}); }
+        }
+    };
+    void drain_profile() {
+        if (recs.empty()) return;
+        cudaStreamSynchronize(st);
+        for (auto& r : recs) {
+            float ms = 0; cudaEventElapsedTime(&ms, r.a, r.b);
+            fam_ms[r.fam] += ms; pool.push_back(r.a); pool.push_back(r.b);
+        }
+        recs.clear();
+    }
+};
+
+namespace {
+
+int check_cuda(mhd_ctx* c, const char* what) {
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return c->fail(MHD_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+    return MHD_OK;
+}
+
+// ---- sweeps --------------------------------------------------------------------------------------------------
+// strided pass over nf arrays; axis 1 = y, 2 = z; hx = row pitch of the arrays (N/2, or 8 for the Nyquist planes)
+void strided_pass(mhd_ctx* c, int dir, int axis, int nf, const cd* const in[], cd* const out[], int hx, int ncols_full,
+                  bool prune) {
+    const int N = c->N, kc = c->kc();
+    int done = 0;
+    while (done < nf) {
+        const int nb = std::min(nf - done, MAXF);
+        StridedArgs a;
+        std::memset(&a, 0, sizeof(a));
+        for (int f = 0; f < nb; ++f) { a.in[f] = in[done + f]; a.out[f] = out[done + f]; }
+        a.tw = c->tw;
+        a.kc = kc;
+        a.nfields = nb;
+        const int C = N >= 1024 ? 4 : 8;
+        a.ncols = prune ? std::min(kc + 1, ncols_full) : ncols_full;
+        a.nchunks = (a.ncols + C - 1) / C;
+        if (axis == 1) {            // y pass: rows along y, outer = z (all planes)
+            a.row_stride = hx; a.outer_stride = (long long)N * hx;
+            a.n_outer = N; a.outer_split = N; a.outer_skip = 0;
+        } else {                    // z pass: rows along z, outer = ky (pruned to the mask)
+            a.row_stride = (long long)N * hx; a.outer_stride = hx;
+            if (prune) { a.n_outer = 2 * kc + 1; a.outer_split = kc + 1; a.outer_skip = N - (2 * kc + 1); }
+            else { a.n_outer = N; a.outer_split = N; a.outer_skip = 0; }
+        }
+        a.in_pruned = (prune && dir > 0) ? 1 : 0;     // inverse: input rows outside the mask are zero
+        a.out_pruned = (prune && dir < 0) ? 1 : 0;    // forward: output rows outside the mask are not needed
+        mhd_ctx::Scope s(c, dir > 0 ? F_STRIDED_INV : F_STRIDED_FWD);
+        launch_strided(N, dir, a, c->st);
+        done += nb;
+    }
+}
+
+// spec (destroyed unless work != spec) -> real.  work may alias spec; real_out may alias work.
+void inverse3d(mhd_ctx* c, int nf, const cd* const spec[], cd* const work[], double* const real_out[], bool prune) {
+    const int N = c->N;
+    strided_pass(c, +1, 2, nf, spec, work, c->hx(), c->hx(), prune);
+    strided_pass(c, +1, 1, nf, work, work, c->hx(), c->hx(), prune);
+    int done = 0;
+    while (done < nf) {
+        const int nb = std::min(nf - done, MAXF);
+        XArgs a; std::memset(&a, 0, sizeof(a));
+        for (int f = 0; f < nb; ++f) { a.spec_in[f] = work[done + f]; a.real_out[f] = real_out[done + f]; }
+        a.tw = c->tw; a.nlines = (long long)N * N; a.nfields = nb;
+        a.kmax = prune ? c->kc() : c->hx() - 1;
+        a.scale = 1.0 / ((double)N * N * N);
+        mhd_ctx::Scope s(c, F_X_C2R);
+        launch_x_c2r(N, a, c->st);
+        done += nb;
+    }
+}
+
+// real -> spec (may alias real storage); nyq (optional, unpruned only) receives the kx = N/2 plane
+void forward3d(mhd_ctx* c, int nf, const double* const real_in[], cd* const spec[], cd* const nyq[], bool prune) {
+    const int N = c->N;
+    int done = 0;
+    while (done < nf) {
+        const int nb = std::min(nf - done, MAXF);
+        XArgs a; std::memset(&a, 0, sizeof(a));
+        for (int f = 0; f < nb; ++f) {
+            a.real_in[f] = real_in[done + f]; a.spec_out[f] = spec[done + f];
+            a.nyq_out[f] = nyq ? nyq[done + f] : nullptr;
+        }
+        a.tw = c->tw; a.nlines = (long long)N * N; a.nfields = nb;
+        a.kmax = prune ? c->kc() : c->hx() - 1;
+        a.scale = 1.0;
+        mhd_ctx::Scope s(c, F_X_R2C);
+        launch_x_r2c(N, a, c->st);
+        done += nb;
+    }
+    strided_pass(c, -1, 1, nf, spec, spec, c->hx(), c->hx(), prune);
+    strided_pass(c, -1, 2, nf, spec, spec, c->hx(), c->hx(), prune);
+    if (nyq) {
+        strided_pass(c, -1, 1, nf, nyq, nyq, 8, 1, false);
+        strided_pass(c, -1, 2, nf, nyq, nyq, 8, 1, false);
+    }
+}
+
+// products W[0..15] <- state Uin (k-space); sweeps S1-S4 and the forward z pass of S5
+void products(mhd_ctx* c, cd* const Uin[8]) {
+    const int N = c->N;
+    const bool prune = c->opt_prune != 0;
+    const SpecGeom g = c->geom();
+    const Phys ph = c->phys();
+    {   // S1a: J^ = M i k x B^ -> W[8..10]
+        mhd_ctx::Scope s(c, F_CURRENT);
+        launch_build_current(g, Uin + 5, c->W + 8, ph, c->st);
+    }
+    const cd* in[11];
+    for (int f = 0; f < 8; ++f) in[f] = Uin[f];
+    for (int f = 8; f < 11; ++f) in[f] = c->W[f];
+    strided_pass(c, +1, 2, 11, in, c->W, c->hx(), c->hx(), prune);        // S1b
+    strided_pass(c, +1, 1, 11, c->W, c->W, c->hx(), c->hx(), prune);      // S2
+    const int kmax = prune ? c->kc() : c->hx() - 1;
+    const double scale = 1.0 / ((double)N * N * N);
+    if (c->opt_fused) {                                                   // S3
+        FusedXArgs a; std::memset(&a, 0, sizeof(a));
+        for (int f = 0; f < 11; ++f) a.in[f] = c->W[f];
+        for (int f = 0; f < 16; ++f) a.out[f] = c->W[f];
+        a.tw = c->tw; a.nlines = (long long)N * N; a.kmax_in = kmax; a.kmax_out = kmax; a.scale = scale; a.ph = ph;
+        mhd_ctx::Scope s(c, F_X_FUSED);
+        launch_x_fused(N, a, c->st);
+    } else {
+        XArgs a; std::memset(&a, 0, sizeof(a));
+        for (int f = 0; f < 11; ++f) { a.spec_in[f] = c->W[f]; a.real_out[f] = reinterpret_cast<double*>(c->W[f]); }
+        a.tw = c->tw; a.nlines = (long long)N * N; a.nfields = 11; a.kmax = kmax; a.scale = scale;
+        { mhd_ctx::Scope s(c, F_X_C2R); launch_x_c2r(N, a, c->st); }
+        const double* rin[11]; double* rout[16];
+        for (int f = 0; f < 11; ++f) rin[f] = reinterpret_cast<const double*>(c->W[f]);
+        for (int f = 0; f < 16; ++f) rout[f] = reinterpret_cast<double*>(c->W[f]);
+        { mhd_ctx::Scope s(c, F_FLUX); launch_flux_real(c->n3(), rin, rout, ph, c->st); }
+        XArgs b; std::memset(&b, 0, sizeof(b));
+        for (int f = 0; f < 16; ++f) { b.real_in[f] = rout[f]; b.spec_out[f] = c->W[f]; }
+        b.tw = c->tw; b.nlines = (long long)N * N; b.nfields = 16; b.kmax = kmax; b.scale = 1.0;
+        { mhd_ctx::Scope s(c, F_X_R2C); launch_x_r2c(N, b, c->st); }
+    }
+    strided_pass(c, -1, 1, 16, c->W, c->W, c->hx(), c->hx(), prune);      // S4
+    strided_pass(c, -1, 2, 16, c->W, c->W, c->hx(), c->hx(), prune);      // S5a
+}
+
+// R^(Uin) -> rout (mode 0) or explicit update of Uin / Rold (mode 1 Euler, 2 AB2)
+void rhs_spectral(mhd_ctx* c, cd* const Uin[8], cd* const rout[8], int mode) {
+    products(c, Uin);
+    mhd_ctx::Scope s(c, F_ASSEMBLE);
+    launch_assemble(c->geom(), c->W, Uin, c->Rold, rout, mode, c->dt, c->phys(), c->st);
+}
+
+int copy_in(mhd_ctx* c, int where, const double* const src[8], double* const dst[8]) {
+    const size_t bytes = (size_t)c->n3() * sizeof(double);
+    for (int f = 0; f < 8; ++f) {
+        if (!src[f]) return c->fail(MHD_ERR_INVALID_ARG, "null field pointer");
+        cudaMemcpyAsync(dst[f], src[f], bytes, where == MHD_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, c->st);
+    }
+    return check_cuda(c, "copy in");
+}
+int copy_out(mhd_ctx* c, int where, double* const src[8], double* const dst[8]) {
+    const size_t bytes = (size_t)c->n3() * sizeof(double);
+    for (int f = 0; f < 8; ++f) {
+        if (!dst[f]) return c->fail(MHD_ERR_INVALID_ARG, "null field pointer");
+        if (dst[f] != src[f])
+            cudaMemcpyAsync(dst[f], src[f], bytes, where == MHD_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, c->st);
+    }
+    if (where == MHD_HOST) cudaStreamSynchronize(c->st);
+    return check_cuda(c, "copy out");
+}
+
+}  // namespace
+
+// =====================================================================================================================
+extern "C" {
+
+int mhd_init(mhd_ctx** out, int N, double L, double gamma, double mu, double eta, double dt) {
+    if (!out) return MHD_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!valid_N(N) || !(L > 0) || !(gamma > 1) || !(mu >= 0) || !(eta >= 0) || !(dt > 0)) return MHD_ERR_INVALID_ARG;
+    mhd_ctx* c = new (std::nothrow) mhd_ctx();
+    if (!c) return MHD_ERR_NOMEM;
+    c->N = N; c->L = L; c->gamma = gamma; c->mu = mu; c->eta = eta; c->dt = dt;
+    *out = c;
+    return MHD_OK;
+}
+
+size_t mhd_workspace_bytes(int N, unsigned flags) {
+    (void)flags;
+    if (!valid_N(N)) return 0;
+    return make_layout(N).total;
+}
+size_t mhd_pinned_bytes(int N, unsigned flags) { (void)N; (void)flags; return 0; }
+int mhd_nspec(int N) { return nspec_of(N); }
+
+int mhd_bind(mhd_ctx* c, void* dev_workspace, size_t bytes, void* cuda_stream, unsigned flags, void* pinned_host,
+             size_t pinned_bytes) {
+    if (!c) return MHD_ERR_INVALID_ARG;
+    (void)pinned_host; (void)pinned_bytes;
+    if (flags & MHD_FLAG_OUT_OF_CORE) return c->fail(MHD_ERR_INVALID_ARG, "out-of-core path not available in this build");
+    const Layout l = make_layout(c->N);
+    if (!dev_workspace || ((uintptr_t)dev_workspace & 255) != 0) return c->fail(MHD_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+    if (bytes < l.total) return c->fail(MHD_ERR_NOMEM, "workspace too small");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return c->fail(MHD_ERR_CUDA, "no CUDA device (libmhd has no CPU fallback)");
+    }
+    char* base = static_cast<char*>(dev_workspace);
+    c->st = static_cast<cudaStream_t>(cuda_stream);
+    c->flags = flags;
+    c->tw = reinterpret_cast<cd*>(base + l.tw_off);
+    const size_t fb = align_up(l.field_bytes);
+    char* fp = base + l.field_off;
+    int k = 0;
+    for (int f = 0; f < 8; ++f) c->U[f] = reinterpret_cast<cd*>(fp + (size_t)(k++) * fb);
+    for (int f = 0; f < 8; ++f) c->Rold[f] = reinterpret_cast<cd*>(fp + (size_t)(k++) * fb);
+    for (int f = 0; f < 16; ++f) c->W[f] = reinterpret_cast<cd*>(fp + (size_t)(k++) * fb);
+    for (int f = 0; f < 8; ++f) c->X[f] = reinterpret_cast<cd*>(fp + (size_t)(k++) * fb);
+    for (int f = 0; f < 8; ++f) c->Y[f] = reinterpret_cast<cd*>(fp + (size_t)(k++) * fb);
+    for (int f = 0; f < 3; ++f) c->nyq[f] = reinterpret_cast<cd*>(base + l.nyq_off + (size_t)f * l.nyq_bytes);
+    c->scratch = reinterpret_cast<double*>(base + l.scratch_off);
+    c->res = reinterpret_cast<double*>(base + l.res_off);
+    launch_twiddle_table(c->N, c->tw, c->st);
+    c->launches += 1;
+    int rc = check_cuda(c, "bind");
+    if (rc) return rc;
+    c->bound = true; c->have_fields = false; c->have_old = false; c->step = 0;
+    return MHD_OK;
+}
+
+int mhd_set_option(mhd_ctx* c, int option, int value) {
+    if (!c) return MHD_ERR_INVALID_ARG;
+    switch (option) {
+        case MHD_OPT_FUSED: c->opt_fused = value ? 1 : 0; return MHD_OK;
+        case MHD_OPT_PRUNE: c->opt_prune = value ? 1 : 0; return MHD_OK;
+        case MHD_OPT_INTEGRATOR:
+            if (value < 0 || value > 2) return c->fail(MHD_ERR_INVALID_ARG, "integrator must be 0, 1 or 2");
+            c->integrator = value; c->have_old = false; return MHD_OK;
+        default: return c->fail(MHD_ERR_INVALID_ARG, "unknown option");
+    }
+}
+
+int mhd_set_fields(mhd_ctx* c, int kind, int where, const double* const f[8]) {
+    if (!c || !f) return MHD_ERR_INVALID_ARG;
+    if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
+    if ((kind != 0 && kind != 1) || (where != 0 && where != 1)) return c->fail(MHD_ERR_INVALID_ARG, "kind/where");
+    double* real[8];
+    for (int i = 0; i < 8; ++i) real[i] = reinterpret_cast<double*>(c->W[i]);
+    int rc = copy_in(c, where, f, real);
+    if (rc) return rc;
+    if (kind == MHD_PRIMITIVE) { mhd_ctx::Scope s(c, F_POINT); launch_prim_to_cons(c->n3(), real, c->gamma, c->st); }
+    const size_t bytes = (size_t)c->n3() * sizeof(double);
+    for (int i = 0; i < 8; ++i) cudaMemsetAsync(c->U[i], 0, bytes, c->st);
+    // projection U <- M FFT U: the pruned forward transform writes exactly the modes inside the mask
+    const double* rin[8];
+    for (int i = 0; i < 8; ++i) rin[i] = real[i];
+    forward3d(c, 8, rin, c->W, nullptr, true);
+    {
+        SpecGeom g = c->geom(); g.pruned = 1;
+        const cd* src[8];
+        for (int i = 0; i < 8; ++i) src[i] = c->W[i];
+        mhd_ctx::Scope s(c, F_AXPBY);
+        launch_copy_masked(g, 8, c->U, src, c->st);
+    }
+    if (where == MHD_HOST) cudaStreamSynchronize(c->st);
+    rc = check_cuda(c, "set_fields");
+    if (rc) return rc;
+    c->have_fields = true; c->have_old = false; c->step = 0;
+    return MHD_OK;
+}
+
+int mhd_rhs(mhd_ctx* c, int where, double* const out[8]) {
+    if (!c || !out) return MHD_ERR_INVALID_ARG;
+    if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
+    if (!c->have_fields) return c->fail(MHD_ERR_NO_FIELDS, "mhd_set_fields has not been called");
+    if (where != 0 && where != 1) return c->fail(MHD_ERR_INVALID_ARG, "where");
+    rhs_spectral(c, c->U, c->X, 0);
+    double* real[8];
+    for (int i = 0; i < 8; ++i) real[i] = (where == MHD_DEVICE) ? out[i] : reinterpret_cast<double*>(c->X[i]);
+    inverse3d(c, 8, c->X, c->X, real, c->opt_prune != 0);
+    int rc = copy_out(c, where, real, out);
+    return rc ? rc : check_cuda(c, "rhs");
+}
+
+int mhd_step(mhd_ctx* c, int nsteps) {
+    if (!c || nsteps < 0) return MHD_ERR_INVALID_ARG;
+    if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
+    if (!c->have_fields) return c->fail(MHD_ERR_NO_FIELDS, "mhd_set_fields has not been called");
+    const SpecGeom g = c->geom();
+    SpecGeom gp = g; gp.pruned = 1;
+    for (int s = 0; s < nsteps; ++s) {
+        if (c->integrator == 0) {                       // Adams-Bashforth 2, Euler start (R6)
+            rhs_spectral(c, c->U, nullptr, c->have_old ? 2 : 1);
+            c->have_old = true;
+        } else if (c->integrator == 1) {                // classical RK4
+            // U0 = Rold, acc = Y, k = X, stage state in U
+            const cd* Uc[8]; const cd* Xc[8]; const cd* U0c[8]; const cd* Yc[8];
+            for (int f = 0; f < 8; ++f) { Uc[f] = c->U[f]; Xc[f] = c->X[f]; U0c[f] = c->Rold[f]; Yc[f] = c->Y[f]; }
+            const double dt = c->dt;
+            auto ax = [&](double a, cd* const y[], double b, const cd* const x[]) { mhd_ctx::Scope sc(c, F_AXPBY); launch_axpby(gp, 8, a, y, b, x, c->st); };
+            ax(0.0, c->Rold, 1.0, Uc);                  // U0 = U
+            rhs_spectral(c, c->U, c->X, 0);             // k1
+            ax(0.0, c->Y, dt / 6.0, Xc);                // acc = dt/6 k1
+            ax(0.0, c->U, 1.0, U0c); ax(1.0, c->U, 0.5 * dt, Xc);
+            rhs_spectral(c, c->U, c->X, 0);             // k2
+            ax(1.0, c->Y, dt / 3.0, Xc);
+            ax(0.0, c->U, 1.0, U0c); ax(1.0, c->U, 0.5 * dt, Xc);
+            rhs_spectral(c, c->U, c->X, 0);             // k3
+            ax(1.0, c->Y, dt / 3.0, Xc);
+            ax(0.0, c->U, 1.0, U0c); ax(1.0, c->U, dt, Xc);
+            rhs_spectral(c, c->U, c->X, 0);             // k4
+            ax(1.0, c->Y, dt / 6.0, Xc);
+            ax(0.0, c->U, 1.0, U0c); ax(1.0, c->U, 1.0, Yc);
+        } else {                                        // predictor-corrector (Heun): U* = U + dt R(U); U+ = U + dt/2 (R(U) + R(U*))
+            const cd* Uc[8]; const cd* Xc[8]; const cd* U0c[8]; const cd* Yc[8];
+            for (int f = 0; f < 8; ++f) { Uc[f] = c->U[f]; Xc[f] = c->X[f]; U0c[f] = c->Rold[f]; Yc[f] = c->Y[f]; }
+            const double dt = c->dt;
+            auto ax = [&](double a, cd* const y[], double b, const cd* const x[]) { mhd_ctx::Scope sc(c, F_AXPBY); launch_axpby(gp, 8, a, y, b, x, c->st); };
+            ax(0.0, c->Rold, 1.0, Uc);                  // U0 = U
+            rhs_spectral(c, c->U, c->X, 0);             // R(U)
+            ax(0.0, c->Y, 0.5 * dt, Xc);
+            ax(1.0, c->U, dt, Xc);                      // predictor
+            rhs_spectral(c, c->U, c->X, 0);             // R(U*)
+            ax(1.0, c->Y, 0.5 * dt, Xc);
+            ax(0.0, c->U, 1.0, U0c); ax(1.0, c->U, 1.0, Yc);
+        }
+        ++c->step;
+    }
+    return check_cuda(c, "step");
+}
+
+int mhd_get_fields(mhd_ctx* c, int kind, int where, double* const out[8]) {
+    if (!c || !out) return MHD_ERR_INVALID_ARG;
+    if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
+    if (!c->have_fields) return c->fail(MHD_ERR_NO_FIELDS, "mhd_set_fields has not been called");
+    if ((kind != 0 && kind != 1) || (where != 0 && where != 1)) return c->fail(MHD_ERR_INVALID_ARG, "kind/where");
+    double* real[8];
+    for (int i = 0; i < 8; ++i) real[i] = (where == MHD_DEVICE) ? out[i] : reinterpret_cast<double*>(c->W[i]);
+    inverse3d(c, 8, c->U, c->W, real, true);
+    if (kind == MHD_PRIMITIVE) { mhd_ctx::Scope s(c, F_POINT); launch_cons_to_prim(c->n3(), real, c->gamma, c->st); }
+    int rc = copy_out(c, where, real, out);
+    return rc ? rc : check_cuda(c, "get_fields");
+}
+
+int mhd_diagnostics(mhd_ctx* c, mhd_diag* d, double* spec_kin, double* spec_mag, int nspec) {
+    if (!c || !d) return MHD_ERR_INVALID_ARG;
+    if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
+    if (!c->have_fields) return c->fail(MHD_ERR_NO_FIELDS, "mhd_set_fields has not been called");
+    const int ns = nspec_of(c->N);
+    if ((spec_kin || spec_mag) && nspec != ns) return c->fail(MHD_ERR_INVALID_ARG, "nspec must equal mhd_nspec(N)");
+    const long long n3 = c->n3();
+    double* real[8];
+    for (int i = 0; i < 8; ++i) real[i] = reinterpret_cast<double*>(c->W[i]);
+    inverse3d(c, 8, c->U, c->W, real, true);
+    const double* rc8[8];
+    for (int i = 0; i < 8; ++i) rc8[i] = real[i];
+    { mhd_ctx::Scope s(c, F_DIAG, 2); launch_diag_reduce(n3, rc8, c->gamma, c->scratch, c->res, c->st); }
+    {   // max |div~ B|
+        SpecGeom g = c->geom(); g.pruned = 1;
+        const cd* B[3] = {c->U[5], c->U[6], c->U[7]};
+        { mhd_ctx::Scope s(c, F_POINT); launch_divergence(g, B, c->W[8], c->phys(), c->st); }
+        const cd* sp[1] = {c->W[8]}; cd* wk[1] = {c->W[8]}; double* ro[1] = {reinterpret_cast<double*>(c->W[8])};
+        inverse3d(c, 1, sp, wk, ro, true);
+        mhd_ctx::Scope s(c, F_DIAG, 2);
+        launch_absmax(n3, ro[0], c->scratch, c->res + 16, c->st);
+    }
+    if (spec_kin) {
+        double* w[3] = {reinterpret_cast<double*>(c->W[9]), reinterpret_cast<double*>(c->W[10]), reinterpret_cast<double*>(c->W[11])};
+        { mhd_ctx::Scope s(c, F_POINT); launch_sqrt_rho_u(n3, rc8, w, c->st); }
+        const double* wc[3] = {w[0], w[1], w[2]};
+        cd* sp[3] = {c->W[9], c->W[10], c->W[11]};
+        forward3d(c, 3, wc, sp, c->nyq, false);
+        const cd* spc[3] = {sp[0], sp[1], sp[2]}; const cd* nq[3] = {c->nyq[0], c->nyq[1], c->nyq[2]};
+        mhd_ctx::Scope s(c, F_DIAG, 2);
+        launch_shell_spectrum(c->N, spc, nq, c->scratch, c->res + 64, ns, c->st);
+    }
+    if (spec_mag) {
+        const cd* spc[3] = {c->U[5], c->U[6], c->U[7]};
+        mhd_ctx::Scope s(c, F_DIAG, 2);
+        launch_shell_spectrum(c->N, spc, nullptr, c->scratch, c->res + 64 + ns, ns, c->st);
+    }
+    std::vector<double> host(64 + 2 * ns);
+    cudaMemcpyAsync(host.data(), c->res, host.size() * sizeof(double), cudaMemcpyDeviceToHost, c->st);
+    cudaStreamSynchronize(c->st);
+    int rc = check_cuda(c, "diagnostics");
+    if (rc) return rc;
+    d->t = (double)c->step * c->dt; d->step = c->step;
+    d->ke = host[0]; d->me = host[1]; d->ie = host[2]; d->mass = host[3];
+    d->mom[0] = host[4]; d->mom[1] = host[5]; d->mom[2] = host[6]; d->etot = host[7];
+    d->rho_min = host[8]; d->p_min = host[9]; d->max_divb = host[16];
+    if (spec_kin) std::memcpy(spec_kin, host.data() + 64, ns * sizeof(double));
+    if (spec_mag) std::memcpy(spec_mag, host.data() + 64 + ns, ns * sizeof(double));
+    return MHD_OK;
+}
+
+int mhd_fft3d_r2c(mhd_ctx* c, int nfields, const double* const real[], double* const spec[], double* const nyq[], int prune) {
+    if (!c || !real || !spec || nfields < 1) return MHD_ERR_INVALID_ARG;
+    if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
+    std::vector<cd*> sp(nfields), nq(nfields);
+    for (int f = 0; f < nfields; ++f) { sp[f] = reinterpret_cast<cd*>(spec[f]); nq[f] = nyq ? reinterpret_cast<cd*>(nyq[f]) : nullptr; }
+    forward3d(c, nfields, real, sp.data(), (nyq && !prune) ? nq.data() : nullptr, prune != 0);
+    return check_cuda(c, "fft3d_r2c");
+}
+int mhd_fft3d_c2r(mhd_ctx* c, int nfields, double* const spec[], double* const real[], int prune) {
+    if (!c || !real || !spec || nfields < 1) return MHD_ERR_INVALID_ARG;
+    if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
+    std::vector<cd*> sp(nfields); std::vector<const cd*> spc(nfields);
+    for (int f = 0; f < nfields; ++f) { sp[f] = reinterpret_cast<cd*>(spec[f]); spc[f] = sp[f]; }
+    inverse3d(c, nfields, spc.data(), sp.data(), real, prune != 0);
+    return check_cuda(c, "fft3d_c2r");
+}
+
+long long mhd_launch_count(const mhd_ctx* c) { return c ? c->launches : 0; }
+
+int mhd_profile_enable(mhd_ctx* c, int on) {
+    if (!c) return MHD_ERR_INVALID_ARG;
+    if (c->bound) c->drain_profile();
+    c->prof = on != 0;
+    for (int i = 0; i < F_COUNT; ++i) { c->fam_ms[i] = 0; c->fam_n[i] = 0; }
+    return MHD_OK;
+}
+int mhd_profile_get(mhd_ctx* c, int max_entries, const char** names, double* ms, long long* launches) {
+    if (!c) return MHD_ERR_INVALID_ARG;
+    c->drain_profile();
+    int n = 0;
+    for (int i = 0; i < F_COUNT && n < max_entries; ++i, ++n) {
+        if (names) names[n] = kFamilyNames[i];
+        if (ms) ms[n] = c->fam_ms[i];
+        if (launches) launches[n] = c->fam_n[i];
+    }
+    return n;
+}
+
+const char* mhd_last_error(const mhd_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+int mhd_destroy(mhd_ctx* c) {
+    if (!c) return MHD_OK;
+    if (c->bound) c->drain_profile();
+    for (auto e : c->pool) cudaEventDestroy(e);
+    delete c;
+    return MHD_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,76 @@
+"""Host-side checks of the C ABI (no GPU needed): libmhd.so loads, exports every symbol include/mhd.h
+declares, validates its arguments and fails loudly without a device."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_1810_12707_b200 import build, binding
+    build.build()
+    return binding.lib()
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "mhd.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(mhd_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_header_symbols_exported(lib):
+    from paper_1810_12707_b200 import binding
+    names = declared_symbols()
+    assert len(names) >= 15
+    for n in names:
+        assert hasattr(lib, n), "libmhd.so does not export %s" % n
+    assert sorted(binding.SYMBOLS) == names
+
+
+def test_init_argument_validation(lib):
+    h = C.c_void_p()
+    two_pi = 6.283185307179586
+    assert lib.mhd_init(C.byref(h), 48, two_pi, 5 / 3, 0.0, 0.0, 1e-3) == -1      # not a power of two
+    assert lib.mhd_init(C.byref(h), 8, two_pi, 5 / 3, 0.0, 0.0, 1e-3) == -1       # below the minimum
+    assert lib.mhd_init(C.byref(h), 2048, two_pi, 5 / 3, 0.0, 0.0, 1e-3) == -1    # above the maximum
+    assert lib.mhd_init(C.byref(h), 32, -1.0, 5 / 3, 0.0, 0.0, 1e-3) == -1
+    assert lib.mhd_init(C.byref(h), 32, two_pi, 1.0, 0.0, 0.0, 1e-3) == -1        # gamma must exceed 1
+    assert lib.mhd_init(C.byref(h), 32, two_pi, 5 / 3, -0.1, 0.0, 1e-3) == -1
+    assert lib.mhd_init(C.byref(h), 32, two_pi, 5 / 3, 0.0, 0.0, 0.0) == -1
+    assert lib.mhd_init(C.byref(h), 32, two_pi, 5 / 3, 0.01, 0.01, 1e-3) == 0 and h.value
+    # unbound context: every compute call refuses
+    assert lib.mhd_step(h, 1) == -2
+    ptrs = (C.c_void_p * 8)()
+    assert lib.mhd_rhs(h, 0, ptrs) == -2
+    assert lib.mhd_set_fields(h, 1, 0, ptrs) == -2
+    assert b"mhd_bind" in lib.mhd_last_error(h)
+    assert lib.mhd_set_option(h, 99, 0) == -1
+    assert lib.mhd_destroy(h) == 0
+
+
+def test_workspace_sizes(lib):
+    assert lib.mhd_workspace_bytes(48, 0) == 0
+    b32, b64 = lib.mhd_workspace_bytes(32, 0), lib.mhd_workspace_bytes(64, 0)
+    assert b32 >= 48 * 32 ** 3 * 8 and b64 >= 48 * 64 ** 3 * 8 and b64 < 9 * b32
+    # 512^3 must fit a B200's 180 GB with room to spare
+    assert lib.mhd_workspace_bytes(512, 0) < 80e9
+    assert lib.mhd_nspec(32) == 29 and lib.mhd_nspec(256) == 223
+
+
+def test_bind_without_device_fails_loudly(lib):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    h = C.c_void_p()
+    assert lib.mhd_init(C.byref(h), 16, 6.283185307179586, 5 / 3, 0.0, 0.0, 1e-3) == 0
+    n = lib.mhd_workspace_bytes(16, 0)
+    rc = lib.mhd_bind(h, C.c_void_p(256), n, None, 0, None, 0)
+    assert rc == -4 and b"no CUDA device" in lib.mhd_last_error(h)
+    lib.mhd_destroy(h)
+    from paper_1810_12707_b200 import MHD
+    with pytest.raises(RuntimeError):
+        MHD(16)

@@ -1,0 +1,376 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Run on the B200 box with `-m gpu`.
+
+Tolerances (north_star: rel. L2 <= 1e-12 per RHS, <= 1e-9 after
+100 steps).  Per field f of one RHS evaluation:
+  literal        rho_f  = |g - o|_2 / |o|_2                          <= 1e-12   (where |o|_2 is not ~0)
+  backward error beta_f = |g - o|_2 / (kc |Phi_f|_2 + kc^2 d_f)      <= 2e-15   (always; covers exactly
+                 cancelling fields such as R_rho of a uniform-density solenoidal flow)
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1810_12707_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+NAMES = ["rho", "mx", "my", "mz", "E", "Bx", "By", "Bz"]
+
+
+@pytest.fixture(scope="module")
+def MHD():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1810_12707_b200 import build, binding
+    build.build()
+    return binding.MHD
+
+
+def both(orc, MHD, cfg, opts=None):
+    o = orc.Oracle(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+    o.set_fields(cfg.prim, "primitive")
+    g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+    for k, v in (opts or {}).items():
+        g.set_option(k, v)
+    g.set_fields(cfg.prim, "primitive")
+    return o, g
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+def check_rhs(o, g, N, literal=1e-12, beta_tol=2e-15):
+    Ro, phi, dsc = o.rhs_scales()
+    Rg = g.rhs()
+    kc = N // 3
+    report = {}
+    for f in range(8):
+        err = float(np.linalg.norm(Rg[f] - Ro[f]))
+        scale = kc * phi[f] + kc * kc * dsc[f]
+        beta = err / max(scale, 1e-300)
+        rho = err / max(float(np.linalg.norm(Ro[f])), 1e-300)
+        report[NAMES[f]] = (rho, beta)
+        assert beta <= beta_tol, (NAMES[f], "beta", beta, report)
+        if np.linalg.norm(Ro[f]) > 1e-9 * max(scale, 1e-300):   # not an exactly cancelling field
+            assert rho <= literal, (NAMES[f], "rho", rho, report)
+    return report
+
+
+# ---------------------------------------------------------------------------------------------------------
+# 3-D FFT alone: in-house R2C / C2R against the oracle's own FFT
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N", [16, 32, 64, 128])
+def test_fft3d_matches_oracle(orc, MHD, N):
+    import torch
+    rng = np.random.default_rng(100 + N)
+    x = rng.standard_normal((2, N, N, N))
+    ref = [orc.fft3(x[i].astype(complex), -1) for i in range(2)]
+    g = MHD(N)
+    H = N // 2
+    real = [torch.from_numpy(x[i]).cuda() for i in range(2)]
+    spec = [torch.zeros((N, N, H, 2), dtype=torch.float64, device="cuda") for _ in range(2)]
+    nyq = [torch.zeros((N, N, 8, 2), dtype=torch.float64, device="cuda") for _ in range(2)]
+    g.fft3d_r2c(real, spec, nyq, prune=False)
+    for i in range(2):
+        s = spec[i].cpu().numpy()
+        got = s[..., 0] + 1j * s[..., 1]
+        assert rel_l2(got, ref[i][:, :, :H]) <= 1e-14
+        q = nyq[i].cpu().numpy()
+        gotn = q[:, :, 0, 0] + 1j * q[:, :, 0, 1]
+        assert rel_l2(gotn, ref[i][:, :, H]) <= 1e-14
+    # pruned transform: exactly the modes inside the 2/3 mask, nothing else written
+    spec_p = [torch.full((N, N, H, 2), 7.0, dtype=torch.float64, device="cuda") for _ in range(2)]
+    g.fft3d_r2c(real, spec_p, None, prune=True)
+    kc = N // 3
+    n = np.fft.fftfreq(N, 1.0 / N).astype(int)
+    inside = (np.abs(n)[:, None, None] <= kc) & (np.abs(n)[None, :, None] <= kc) & (np.arange(H)[None, None, :] <= kc)
+    for i in range(2):
+        s = spec_p[i].cpu().numpy()
+        got = s[..., 0] + 1j * s[..., 1]
+        assert rel_l2(got[inside], ref[i][:, :, :H][inside]) <= 1e-14
+    # C2R round trip of the band-limited part: equals the oracle's inverse of the masked spectrum
+    full = ref[0].copy()
+    m3 = (np.abs(n)[:, None, None] <= kc) & (np.abs(n)[None, :, None] <= kc) & (np.abs(n)[None, None, :] <= kc)
+    full[~m3] = 0
+    back_ref = orc.fft3(full, +1).real
+    out = [torch.empty((N, N, N), dtype=torch.float64, device="cuda")]
+    g.fft3d_c2r([spec_p[0]], out, prune=True)
+    assert rel_l2(out[0].cpu().numpy(), back_ref) <= 1e-14
+    # unpruned C2R of the full half spectrum (Nyquist dropped)
+    full = ref[1].copy()
+    full[:, :, H] = 0
+    back_ref = orc.fft3(full, +1).real
+    g.fft3d_c2r([spec[1]], out, prune=False)
+    assert rel_l2(out[0].cpu().numpy(), back_ref) <= 1e-14
+
+
+# ---------------------------------------------------------------------------------------------------------
+# one RHS evaluation
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("fused,prune", [(1, 1), (0, 1), (1, 0), (0, 0)])
+def test_rhs_random_state_32(orc, MHD, fused, prune):
+    from paper_1810_12707_b200 import binding as b
+    N = 32
+    cfg = inputs.Config("random", N, 2 * math.pi, 5 / 3, 0.01, 0.02, 1e-3, 1, inputs.random_smooth_state(N, 7, kmax=4))
+    o, g = both(orc, MHD, cfg, {b.MHD_OPT_FUSED: fused, b.MHD_OPT_PRUNE: prune})
+    check_rhs(o, g, N)
+
+
+@pytest.mark.parametrize("cfgname,N", [("1", 32), ("2", 64), ("3", 64), ("5", 64), ("1", 16), ("3", 128)])
+def test_rhs_configs(orc, MHD, cfgname, N):
+    cfg = inputs.by_name(cfgname, N)
+    o, g = both(orc, MHD, cfg)
+    rep = check_rhs(o, g, N)
+    print(cfgname, N, rep)
+
+
+def test_rhs_non_2pi_box(orc, MHD):
+    N = 32
+    prim = inputs.random_smooth_state(N, 11, kmax=3)
+    cfg = inputs.Config("box3", N, 3.0, 1.4, 0.02, 0.01, 1e-3, 1, prim)
+    o, g = both(orc, MHD, cfg)
+    check_rhs(o, g, N)
+
+
+def test_rhs_does_not_change_state(orc, MHD):
+    cfg = inputs.config1(32)
+    o, g = both(orc, MHD, cfg)
+    a = g.get_fields()
+    g.rhs()
+    g.rhs()
+    b = g.get_fields()
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+    assert g.diagnostics()["step"] == 0
+
+
+def test_device_pointers_match_host_pointers(orc, MHD):
+    import torch
+    cfg = inputs.config1(32)
+    g1 = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+    g1.set_fields(cfg.prim, "primitive")
+    g2 = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+    g2.set_fields([torch.from_numpy(p).cuda() for p in cfg.prim], "primitive")
+    r1 = g1.rhs("host")
+    r2 = g2.rhs("device")
+    for a, b in zip(r1, r2):
+        assert np.array_equal(a, b.cpu().numpy())
+    u1 = g1.get_fields("primitive", "host")
+    u2 = g2.get_fields("primitive", "device")
+    for a, b in zip(u1, u2):
+        assert np.array_equal(a, b.cpu().numpy())
+
+
+# ---------------------------------------------------------------------------------------------------------
+# state in/out and the dealias projection of set_fields
+# ---------------------------------------------------------------------------------------------------------
+def test_set_get_fields_and_projection(orc, MHD):
+    N = 32
+    prim = inputs.random_smooth_state(N, 5, kmax=5)       # products exceed kc = 10: the projection truncates
+    cfg = inputs.Config("proj", N, 2 * math.pi, 5 / 3, 0.0, 0.0, 1e-3, 1, prim)
+    o, g = both(orc, MHD, cfg)
+    for kind in ("conservative", "primitive"):
+        a, b = o.get_fields(kind), g.get_fields(kind)
+        for f in range(8):
+            assert rel_l2(b[f], a[f]) <= 1e-14, (kind, NAMES[f])
+
+
+# ---------------------------------------------------------------------------------------------------------
+# time stepping
+# ---------------------------------------------------------------------------------------------------------
+def test_config1_full_run_10_steps(orc, MHD):
+    cfg = inputs.config1(32)
+    o, g = both(orc, MHD, cfg)
+    o.step(cfg.nsteps)
+    g.step(cfg.nsteps)
+    a, b = o.get_fields(), g.get_fields()
+    for f in range(8):
+        assert rel_l2(b[f], a[f]) <= 1e-12, NAMES[f]
+    do, dg = o.diagnostics(), g.diagnostics()
+    assert dg["step"] == 10 and abs(dg["t"] - do["t"]) < 1e-15
+
+
+@pytest.mark.parametrize("cfgname,N", [("1", 32), ("2", 32), ("3", 32)])
+def test_100_steps(orc, MHD, cfgname, N):
+    cfg = inputs.by_name(cfgname, N) if cfgname != "3" else inputs.config3(N, kmax=6)
+    o, g = both(orc, MHD, cfg)
+    o.step(100)
+    g.step(100)
+    a, b = o.get_fields(), g.get_fields()
+    for f in range(8):
+        if np.linalg.norm(a[f]) == 0:
+            assert np.linalg.norm(b[f]) == 0
+            continue
+        assert rel_l2(b[f], a[f]) <= 1e-9, NAMES[f]
+
+
+def test_step_split_is_bitwise_and_step0_is_noop(orc, MHD):
+    cfg = inputs.config1(32)
+    _, g1 = both(orc, MHD, cfg)
+    g2 = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+    g2.set_fields(cfg.prim, "primitive")
+    g1.step(7)
+    g2.step(3); g2.step(0); g2.step(4)
+    for a, b in zip(g1.get_fields(), g2.get_fields()):
+        assert np.array_equal(a, b)
+
+
+def test_unfused_and_unpruned_paths_agree_over_steps(orc, MHD):
+    from paper_1810_12707_b200 import binding as b
+    cfg = inputs.config3(32, kmax=6)
+    ref = None
+    for fused, prune in [(1, 1), (0, 1), (1, 0)]:
+        g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+        g.set_option(b.MHD_OPT_FUSED, fused)
+        g.set_option(b.MHD_OPT_PRUNE, prune)
+        g.set_fields(cfg.prim, "primitive")
+        g.step(20)
+        U = g.get_fields()
+        if ref is None:
+            ref = U
+        else:
+            for f in range(8):
+                assert rel_l2(U[f], ref[f]) <= 1e-13, (fused, prune, NAMES[f])
+
+
+@pytest.mark.parametrize("integ", [1, 2])
+def test_other_integrators_agree_with_ab2(orc, MHD, integ):
+    # "all the solvers has been checked to provide identical results" — to truncation error
+    from paper_1810_12707_b200 import binding as b
+    cfg = inputs.config1(32)
+    g0 = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+    g0.set_fields(cfg.prim, "primitive")
+    g0.step(20)
+    g1 = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+    g1.set_option(b.MHD_OPT_INTEGRATOR, integ)
+    g1.set_fields(cfg.prim, "primitive")
+    g1.step(20)
+    for f, (a, c) in enumerate(zip(g0.get_fields(), g1.get_fields())):
+        assert rel_l2(c, a) <= 1e-7, NAMES[f]
+
+
+def test_rk4_alfven_wave_fourth_order(MHD):
+    # exact nonlinear circularly polarised Alfven wave (pin P8): RK4 error falls 16x per halving of dt
+    from paper_1810_12707_b200 import binding as b
+    N, r0, P0, B0, amp, k, T = 16, 1.0, 1.0, 1.0, 0.1, 1, 0.4
+    c = np.arange(N) * (2 * math.pi / N)
+    X = np.broadcast_to(c[None, None, :], (N, N, N))
+
+    def state(t):
+        ph = k * (X - B0 / math.sqrt(r0) * t)
+        b1, b2 = amp * np.cos(ph), amp * np.sin(ph)
+        one = np.ones((N, N, N))
+        return [r0 * one, 0 * one, -b1 / math.sqrt(r0), -b2 / math.sqrt(r0), P0 * one, B0 * one, b1, b2]
+
+    errs = []
+    for dt in (0.1, 0.05):
+        g = MHD(N, dt=dt)
+        g.set_option(b.MHD_OPT_INTEGRATOR, 1)
+        g.set_fields(state(0.0), "primitive")
+        g.step(int(round(T / dt)))
+        got, ref = g.get_fields("primitive"), state(T)
+        errs.append(max(float(np.max(np.abs(got[i] - ref[i]))) for i in range(8)))
+    assert 12.0 <= errs[0] / errs[1] <= 20.0, errs
+
+
+# ---------------------------------------------------------------------------------------------------------
+# diagnostics
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfgname,N", [("1", 32), ("2", 32), ("3", 64)])
+def test_diagnostics_match_oracle(orc, MHD, cfgname, N):
+    cfg = inputs.by_name(cfgname, N)
+    o, g = both(orc, MHD, cfg)
+    o.step(3)
+    g.step(3)
+    do, dg = o.diagnostics(spectra=True), g.diagnostics(spectra=True)
+    for key in ("ke", "me", "ie", "mass", "etot", "rho_min", "p_min"):
+        assert abs(dg[key] - do[key]) <= 1e-12 * abs(do[key]), key
+    mrms = math.sqrt(2 * do["ke"] * do["mass"])
+    for a, b in zip(do["mom"], dg["mom"]):
+        assert abs(a - b) <= 1e-13 * mrms
+    brms = math.sqrt(2 * do["me"])
+    assert dg["max_divb"] <= 1e-13 * (N // 3) * max(brms, 1e-30) + 1e-300
+    for key in ("spec_kin", "spec_mag"):
+        assert len(dg[key]) == len(do[key])
+        assert np.max(np.abs(dg[key] - do[key])) <= 1e-12 * np.max(do[key]), key
+    assert abs(dg["spec_kin"].sum() - dg["ke"]) <= 1e-12 * dg["ke"]
+    assert abs(dg["spec_mag"].sum() - dg["me"]) <= 1e-12 * dg["me"]
+
+
+# ---------------------------------------------------------------------------------------------------------
+# error behaviour at the boundary
+# ---------------------------------------------------------------------------------------------------------
+def test_errors(MHD):
+    g = MHD(16)
+    with pytest.raises(RuntimeError, match="NO_FIELDS"):
+        g.step(1)
+    with pytest.raises(RuntimeError, match="NO_FIELDS"):
+        g.rhs()
+    with pytest.raises(RuntimeError, match="INVALID_ARG"):
+        g.set_option(3, 7)
+    assert g.launch_count() >= 1
+
+
+# ---------------------------------------------------------------------------------------------------------
+# full bench sizes, in the launch configuration bench.py times (fused + pruned, 256^3 and 512^3):
+#   (a) closed forms (pins P4 / P8 evaluated at full size),
+#   (b) resolution independence: the configs are band-limited far below kc of a 64^3 grid, so the RHS on the
+#       big grid, sub-sampled, must equal the ORACLE's RHS on the 64^3 grid,
+#   (c) invariants after steps: mass / momentum / energy conservation, div B.
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N", [256, 512])
+def test_full_size_rhs_against_oracle_subsampled(orc, MHD, N):
+    big = inputs.config45(N)
+    small = inputs.config45(64)
+    o = orc.Oracle(64, small.L, small.gamma, small.mu, small.eta, small.dt)
+    o.set_fields(small.prim, "primitive")
+    Ro, phi, dsc = o.rhs_scales()
+    g = MHD(N, big.L, big.gamma, big.mu, big.eta, big.dt)
+    g.set_fields(big.prim, "primitive")
+    Rg = g.rhs()
+    s = N // 64
+    kc = N // 3
+    for f in range(8):
+        sub = Rg[f][::s, ::s, ::s]
+        err = float(np.linalg.norm(sub - Ro[f]))
+        # conditioning of the big-grid evaluation (kc of the big grid), norms taken over the sampled points
+        beta = err / (kc * phi[f] + kc * kc * dsc[f])
+        assert beta <= 2e-15, (NAMES[f], beta)
+    del Rg
+    # invariants over 10 steps
+    d0 = g.diagnostics()
+    g.step(10)
+    d1 = g.diagnostics()
+    assert abs(d1["mass"] - d0["mass"]) <= 1e-13 * d0["mass"]
+    assert abs(d1["etot"] - d0["etot"]) <= 1e-13 * d0["etot"]
+    assert d1["max_divb"] <= 1e-13 * kc * math.sqrt(2 * d1["me"])
+    assert abs(d0["ke"] - 1.5) <= 1e-12 and abs(d0["ie"] - 90.0) <= 1e-10 and abs(d0["me"] - 5e-9) <= 1e-20
+
+
+@pytest.mark.parametrize("N", [256])
+def test_full_size_abc_closed_form(MHD, N):
+    U0, P0, mu = 0.7, 2.0, 0.013
+    c = np.arange(N) * (2 * math.pi / N)
+    X, Y, Z = c[None, None, :], c[None, :, None], c[:, None, None]
+    sx, cx, sy, cy, sz, cz = np.sin(X), np.cos(X), np.sin(Y), np.cos(Y), np.sin(Z), np.cos(Z)
+    shape = (N, N, N)
+    u = [np.ascontiguousarray(np.broadcast_to(a, shape)) for a in (U0 * (sz + cy), U0 * (sx + cz), U0 * (sy + cx))]
+    one = np.ones(shape)
+    g = MHD(N, mu=mu, eta=0.02)
+    g.set_fields([one, u[0], u[1], u[2], P0 * one, 0 * one, 0 * one, 0 * one], "primitive")
+    R = g.rhs()
+    gq = [U0 ** 2 * (cx * cz - sy * sx), U0 ** 2 * (-sz * sy + cy * cx), U0 ** 2 * (cz * cy - sx * sz)]
+    q = U0 ** 2 * (1.5 + sz * cy + sx * cz + sy * cx)
+    kc = N // 3
+    # absolute error bound: kc * |flux| * eps  with |flux| ~ P0 + E ~ 5
+    tol = 2e-15 * kc * 5.0 * 10
+    assert np.max(np.abs(R[0])) <= tol
+    for i in range(3):
+        assert np.max(np.abs(R[1 + i] - (-gq[i] - mu * u[i]))) <= tol
+    RE = -(u[0] * gq[0] + u[1] * gq[1] + u[2] * gq[2]) - 2 * mu * (q - 1.5 * U0 ** 2)
+    assert np.max(np.abs(R[4] - RE)) <= tol
+    for i in range(3):
+        assert np.max(np.abs(R[5 + i])) == 0.0
