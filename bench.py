@@ -1,0 +1,368 @@
+#!/usr/bin/env python
+"""bench.py — fp64 grid-point-steps/s of the MHD step (BASELINE.json metric) on B200, one JSON line.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--size 512] [--impl ours|reference]
+
+A "step" is one explicit time step (one pass of the whole hot path: sweeps S1-S5) of the 512^3 ABC-dynamo
+config of BASELINE.json (config 5; `--size 256` gives config 4).  Inputs are seeded and synthetic.
+  value        N^3 * K * n_gpus / (max over ranks of the device time of mhd_step(K)), state resident in HBM
+  e2e          same metric through the C ABI with HOST (pinned) buffers: set_fields + step(K) + get_fields
+  roofline     dominant kernel family: algorithmic bytes per launch / CUDA-event time, vs measured HBM peak
+  cpu_baseline the CPU oracle, as it stands, on a bounded sample (64^3 grid of the same config)
+Multi-GPU: the path does not shard without an all-to-all: `--gpus N` runs N independent
+replicas (weak scaling), one process per GPU under torchrun, timed as the max over ranks.
+`--impl reference` times the oracle (the reference arm of this tier) on the host cores of rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64 grid-point-steps/s"
+UNIT = "grid-point-steps/s"
+FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# clocks during the timed region (profiling recipe)
+# ----------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index = index
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.FIELDS,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            self.proc = None
+        return self
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except Exception:
+            self.proc.kill()
+            out = ""
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            p = [x.strip() for x in line.split(",")]
+            if len(p) < 7:
+                continue
+            try:
+                sm.append(float(p[0])); mx.append(float(p[1]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, p[3:7]):
+                if val.lower() == "active":
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# distributed plumbing (one process per GPU; replicas only)
+# ----------------------------------------------------------------------------------------------------------------
+def dist_env():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+def aggregate(ms_local: float, units_local: float, dist=None):
+    """max-over-ranks time and summed work: (ms_max, units_total).  `dist` = torch.distributed or None."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return ms_local, units_local
+    import torch
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([ms_local], dtype=torch.float64, device=dev)
+    u = torch.tensor([units_local], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# algorithmic bytes per launch; one field-sweep = 8 B per grid point
+# ----------------------------------------------------------------------------------------------------------------
+def sweep_bytes(N: int, prune: bool):
+    """Per-family algorithmic bytes of ONE right-hand side: what the kernels must read + write."""
+    kc = N // 3
+    H = N // 2
+    a = (2 * kc + 1) / N if prune else 1.0          # kept fraction of a full axis
+    ah = (kc + 1) / H if prune else 1.0             # kept fraction of the stored half axis
+    f = 8.0 * N ** 3                                # bytes of one full field sweep
+    b = {}
+    b["build_current"] = (3 + 3) * f * ah * a * a
+    b["strided_inverse"] = 11 * f * ah * (a * a + a) + 11 * f * ah * (a + 1.0)       # z pass, y pass (read + write)
+    b["x_fused"] = (11 + 16) * f * ah
+    b["strided_forward"] = 16 * f * ah * (1.0 + a) + 16 * f * ah * (a + a * a)       # y pass, z pass
+    b["assemble"] = (16 + 8 + 8 + 8 + 8) * f * ah * a * a
+    return b
+
+
+def unpruned_reference_bytes(N: int) -> float:
+    """148 field-sweeps x 8 B = 1184 B per grid-point-step (fused, unpruned three-pass design)."""
+    return 1184.0 * N ** 3
+
+
+# ----------------------------------------------------------------------------------------------------------------
+def run_reference(args):
+    """Reference arm of this tier = the CPU oracle, as it stands, on a bounded sample of the workload."""
+    rank, _, world = dist_env()
+    if rank != 0:
+        return 0
+    import oracle
+    from paper_1810_12707_b200 import inputs
+    n = 64
+    cfg = inputs.config45(n)
+    o = oracle.Oracle(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+    o.set_fields(cfg.prim, "primitive")
+    for _ in range(args.warmup):
+        o.step(1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.step(1)
+    dt = time.perf_counter() - t0
+    value = n ** 3 * args.steps / dt
+    cores = oracle.get_threads()
+    sample = "config 4/5 initial condition on a 64^3 grid, %d AB2 steps (bounded sample of the %d^3 workload)" % (args.steps, args.size)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "config5_abc_dynamo_%d" % args.size, "reference_grid": n, "integrator": "AB2"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def cpu_baseline(size):
+    import oracle
+    from paper_1810_12707_b200 import inputs
+    n, steps = 64, 12
+    cfg = inputs.config45(n)
+    o = oracle.Oracle(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+    o.set_fields(cfg.prim, "primitive")
+    o.step(1)
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    return {"value": n ** 3 * steps / dt, "unit": UNIT, "cores": oracle.get_threads(), "kind": "oracle",
+            "sample": "config 4/5 initial condition on a 64^3 grid, %d AB2 steps, %.1f s (bounded sample of the %d^3 workload)"
+                      % (steps, dt, size)}
+
+
+def time_steps(g, torch, nsteps, dist):
+    """Device time of mhd_step(nsteps) on the solver's stream, barrier + synchronize on both sides."""
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(g.stream)
+    g.step(nsteps)
+    e1.record(g.stream)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    return e0.elapsed_time(e1)
+
+
+def fft_metric(g, torch, N, nf=8, reps=5):
+    """Stand-alone batched 3-D R2C + C2R (BASELINE.json: '3D FFT achieved HBM GB/s vs peak')."""
+    H = N // 2
+    real = [torch.randn((N, N, N), dtype=torch.float64, device=g.device) for _ in range(nf)]
+    spec = [torch.empty((N, N, H, 2), dtype=torch.float64, device=g.device) for _ in range(nf)]
+    out = {}
+    for prune in (False, True):
+        for name, fn in (("r2c", lambda: g.fft3d_r2c(real, spec, None, prune)), ("c2r", lambda: g.fft3d_c2r(spec, real, prune))):
+            fn(); fn()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(g.stream)
+            for _ in range(reps):
+                fn()
+            e1.record(g.stream)
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / reps
+            out[name + ("_pruned" if prune else "")] = {"ms_per_field": ms / nf,
+                                                         "gbs_3pass_48B_per_pt": 48.0 * N ** 3 * nf / ms / 1e6,
+                                                         "gbs_1r1w_16B_per_pt": 16.0 * N ** 3 * nf / ms / 1e6}
+    # cuFFT (via torch.fft) as a timing reference only — never on the product path
+    x = real[0]
+    torch.fft.rfftn(x); torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        y = torch.fft.rfftn(x)
+    e1.record()
+    torch.cuda.synchronize()
+    out["cufft_d2z_reference_ms_per_field"] = e0.elapsed_time(e1) / reps
+    del y, real, spec
+    return out
+
+
+def run_ours(args):
+    rank, local_rank, world = dist_env()
+    import torch
+    if not torch.cuda.is_available():
+        print(json.dumps({"error": "no CUDA device; the product path has no CPU fallback"}))
+        return 2
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        dist = dist_mod
+    from paper_1810_12707_b200 import build as mhd_build
+    if rank == 0:
+        mhd_build.build()
+    if dist is not None:
+        dist.barrier()
+    from paper_1810_12707_b200 import MHD, inputs
+
+    N = args.size
+    cfg = inputs.config45(N)
+    g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, device="cuda:%d" % local_rank)
+    host = [torch.from_numpy(p).pin_memory() for p in cfg.prim]      # pinned host inputs
+    cfg.prim = None
+    g.set_fields(host, "primitive")
+    K, W = args.steps, max(args.warmup, 3)
+
+    # ---- device-resident timing -----------------------------------------------------------------------------
+    g.step(W)
+    sampler = ClockSampler(local_rank).start()
+    g.profile_enable(True)
+    l0 = g.launch_count()
+    ms = time_steps(g, torch, K, dist)
+    launches = g.launch_count() - l0
+    prof = g.profile_get()
+    g.profile_enable(False)
+    clocks = sampler.stop()
+    ms_max, units = aggregate(ms, float(N) ** 3 * K, dist)
+    value = units / (ms_max * 1e-3)
+
+    # ---- roofline of the dominant kernel family ---------------------------------------------------------------
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(peaks_path):
+        peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    else:
+        peak, peak_src = FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+    sb = sweep_bytes(N, prune=True)
+    fam = {}
+    for name, b in sb.items():
+        p = prof.get(name, {"ms": 0.0, "launches": 0})
+        if p["launches"] == 0:
+            continue
+        per_launch_bytes = b * K / p["launches"]
+        avg_ms = p["ms"] / p["launches"]
+        fam[name] = {"ms_per_step": p["ms"] / K, "launches_per_step": p["launches"] / K,
+                     "alg_bytes_per_launch": per_launch_bytes, "avg_launch_ms": avg_ms,
+                     "gbs": per_launch_bytes / avg_ms / 1e6, "frac_of_peak": per_launch_bytes / avg_ms / 1e6 / peak}
+    dom = max(fam, key=lambda k: fam[k]["ms_per_step"]) if fam else None
+    step_ms_local = ms / K
+    alg_pruned = sum(sb.values())
+    roofline = None
+    if dom:
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": fam[dom]["gbs"], "peak": peak, "unit": "GB/s",
+                    "frac": fam[dom]["frac_of_peak"], "traffic": None, "peak_source": peak_src,
+                    "share_of_step": fam[dom]["ms_per_step"] / step_ms_local,
+                    "whole_step": {"alg_bytes_pruned": alg_pruned, "gbs_pruned": alg_pruned / step_ms_local / 1e6,
+                                   "frac_pruned": alg_pruned / step_ms_local / 1e6 / peak,
+                                   "alg_bytes_unpruned_1184B": unpruned_reference_bytes(N),
+                                   "gbs_vs_1184B": unpruned_reference_bytes(N) / step_ms_local / 1e6,
+                                   "frac_vs_1184B": unpruned_reference_bytes(N) / step_ms_local / 1e6 / peak,
+                                   "frac_vs_1184B_nominal_8TBs": unpruned_reference_bytes(N) / step_ms_local / 1e6 / 8000.0},
+                    "families": fam}
+        tpath = os.path.join(ROOT, "profiles", "traffic_r01.json")
+        if os.path.exists(tpath):   # DRAM bytes per launch from the committed ncu --set full capture
+            try:
+                roofline["traffic"] = json.load(open(tpath)).get(str(N), {}).get(dom)
+            except Exception:
+                pass
+
+    # ---- end to end through the C ABI with host buffers ----------------------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        outh = host   # results land in the same pinned buffers
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        g.set_fields(host, "primitive")
+        g.step(K)
+        g.get_fields("primitive", "host", out=outh)
+        torch.cuda.synchronize()
+        t_e2e = (time.perf_counter() - t0) * 1e3
+        ms_e, units_e = aggregate(t_e2e, float(N) ** 3 * K, dist)
+        fb = 8.0 * N ** 3 * 8
+        e2e = {"value": units_e / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": fb / K, "d2h_bytes_per_step": fb / K,
+               "what": "mhd_set_fields(pinned host) + mhd_step(%d) + mhd_get_fields(pinned host), wall clock" % K}
+
+    extra = {}
+    if rank == 0 and not args.no_fft:
+        del host
+        extra["fft3d"] = fft_metric(g, torch, N)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        cpu = cpu_baseline(N)
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+                "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": "config%d_abc_dynamo_%d^3" % (5 if N == 512 else 4, N), "N": N, "dt": cfg.dt,
+                           "mu": cfg.mu, "eta": cfg.eta, "integrator": "AB2", "fused": 1, "pruned": 1,
+                           "parallelism": "replicas x%d" % world,
+                           "l2": "no flush: one step streams %.1f GB, far beyond the 126 MB L2" % (alg_pruned / 1e9)},
+                "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+                "paper_context": {"256^3 s/step P100/V100": [0.32, 0.22], "512^3 s/step P100/V100 (out-of-core)": [80.97, 92.81],
+                                  "source": "PAPER.md Table III L368-375; other hardware, context only"}}
+        line.update(extra)
+        print(json.dumps(line))
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--size", type=int, default=512, choices=[64, 128, 256, 512])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-fft", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -53,7 +53,8 @@ extern "C" {
 #define MHD_FLAG_OUT_OF_CORE 1u /* field storage in pinned host memory, slabs streamed (Sec. VII-C) */
 
 /* options for mhd_set_option() */
-#define MHD_OPT_FUSED 1      /* 1 (default): fused kernels; 0: one kernel per step of the path (debug/bisect)  */
+#define MHD_OPT_FUSED 1      /* 1 (default): fused kernels; 2: first-generation fused x sweep;
+                                0: one kernel per step of the path (debug / bisect)                            */
 #define MHD_OPT_PRUNE 2      /* 1 (default): skip pencils the 2/3 mask makes identically zero; 0: full sweeps  */
 #define MHD_OPT_INTEGRATOR 3 /* 0 (default): Adams-Bashforth 2 with Euler start; 1: RK4; 2: predictor-corrector
                                 (Table I; R6)                                 */

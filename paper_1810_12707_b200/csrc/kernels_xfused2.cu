@@ -1,0 +1,223 @@
+// kernels_xfused2.cu — sweep S3, second generation: the fused real-axis kernel for N = 128, 256, 512.
+//
+// Per (y,z) line: C2R of 11 half-spectrum lines, 16 flux products, R2C of the 16 products.  Compared with the
+// generic tile version (kernels_x.cu) this kernel
+//   * maps lanes along the ROW index (t fastest): every quarter-warp reads / writes one full 128-byte line of one
+//     field straight from / to global memory, E = 2*R0 independent 16-byte loads in flight per thread;
+//   * folds the real-FFT split (C2R) and merge (R2C) into registers: the H-point transform is two stages
+//     H = R0 x R1; thread t owns the first-stage butterflies j = t and j = R1 - t (t = 0: j = 0 and R1/2), whose
+//     input rows j + r*R1 are exactly each other's mirror images k <-> H-k, so X[k], X[H-k] pairs meet in one thread;
+//   * therefore moves 108 instead of 162 line-passes through shared memory per line (33 inverse, 27 point-wise,
+//     48 forward) — shared-memory wavefronts were the largest term of the first version (ncu: profiles/);
+//   * skips the arithmetic of the 5 idle slots of the inverse transform at warp granularity.
+// The tile is [row][16 slots] with the slot XOR-swizzled by (row ^ row>>1 ^ row>>4) & 7, found by exhaustive search
+// to make every scatter / gather / point-wise access of the H = 128 and H = 256 plans bank-conflict free.
+#include "fft_core.cuh"
+#include "kernels.h"
+#include "physics.cuh"
+
+namespace mhd {
+
+template <int H> struct FPlan;
+template <> struct FPlan<64>  { static constexpr int R0 = 8,  R1 = 8;  };
+template <> struct FPlan<128> { static constexpr int R0 = 8,  R1 = 16; };
+template <> struct FPlan<256> { static constexpr int R0 = 16, R1 = 16; };
+
+template <int H> struct F2 {
+    static constexpr int R0 = FPlan<H>::R0, R1 = FPlan<H>::R1;
+    static constexpr int T = R1 / 2;            // threads per slot
+    static constexpr int NB = 2 * R0 / R1;      // radix-R1 butterflies per thread
+    static constexpr int THREADS = 16 * T;
+    static constexpr size_t SMEM = size_t(H) * 16 * sizeof(cd);
+    static_assert(R0 * R1 == H, "two-stage plan");
+};
+
+template <int H> __device__ __forceinline__ int swz(int row) {
+    if constexpr (H == 64) return (row ^ (row >> 1) ^ (row >> 2)) & 7;
+    else return (row ^ (row >> 1) ^ (row >> 4)) & 7;
+}
+template <int H> __device__ __forceinline__ int tidx(int row, int slot) { return row * 16 + (slot ^ swz<H>(row)); }
+
+// C2R split of one mirror pair: A = X[k], B = X[H-k], w = exp(-2 pi i k/N):  Z'[k] -> A, Z'[H-k] -> B (scaled)
+__device__ __forceinline__ void c2r_pair(cd& A, cd& B, cd w, double scale) {
+    const double Sx = A.x + B.x, Sy = A.y - B.y;
+    const double Dx = A.x - B.x, Dy = A.y + B.y;
+    const double p = w.x * Dx + w.y * Dy, q = w.x * Dy - w.y * Dx;
+    A = mk(scale * (Sx - q), scale * (Sy + p));
+    B = mk(scale * (Sx + q), scale * (p - Sy));
+}
+// R2C merge of one mirror pair: Zk = Z[k], Zm = Z[H-k]:  X[k] -> Zk, X[H-k] -> Zm
+__device__ __forceinline__ void r2c_pair(cd& Zk, cd& Zm, cd w) {
+    const double Sx = Zk.x + Zm.x, Sy = Zk.y - Zm.y;
+    const double Dx = Zk.x - Zm.x, Dy = Zk.y + Zm.y;
+    const double gx = w.x * Dx - w.y * Dy, gy = w.x * Dy + w.y * Dx;
+    Zk = mk(0.5 * (Sx + gy), 0.5 * (Sy - gx));
+    Zm = mk(0.5 * (Sx - gy), -0.5 * (Sy + gx));
+}
+
+template <int N>
+__global__ void __launch_bounds__(F2<N / 2>::THREADS, (N / 2 == 256) ? 2 : 4)
+x_fused2_kernel(const __grid_constant__ FusedXArgs a) {
+    constexpr int H = N / 2;
+    typedef F2<H> P;
+    constexpr int R0 = P::R0, R1 = P::R1, T = P::T, NB = P::NB, NT = P::THREADS;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cd* sm = reinterpret_cast<cd*>(smem_raw);
+    const cd* __restrict__ tw = a.tw;
+
+    const int t = threadIdx.x % T, slot = threadIdx.x / T;
+    const long long off = (long long)blockIdx.x * H;
+    const int jA = t, jB = (t == 0) ? R1 / 2 : R1 - t;
+
+    // ================= inverse: 11 lines, global -> registers -> tile =========================================
+    if (slot < S_NIN) {
+        const cd* __restrict__ line = a.in[slot] + off;
+        const int kmax = a.kmax_in;
+        const double scale = a.scale;
+        cd xa[R0], xb[R0];
+#pragma unroll
+        for (int r = 0; r < R0; ++r) {
+            const int ka = jA + r * R1, kb = jB + r * R1;
+            xa[r] = (ka <= kmax) ? line[ka] : mk(0.0, 0.0);
+            xb[r] = (kb <= kmax) ? line[kb] : mk(0.0, 0.0);
+        }
+        if (t != 0) {
+#pragma unroll
+            for (int r = 0; r < R0; ++r) c2r_pair(xa[r], xb[R0 - 1 - r], __ldg(&tw[jA + r * R1]), scale);
+        } else {
+            // rows r*R1: r = 0 is the mean mode (its mirror is the dropped Nyquist mode), r = R0/2 is k = H/2
+            xa[0] = mk(scale * xa[0].x, scale * xa[0].x);
+            xa[R0 / 2] = mk(2.0 * scale * xa[R0 / 2].x, -2.0 * scale * xa[R0 / 2].y);
+#pragma unroll
+            for (int r = 1; r < R0 / 2; ++r) c2r_pair(xa[r], xa[R0 - r], __ldg(&tw[r * R1]), scale);
+#pragma unroll
+            for (int r = 0; r < R0 / 2; ++r) c2r_pair(xb[r], xb[R0 - 1 - r], __ldg(&tw[R1 / 2 + r * R1]), scale);
+        }
+        Dft<R0, +1>::run(xa);
+        Dft<R0, +1>::run(xb);
+#pragma unroll
+        for (int q = 0; q < R0; ++q) {
+            sm[tidx<H>(jA * R0 + q, slot)] = xa[q];
+            sm[tidx<H>(jB * R0 + q, slot)] = xb[q];
+        }
+    }
+    __syncthreads();
+    {
+        cd u[NB][R1];
+        if (slot < S_NIN) {
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+                const int j = t + b * T;
+#pragma unroll
+                for (int r = 0; r < R1; ++r) u[b][r] = sm[tidx<H>(j + r * R0, slot)];
+#pragma unroll
+                for (int r = 1; r < R1; ++r) u[b][r] = twmul<+1>(u[b][r], __ldg(&tw[2 * r * j]));
+                Dft<R1, +1>::run(u[b]);
+            }
+        }
+        __syncthreads();
+        if (slot < S_NIN) {
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+                const int j = t + b * T;
+#pragma unroll
+                for (int q = 0; q < R1; ++q) sm[tidx<H>(j + q * R0, slot)] = u[b][q];
+            }
+        }
+    }
+    __syncthreads();
+
+    // ================= point-wise products: row n holds (f(x=2n), f(x=2n+1)) of every field ===================
+#pragma unroll 1
+    for (int n = threadIdx.x; n < H; n += NT) {
+        double s0[S_NIN], s1[S_NIN], o0[P_NOUT], o1[P_NOUT];
+#pragma unroll
+        for (int f = 0; f < S_NIN; ++f) {
+            const cd z = sm[tidx<H>(n, f)];
+            s0[f] = z.x; s1[f] = z.y;
+        }
+        flux_point(s0, o0, a.ph);
+        flux_point(s1, o1, a.ph);
+#pragma unroll
+        for (int f = 0; f < P_NOUT; ++f) sm[tidx<H>(n, f)] = mk(o0[f], o1[f]);
+    }
+    __syncthreads();
+
+    // ================= forward: 16 lines, tile -> registers -> global ==========================================
+    {
+        cd u[NB][R1];
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            const int j = t + b * T;
+#pragma unroll
+            for (int r = 0; r < R1; ++r) u[b][r] = sm[tidx<H>(j + r * R0, slot)];
+            Dft<R1, -1>::run(u[b]);
+        }
+        __syncthreads();
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            const int j = t + b * T;
+#pragma unroll
+            for (int q = 0; q < R1; ++q) sm[tidx<H>(j * R1 + q, slot)] = u[b][q];
+        }
+    }
+    __syncthreads();
+    {
+        cd* __restrict__ line = a.out[slot] + off;
+        const int kmax = a.kmax_out;
+        cd za[R0], zb[R0];
+#pragma unroll
+        for (int r = 0; r < R0; ++r) {
+            za[r] = sm[tidx<H>(jA + r * R1, slot)];
+            zb[r] = sm[tidx<H>(jB + r * R1, slot)];
+        }
+#pragma unroll
+        for (int r = 1; r < R0; ++r) {
+            za[r] = twmul<-1>(za[r], __ldg(&tw[2 * r * jA]));
+            zb[r] = twmul<-1>(zb[r], __ldg(&tw[2 * r * jB]));
+        }
+        Dft<R0, -1>::run(za);
+        Dft<R0, -1>::run(zb);
+        // za[q] = Z[jA + q*R1], zb[q] = Z[jB + q*R1]
+        if (t != 0) {
+#pragma unroll
+            for (int q = 0; q < R0; ++q) r2c_pair(za[q], zb[R0 - 1 - q], __ldg(&tw[jA + q * R1]));
+        } else {
+            za[0] = mk(za[0].x + za[0].y, 0.0);                         // k = 0 (Nyquist partner dropped)
+            za[R0 / 2] = mk(za[R0 / 2].x, -za[R0 / 2].y);               // k = H/2
+#pragma unroll
+            for (int q = 1; q < R0 / 2; ++q) r2c_pair(za[q], za[R0 - q], __ldg(&tw[q * R1]));
+#pragma unroll
+            for (int q = 0; q < R0 / 2; ++q) r2c_pair(zb[q], zb[R0 - 1 - q], __ldg(&tw[R1 / 2 + q * R1]));
+        }
+#pragma unroll
+        for (int q = 0; q < R0; ++q) {
+            const int ka = jA + q * R1, kb = jB + q * R1;
+            if (ka <= kmax) line[ka] = za[q];
+            if (kb <= kmax) line[kb] = zb[q];
+        }
+    }
+}
+
+template <int N> static void fused2_one(const FusedXArgs& a, cudaStream_t st) {
+    typedef F2<N / 2> P;
+    static bool cfg = false;
+    if (!cfg) {
+        cudaFuncSetAttribute(x_fused2_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::SMEM);
+        cfg = true;
+    }
+    x_fused2_kernel<N><<<(unsigned)a.nlines, P::THREADS, P::SMEM, st>>>(a);
+}
+
+bool x_fused2_supported(int N) { return N == 128 || N == 256 || N == 512; }
+
+void launch_x_fused2(int N, const FusedXArgs& a, cudaStream_t st) {
+    switch (N) {
+        case 128: fused2_one<128>(a, st); break;
+        case 256: fused2_one<256>(a, st); break;
+        case 512: fused2_one<512>(a, st); break;
+        default: break;
+    }
+}
+
+}  // namespace mhd

@@ -217,7 +217,8 @@ void products(mhd_ctx* c, cd* const Uin[8]) {
         for (int f = 0; f < 16; ++f) a.out[f] = c->W[f];
         a.tw = c->tw; a.nlines = (long long)N * N; a.kmax_in = kmax; a.kmax_out = kmax; a.scale = scale; a.ph = ph;
         mhd_ctx::Scope s(c, F_X_FUSED);
-        launch_x_fused(N, a, c->st);
+        if (c->opt_fused == 1 && x_fused2_supported(N)) launch_x_fused2(N, a, c->st);
+        else launch_x_fused(N, a, c->st);
     } else {
         XArgs a; std::memset(&a, 0, sizeof(a));
         for (int f = 0; f < 11; ++f) { a.spec_in[f] = c->W[f]; a.real_out[f] = reinterpret_cast<double*>(c->W[f]); }
@@ -325,7 +326,9 @@ int mhd_bind(mhd_ctx* c, void* dev_workspace, size_t bytes, void* cuda_stream, u
 int mhd_set_option(mhd_ctx* c, int option, int value) {
     if (!c) return MHD_ERR_INVALID_ARG;
     switch (option) {
-        case MHD_OPT_FUSED: c->opt_fused = value ? 1 : 0; return MHD_OK;
+        case MHD_OPT_FUSED:
+            if (value < 0 || value > 2) return c->fail(MHD_ERR_INVALID_ARG, "fused must be 0, 1 or 2");
+            c->opt_fused = value; return MHD_OK;
         case MHD_OPT_PRUNE: c->opt_prune = value ? 1 : 0; return MHD_OK;
         case MHD_OPT_INTEGRATOR:
             if (value < 0 || value > 2) return c->fail(MHD_ERR_INVALID_ARG, "integrator must be 0, 1 or 2");

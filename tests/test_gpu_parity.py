@@ -110,7 +110,18 @@ def test_fft3d_matches_oracle(orc, MHD, N):
 # ---------------------------------------------------------------------------------------------------------
 # one RHS evaluation
 # ---------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("fused,prune", [(1, 1), (0, 1), (1, 0), (0, 0)])
+@pytest.mark.parametrize("fused,prune", [(1, 1), (2, 1), (1, 0), (2, 0)])
+def test_rhs_random_state_128_both_fused_kernels(orc, MHD, fused, prune):
+    # N = 128 is the smallest size served by the second-generation fused x sweep (fused = 1); fused = 2 forces
+    # the first-generation tile kernel
+    from paper_1810_12707_b200 import binding as b
+    N = 128
+    cfg = inputs.Config("random", N, 2 * math.pi, 5 / 3, 0.01, 0.02, 1e-3, 1, inputs.random_smooth_state(N, 9, kmax=6))
+    o, g = both(orc, MHD, cfg, {b.MHD_OPT_FUSED: fused, b.MHD_OPT_PRUNE: prune})
+    check_rhs(o, g, N)
+
+
+@pytest.mark.parametrize("fused,prune", [(1, 1), (0, 1), (1, 0), (0, 0), (2, 1)])
 def test_rhs_random_state_32(orc, MHD, fused, prune):
     from paper_1810_12707_b200 import binding as b
     N = 32
