@@ -54,6 +54,39 @@ template <int R, int K, int DIR> __device__ __forceinline__ cd mul_root(cd a) {
     }
 }
 
+// a * exp(DIR * 2*pi*i * K32/32) for any compile-time K32 in [0, 32): constant 32nd roots of unity
+template <int K32, int DIR> __device__ __forceinline__ cd mul_root32(cd a) {
+    constexpr double C[16] = {1.0, 0.98078528040323044913, 0.92387953251128675613, 0.83146961230254523708,
+                              0.70710678118654752440, 0.55557023301960222474, 0.38268343236508977173,
+                              0.19509032201612826785, 0.0, -0.19509032201612826785, -0.38268343236508977173,
+                              -0.55557023301960222474, -0.70710678118654752440, -0.83146961230254523708,
+                              -0.92387953251128675613, -0.98078528040323044913};
+    constexpr double S[16] = {0.0, 0.19509032201612826785, 0.38268343236508977173, 0.55557023301960222474,
+                              0.70710678118654752440, 0.83146961230254523708, 0.92387953251128675613,
+                              0.98078528040323044913, 1.0, 0.98078528040323044913, 0.92387953251128675613,
+                              0.83146961230254523708, 0.70710678118654752440, 0.55557023301960222474,
+                              0.38268343236508977173, 0.19509032201612826785};
+    constexpr int K = ((K32 % 32) + 32) % 32;
+    if constexpr (K >= 16) {
+        const cd b = mul_root32<K - 16, DIR>(a);
+        return mk(-b.x, -b.y);
+    } else if constexpr (K == 0) {
+        return a;
+    } else if constexpr (K == 8) {
+        return (DIR < 0) ? mk(a.y, -a.x) : mk(-a.y, a.x);
+    } else {
+        constexpr double wr = C[K];
+        constexpr double wi = (DIR < 0) ? -S[K] : S[K];
+        if constexpr (K == 4) return mk(wr * (a.x + ((DIR < 0) ? a.y : -a.y)), wr * (a.y + ((DIR < 0) ? -a.x : a.x)));
+        else return mk(fma(a.x, wr, -(a.y * wi)), fma(a.x, wi, a.y * wr));
+    }
+}
+// a * exp(DIR * 2*pi*i * K/R), R in {2,4,8,16,32}, any integer K >= 0
+template <int R, int K, int DIR> __device__ __forceinline__ cd mul_rootN(cd a) {
+    static_assert(32 % R == 0, "R must divide 32");
+    return mul_root32<(K % R) * (32 / R), DIR>(a);
+}
+
 // In-register DFT of R points, natural order in and out:  v[q] <- sum_r v[r] exp(DIR*2*pi*i*r*q/R)
 template <int R, int DIR> struct Dft;
 template <int DIR> struct Dft<1, DIR> {

@@ -63,7 +63,9 @@ struct FusedXArgs {
 void launch_x_fused(int N, const FusedXArgs& a, cudaStream_t st);
 // second-generation fused sweep (kernels_xfused2.cu): N = 128, 256, 512
 bool x_fused2_supported(int N);
-void launch_x_fused2(int N, const FusedXArgs& a, cudaStream_t st);
+void launch_x_fused2(int N, const FusedXArgs& a, cudaStream_t st);   // a.tw = the lane-contiguous tables below
+int x_fused2_table_entries(int N);
+void launch_x_fused2_tables(int N, cd* tab, cudaStream_t st);
 
 // ---- point-wise kernels -------------------------------------------------------------------------------
 // real space: 11 fields in -> 16 product fields out (same slot order as FusedXArgs)

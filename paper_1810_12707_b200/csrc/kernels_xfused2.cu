@@ -16,6 +16,8 @@
 #include "kernels.h"
 #include "physics.cuh"
 
+#include <type_traits>
+
 namespace mhd {
 
 template <int H> struct FPlan;
@@ -38,6 +40,55 @@ template <int H> __device__ __forceinline__ int swz(int row) {
 }
 template <int H> __device__ __forceinline__ int tidx(int row, int slot) { return row * 16 + (slot ^ swz<H>(row)); }
 
+// Lane-contiguous twiddle tables (built once at bind time, exact sincospi): consecutive lanes t read consecutive
+// 16-byte entries, so one warp-wide twiddle load touches a single 128-byte line instead of up to 8 scattered ones
+// (ncu on the first cut of this kernel: 3.4x more L1 load sectors than data because of scattered table reads).
+//   TA[r][t] = exp(-2 pi i (jA(t) + r R1)/N)      split / merge factor of the rows of butterfly jA
+//   TB[r][t] = exp(-2 pi i (jB(t) + r R1)/N)      same for butterfly jB (used by t = 0 only)
+//   TS[b][r][t] = exp(-2 pi i r (t + b T)/H)      second inverse stage
+//   TF[w][r][t] = exp(-2 pi i r j_w(t)/H)         last forward stage, w = 0: jA, 1: jB
+template <int H> struct FTab {
+    typedef F2<H> P;
+    static constexpr int TA = 0;
+    static constexpr int TB = P::R0 * P::T;
+    static constexpr int TS = 2 * P::R0 * P::T;
+    static constexpr int TF = TS + H;
+    static constexpr int SIZE = TF + 2 * P::R0 * P::T;
+};
+
+template <int H> __global__ void fused_twiddle_kernel(cd* tab) {
+    typedef F2<H> P;
+    constexpr int R0 = P::R0, R1 = P::R1, T = P::T, NB = P::NB, N = 2 * H;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= FTab<H>::SIZE) return;
+    long long num; int den;
+    if (i < FTab<H>::TS) {                       // TA, TB
+        const int which = i / (R0 * T), r = (i % (R0 * T)) / T, t = i % T;
+        const int j = which == 0 ? t : (t == 0 ? R1 / 2 : R1 - t);
+        num = j + r * R1; den = N;
+    } else if (i < FTab<H>::TF) {                // TS
+        const int k = i - FTab<H>::TS, b = k / (R1 * T), r = (k % (R1 * T)) / T, t = k % T;
+        num = (long long)r * (t + b * T); den = H;
+        (void)NB;
+    } else {                                     // TF
+        const int k = i - FTab<H>::TF, which = k / (R0 * T), r = (k % (R0 * T)) / T, t = k % T;
+        const int j = which == 0 ? t : (t == 0 ? R1 / 2 : R1 - t);
+        num = (long long)r * j; den = H;
+        if (which == 0 && t == 0) { num = r; den = 2 * R0; }      // lane 0: exp(-2 pi i r/(2 R0)) = w_H^(r R1/2)
+    }
+    double sn, cs;
+    sincospi(2.0 * (double)(num % den) / (double)den, &sn, &cs);
+    tab[i] = mk(cs, -sn);
+}
+
+// compile-time loop: f(std::integral_constant<int, I>) for I = B .. E-1
+template <int B, int E, class F> __device__ __forceinline__ void static_for(F&& f) {
+    if constexpr (B < E) {
+        f(std::integral_constant<int, B>{});
+        static_for<B + 1, E>(f);
+    }
+}
+
 // C2R split of one mirror pair: A = X[k], B = X[H-k], w = exp(-2 pi i k/N):  Z'[k] -> A, Z'[H-k] -> B (scaled)
 __device__ __forceinline__ void c2r_pair(cd& A, cd& B, cd w, double scale) {
     const double Sx = A.x + B.x, Sy = A.y - B.y;
@@ -56,14 +107,15 @@ __device__ __forceinline__ void r2c_pair(cd& Zk, cd& Zm, cd w) {
 }
 
 template <int N>
-__global__ void __launch_bounds__(F2<N / 2>::THREADS, (N / 2 == 256) ? 2 : 4)
+__global__ void __launch_bounds__(F2<N / 2>::THREADS, (N / 2 == 256) ? 3 : 4)
 x_fused2_kernel(const __grid_constant__ FusedXArgs a) {
     constexpr int H = N / 2;
     typedef F2<H> P;
     constexpr int R0 = P::R0, R1 = P::R1, T = P::T, NB = P::NB, NT = P::THREADS;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cd* sm = reinterpret_cast<cd*>(smem_raw);
-    const cd* __restrict__ tw = a.tw;
+    const cd* __restrict__ tab = a.tw;      // lane-contiguous tables (FTab)
+    typedef FTab<H> FT;
 
     const int t = threadIdx.x % T, slot = threadIdx.x / T;
     const long long off = (long long)blockIdx.x * H;
@@ -81,17 +133,27 @@ x_fused2_kernel(const __grid_constant__ FusedXArgs a) {
             xa[r] = (ka <= kmax) ? line[ka] : mk(0.0, 0.0);
             xb[r] = (kb <= kmax) ? line[kb] : mk(0.0, 0.0);
         }
+        // split factors: exp(-2 pi i (j + r R1)/N) = exp(-2 pi i j/N) * (2 R0)-th root^r: one table load per thread
         if (t != 0) {
-#pragma unroll
-            for (int r = 0; r < R0; ++r) c2r_pair(xa[r], xb[R0 - 1 - r], __ldg(&tw[jA + r * R1]), scale);
+            const cd w0 = __ldg(&tab[FT::TA + t]);
+            static_for<0, R0>([&](auto rc) {
+                constexpr int r = decltype(rc)::value;
+                c2r_pair(xa[r], xb[R0 - 1 - r], mul_rootN<2 * R0, r, -1>(w0), scale);
+            });
         } else {
             // rows r*R1: r = 0 is the mean mode (its mirror is the dropped Nyquist mode), r = R0/2 is k = H/2
             xa[0] = mk(scale * xa[0].x, scale * xa[0].x);
             xa[R0 / 2] = mk(2.0 * scale * xa[R0 / 2].x, -2.0 * scale * xa[R0 / 2].y);
-#pragma unroll
-            for (int r = 1; r < R0 / 2; ++r) c2r_pair(xa[r], xa[R0 - r], __ldg(&tw[r * R1]), scale);
-#pragma unroll
-            for (int r = 0; r < R0 / 2; ++r) c2r_pair(xb[r], xb[R0 - 1 - r], __ldg(&tw[R1 / 2 + r * R1]), scale);
+            const cd one = mk(1.0, 0.0);
+            const cd wh = __ldg(&tab[FT::TB]);          // exp(-2 pi i (R1/2)/N)
+            static_for<1, R0 / 2>([&](auto rc) {
+                constexpr int r = decltype(rc)::value;
+                c2r_pair(xa[r], xa[R0 - r], mul_rootN<2 * R0, r, -1>(one), scale);
+            });
+            static_for<0, R0 / 2>([&](auto rc) {
+                constexpr int r = decltype(rc)::value;
+                c2r_pair(xb[r], xb[R0 - 1 - r], mul_rootN<2 * R0, r, -1>(wh), scale);
+            });
         }
         Dft<R0, +1>::run(xa);
         Dft<R0, +1>::run(xb);
@@ -111,7 +173,7 @@ x_fused2_kernel(const __grid_constant__ FusedXArgs a) {
 #pragma unroll
                 for (int r = 0; r < R1; ++r) u[b][r] = sm[tidx<H>(j + r * R0, slot)];
 #pragma unroll
-                for (int r = 1; r < R1; ++r) u[b][r] = twmul<+1>(u[b][r], __ldg(&tw[2 * r * j]));
+                for (int r = 1; r < R1; ++r) u[b][r] = twmul<+1>(u[b][r], __ldg(&tab[FT::TS + (b * R1 + r) * T + t]));
                 Dft<R1, +1>::run(u[b]);
             }
         }
@@ -171,24 +233,36 @@ x_fused2_kernel(const __grid_constant__ FusedXArgs a) {
             za[r] = sm[tidx<H>(jA + r * R1, slot)];
             zb[r] = sm[tidx<H>(jB + r * R1, slot)];
         }
-#pragma unroll
-        for (int r = 1; r < R0; ++r) {
-            za[r] = twmul<-1>(za[r], __ldg(&tw[2 * r * jA]));
-            zb[r] = twmul<-1>(zb[r], __ldg(&tw[2 * r * jB]));
-        }
+        // w^(r jB) = exp(-2 pi i r/R0) * conj(w^(r jA)) for jB = R1 - jA; lane t = 0 (jA = 0, jB = R1/2) finds
+        // exp(-2 pi i r/(2 R0)) in its TF entry instead and skips the (unit) factor of za
+        static_for<1, R0>([&](auto rc) {
+            constexpr int r = decltype(rc)::value;
+            const cd w = __ldg(&tab[FT::TF + r * T + t]);
+            if (t != 0) za[r] = twmul<-1>(za[r], w);
+            zb[r] = mul_rootN<R0, r, -1>(twmul<+1>(zb[r], w));
+        });
         Dft<R0, -1>::run(za);
         Dft<R0, -1>::run(zb);
         // za[q] = Z[jA + q*R1], zb[q] = Z[jB + q*R1]
         if (t != 0) {
-#pragma unroll
-            for (int q = 0; q < R0; ++q) r2c_pair(za[q], zb[R0 - 1 - q], __ldg(&tw[jA + q * R1]));
+            const cd w0 = __ldg(&tab[FT::TA + t]);
+            static_for<0, R0>([&](auto qc) {
+                constexpr int q = decltype(qc)::value;
+                r2c_pair(za[q], zb[R0 - 1 - q], mul_rootN<2 * R0, q, -1>(w0));
+            });
         } else {
             za[0] = mk(za[0].x + za[0].y, 0.0);                         // k = 0 (Nyquist partner dropped)
             za[R0 / 2] = mk(za[R0 / 2].x, -za[R0 / 2].y);               // k = H/2
-#pragma unroll
-            for (int q = 1; q < R0 / 2; ++q) r2c_pair(za[q], za[R0 - q], __ldg(&tw[q * R1]));
-#pragma unroll
-            for (int q = 0; q < R0 / 2; ++q) r2c_pair(zb[q], zb[R0 - 1 - q], __ldg(&tw[R1 / 2 + q * R1]));
+            const cd one = mk(1.0, 0.0);
+            const cd wh = __ldg(&tab[FT::TB]);
+            static_for<1, R0 / 2>([&](auto qc) {
+                constexpr int q = decltype(qc)::value;
+                r2c_pair(za[q], za[R0 - q], mul_rootN<2 * R0, q, -1>(one));
+            });
+            static_for<0, R0 / 2>([&](auto qc) {
+                constexpr int q = decltype(qc)::value;
+                r2c_pair(zb[q], zb[R0 - 1 - q], mul_rootN<2 * R0, q, -1>(wh));
+            });
         }
 #pragma unroll
         for (int q = 0; q < R0; ++q) {
@@ -210,6 +284,26 @@ template <int N> static void fused2_one(const FusedXArgs& a, cudaStream_t st) {
 }
 
 bool x_fused2_supported(int N) { return N == 128 || N == 256 || N == 512; }
+
+int x_fused2_table_entries(int N) {
+    switch (N) {
+        case 128: return FTab<64>::SIZE;
+        case 256: return FTab<128>::SIZE;
+        case 512: return FTab<256>::SIZE;
+        default: return 0;
+    }
+}
+void launch_x_fused2_tables(int N, cd* tab, cudaStream_t st) {
+    const int n = x_fused2_table_entries(N);
+    if (n == 0) return;
+    const int blocks = (n + 127) / 128;
+    switch (N) {
+        case 128: fused_twiddle_kernel<64><<<blocks, 128, 0, st>>>(tab); break;
+        case 256: fused_twiddle_kernel<128><<<blocks, 128, 0, st>>>(tab); break;
+        case 512: fused_twiddle_kernel<256><<<blocks, 128, 0, st>>>(tab); break;
+        default: break;
+    }
+}
 
 void launch_x_fused2(int N, const FusedXArgs& a, cudaStream_t st) {
     switch (N) {

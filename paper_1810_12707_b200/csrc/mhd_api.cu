@@ -33,7 +33,7 @@ size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 constexpr int NFIELD_BUFS = 48;   // U 8, Rold 8, W 16, X 8, Y 8
 
 struct Layout {
-    size_t field_bytes, tw_off, field_off, nyq_off, nyq_bytes, scratch_off, scratch_bytes, res_off, total;
+    size_t field_bytes, tw_off, ftw_off, field_off, nyq_off, nyq_bytes, scratch_off, scratch_bytes, res_off, total;
 };
 int nspec_of(int N) { return (int)std::ceil(std::sqrt(3.0) * N / 2.0) + 1; }
 Layout make_layout(int N) {
@@ -41,6 +41,7 @@ Layout make_layout(int N) {
     l.field_bytes = (size_t)N * N * N * sizeof(double);
     size_t off = 0;
     l.tw_off = off; off += align_up((size_t)N * sizeof(cd));
+    l.ftw_off = off; off += align_up((size_t)(4 * N + 64) * sizeof(cd));
     l.field_off = off; off += (size_t)NFIELD_BUFS * align_up(l.field_bytes);
     l.nyq_bytes = align_up((size_t)N * N * 8 * sizeof(cd));
     l.nyq_off = off; off += 3 * l.nyq_bytes;
@@ -66,6 +67,7 @@ struct mhd_ctx {
     std::string err;
     // device storage (inside the caller's workspace)
     cd* tw = nullptr;
+    cd* ftw = nullptr;     // lane-contiguous tables of the fused x sweep
     cd *U[8], *Rold[8], *W[16], *X[8], *Y[8], *nyq[3];
     double *scratch = nullptr, *res = nullptr;
     // profiling
@@ -217,7 +219,7 @@ void products(mhd_ctx* c, cd* const Uin[8]) {
         for (int f = 0; f < 16; ++f) a.out[f] = c->W[f];
         a.tw = c->tw; a.nlines = (long long)N * N; a.kmax_in = kmax; a.kmax_out = kmax; a.scale = scale; a.ph = ph;
         mhd_ctx::Scope s(c, F_X_FUSED);
-        if (c->opt_fused == 1 && x_fused2_supported(N)) launch_x_fused2(N, a, c->st);
+        if (c->opt_fused == 1 && x_fused2_supported(N)) { a.tw = c->ftw; launch_x_fused2(N, a, c->st); }
         else launch_x_fused(N, a, c->st);
     } else {
         XArgs a; std::memset(&a, 0, sizeof(a));
@@ -304,6 +306,7 @@ int mhd_bind(mhd_ctx* c, void* dev_workspace, size_t bytes, void* cuda_stream, u
     c->st = static_cast<cudaStream_t>(cuda_stream);
     c->flags = flags;
     c->tw = reinterpret_cast<cd*>(base + l.tw_off);
+    c->ftw = reinterpret_cast<cd*>(base + l.ftw_off);
     const size_t fb = align_up(l.field_bytes);
     char* fp = base + l.field_off;
     int k = 0;
@@ -316,7 +319,8 @@ int mhd_bind(mhd_ctx* c, void* dev_workspace, size_t bytes, void* cuda_stream, u
     c->scratch = reinterpret_cast<double*>(base + l.scratch_off);
     c->res = reinterpret_cast<double*>(base + l.res_off);
     launch_twiddle_table(c->N, c->tw, c->st);
-    c->launches += 1;
+    launch_x_fused2_tables(c->N, c->ftw, c->st);
+    c->launches += 2;
     int rc = check_cuda(c, "bind");
     if (rc) return rc;
     c->bound = true; c->have_fields = false; c->have_old = false; c->step = 0;
