@@ -89,13 +89,14 @@ template <int B, int E, class F> __device__ __forceinline__ void static_for(F&& 
     }
 }
 
-// C2R split of one mirror pair: A = X[k], B = X[H-k], w = exp(-2 pi i k/N):  Z'[k] -> A, Z'[H-k] -> B (scaled)
-__device__ __forceinline__ void c2r_pair(cd& A, cd& B, cd w, double scale) {
+// C2R split of one mirror pair: A = X[k], B = X[H-k], ws = scale * exp(-2 pi i k/N):  Z'[k] -> A, Z'[H-k] -> B, both
+// scaled; the scale rides on the twiddle and on four FMAs (no separate multiplications)
+__device__ __forceinline__ void c2r_pair(cd& A, cd& B, cd ws, double scale) {
     const double Sx = A.x + B.x, Sy = A.y - B.y;
     const double Dx = A.x - B.x, Dy = A.y + B.y;
-    const double p = w.x * Dx + w.y * Dy, q = w.x * Dy - w.y * Dx;
-    A = mk(scale * (Sx - q), scale * (Sy + p));
-    B = mk(scale * (Sx + q), scale * (p - Sy));
+    const double p = fma(ws.x, Dx, ws.y * Dy), q = fma(ws.x, Dy, -(ws.y * Dx));
+    A = mk(fma(scale, Sx, -q), fma(scale, Sy, p));
+    B = mk(fma(scale, Sx, q), fma(-scale, Sy, p));
 }
 // R2C merge of one mirror pair: Zk = Z[k], Zm = Z[H-k]:  X[k] -> Zk, X[H-k] -> Zm
 __device__ __forceinline__ void r2c_pair(cd& Zk, cd& Zm, cd w) {
@@ -135,7 +136,7 @@ x_fused2_kernel(const __grid_constant__ FusedXArgs a) {
         }
         // split factors: exp(-2 pi i (j + r R1)/N) = exp(-2 pi i j/N) * (2 R0)-th root^r: one table load per thread
         if (t != 0) {
-            const cd w0 = __ldg(&tab[FT::TA + t]);
+            const cd w0 = scale * __ldg(&tab[FT::TA + t]);
             static_for<0, R0>([&](auto rc) {
                 constexpr int r = decltype(rc)::value;
                 c2r_pair(xa[r], xb[R0 - 1 - r], mul_rootN<2 * R0, r, -1>(w0), scale);
@@ -144,8 +145,8 @@ x_fused2_kernel(const __grid_constant__ FusedXArgs a) {
             // rows r*R1: r = 0 is the mean mode (its mirror is the dropped Nyquist mode), r = R0/2 is k = H/2
             xa[0] = mk(scale * xa[0].x, scale * xa[0].x);
             xa[R0 / 2] = mk(2.0 * scale * xa[R0 / 2].x, -2.0 * scale * xa[R0 / 2].y);
-            const cd one = mk(1.0, 0.0);
-            const cd wh = __ldg(&tab[FT::TB]);          // exp(-2 pi i (R1/2)/N)
+            const cd one = mk(scale, 0.0);
+            const cd wh = scale * __ldg(&tab[FT::TB]);  // scale * exp(-2 pi i (R1/2)/N)
             static_for<1, R0 / 2>([&](auto rc) {
                 constexpr int r = decltype(rc)::value;
                 c2r_pair(xa[r], xa[R0 - r], mul_rootN<2 * R0, r, -1>(one), scale);
@@ -163,31 +164,23 @@ x_fused2_kernel(const __grid_constant__ FusedXArgs a) {
             sm[tidx<H>(jB * R0 + q, slot)] = xb[q];
         }
     }
-    __syncthreads();
-    {
-        cd u[NB][R1];
-        if (slot < S_NIN) {
+    __syncwarp();           // a slot's T threads sit in one warp: its exchanges need no block-wide barrier
+    if (slot < S_NIN) {
+        // second stage: butterfly j reads and writes the same rows j + r*R0 -> in place, one butterfly at a time
+#pragma unroll 1
+        for (int b = 0; b < NB; ++b) {
+            const int j = t + b * T;
+            cd u[R1];
 #pragma unroll
-            for (int b = 0; b < NB; ++b) {
-                const int j = t + b * T;
+            for (int r = 0; r < R1; ++r) u[r] = sm[tidx<H>(j + r * R0, slot)];
 #pragma unroll
-                for (int r = 0; r < R1; ++r) u[b][r] = sm[tidx<H>(j + r * R0, slot)];
+            for (int r = 1; r < R1; ++r) u[r] = twmul<+1>(u[r], __ldg(&tab[FT::TS + (b * R1 + r) * T + t]));
+            Dft<R1, +1>::run(u);
 #pragma unroll
-                for (int r = 1; r < R1; ++r) u[b][r] = twmul<+1>(u[b][r], __ldg(&tab[FT::TS + (b * R1 + r) * T + t]));
-                Dft<R1, +1>::run(u[b]);
-            }
-        }
-        __syncthreads();
-        if (slot < S_NIN) {
-#pragma unroll
-            for (int b = 0; b < NB; ++b) {
-                const int j = t + b * T;
-#pragma unroll
-                for (int q = 0; q < R1; ++q) sm[tidx<H>(j + q * R0, slot)] = u[b][q];
-            }
+            for (int q = 0; q < R1; ++q) sm[tidx<H>(j + q * R0, slot)] = u[q];
         }
     }
-    __syncthreads();
+    __syncthreads();        // the products read every slot of a row
 
     // ================= point-wise products: row n holds (f(x=2n), f(x=2n+1)) of every field ===================
 #pragma unroll 1
@@ -206,32 +199,26 @@ x_fused2_kernel(const __grid_constant__ FusedXArgs a) {
     __syncthreads();
 
     // ================= forward: 16 lines, tile -> registers -> global ==========================================
-    {
-        cd u[NB][R1];
+    // first stage in place: Y[j][q] = sum_r x[j + r*R0] w_R1^(r q) is written back to row j + q*R0
+#pragma unroll 1
+    for (int b = 0; b < NB; ++b) {
+        const int j = t + b * T;
+        cd u[R1];
 #pragma unroll
-        for (int b = 0; b < NB; ++b) {
-            const int j = t + b * T;
+        for (int r = 0; r < R1; ++r) u[r] = sm[tidx<H>(j + r * R0, slot)];
+        Dft<R1, -1>::run(u);
 #pragma unroll
-            for (int r = 0; r < R1; ++r) u[b][r] = sm[tidx<H>(j + r * R0, slot)];
-            Dft<R1, -1>::run(u[b]);
-        }
-        __syncthreads();
-#pragma unroll
-        for (int b = 0; b < NB; ++b) {
-            const int j = t + b * T;
-#pragma unroll
-            for (int q = 0; q < R1; ++q) sm[tidx<H>(j * R1 + q, slot)] = u[b][q];
-        }
+        for (int q = 0; q < R1; ++q) sm[tidx<H>(j + q * R0, slot)] = u[q];
     }
-    __syncthreads();
+    __syncwarp();
     {
         cd* __restrict__ line = a.out[slot] + off;
         const int kmax = a.kmax_out;
         cd za[R0], zb[R0];
 #pragma unroll
         for (int r = 0; r < R0; ++r) {
-            za[r] = sm[tidx<H>(jA + r * R1, slot)];
-            zb[r] = sm[tidx<H>(jB + r * R1, slot)];
+            za[r] = sm[tidx<H>(r + jA * R0, slot)];      // Y[r][jA]
+            zb[r] = sm[tidx<H>(r + jB * R0, slot)];
         }
         // w^(r jB) = exp(-2 pi i r/R0) * conj(w^(r jA)) for jB = R1 - jA; lane t = 0 (jA = 0, jB = R1/2) finds
         // exp(-2 pi i r/(2 R0)) in its TF entry instead and skips the (unit) factor of za
