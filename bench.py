@@ -106,7 +106,7 @@ def aggregate(ms_local: float, units_local: float, dist=None):
 # ----------------------------------------------------------------------------------------------------------------
 # algorithmic bytes per launch; one field-sweep = 8 B per grid point
 # ----------------------------------------------------------------------------------------------------------------
-def sweep_bytes(N: int, prune: bool):
+def sweep_bytes(N: int, prune: bool, fuse_current: bool = True):
     """Per-family algorithmic bytes of ONE right-hand side: what the kernels must read + write."""
     kc = N // 3
     H = N // 2
@@ -114,8 +114,11 @@ def sweep_bytes(N: int, prune: bool):
     ah = (kc + 1) / H if prune else 1.0             # kept fraction of the stored half axis
     f = 8.0 * N ** 3                                # bytes of one full field sweep
     b = {}
-    b["build_current"] = (3 + 3) * f * ah * a * a
-    b["strided_inverse"] = 11 * f * ah * (a * a + a) + 11 * f * ah * (a + 1.0)       # z pass, y pass (read + write)
+    if fuse_current:     # S1 reads the 8 state fields and builds J^ on load; writes 11
+        b["strided_inverse"] = f * ah * (8 * a * a + 11 * a) + 11 * f * ah * (a + 1.0)   # z pass, y pass (read + write)
+    else:
+        b["build_current"] = (3 + 3) * f * ah * a * a
+        b["strided_inverse"] = 11 * f * ah * (a * a + a) + 11 * f * ah * (a + 1.0)
     b["x_fused"] = (11 + 16) * f * ah
     b["strided_forward"] = 16 * f * ah * (1.0 + a) + 16 * f * ah * (a + a * a)       # y pass, z pass
     b["assemble"] = (16 + 8 + 8 + 8 + 8) * f * ah * a * a
@@ -248,6 +251,11 @@ def run_ours(args):
     g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, device="cuda:%d" % local_rank)
     host = [torch.from_numpy(p).pin_memory() for p in cfg.prim]      # pinned host inputs
     cfg.prim = None
+    opts = {}
+    for kv in args.option:
+        k, v = kv.split("=")
+        opts[int(k)] = int(v)
+        g.set_option(int(k), int(v))
     g.set_fields(host, "primitive")
     K, W = args.steps, max(args.warmup, 3)
 
@@ -270,7 +278,7 @@ def run_ours(args):
         peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     else:
         peak, peak_src = FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
-    sb = sweep_bytes(N, prune=True)
+    sb = sweep_bytes(N, prune=True, fuse_current=opts.get(4, 1) != 0)
     fam = {}
     for name, b in sb.items():
         p = prof.get(name, {"ms": 0.0, "launches": 0})
@@ -358,6 +366,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-fft", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--option", action="append", default=[], metavar="ID=VALUE",
+                    help="mhd_set_option(ID, VALUE) before the run (include/mhd.h MHD_OPT_*), for A/B measurements")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

@@ -59,6 +59,9 @@ extern "C" {
 #define MHD_OPT_INTEGRATOR 3 /* 0 (default): Adams-Bashforth 2 with Euler start; 1: RK4; 2: predictor-corrector
                                 (Table I; R6)                                 */
 
+#define MHD_OPT_FUSE_CURRENT 4 /* 1 (default): J^ = M i k x B^ is built on load inside the inverse z pass (sweep S1);
+                                0: separate kernel                                                            */
+
 typedef struct mhd_ctx mhd_ctx; /* opaque, owned by the library */
 
 /* Diagnostics record ("per grid" = volume means; L71 Eq. 9; R8). */

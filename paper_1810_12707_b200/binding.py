@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libmhd.so")
 MHD_OK = 0
 MHD_HOST, MHD_DEVICE = 0, 1
 MHD_CONSERVATIVE, MHD_PRIMITIVE = 0, 1
-MHD_OPT_FUSED, MHD_OPT_PRUNE, MHD_OPT_INTEGRATOR = 1, 2, 3
+MHD_OPT_FUSED, MHD_OPT_PRUNE, MHD_OPT_INTEGRATOR, MHD_OPT_FUSE_CURRENT = 1, 2, 3, 4
 ERRORS = {-1: "MHD_ERR_INVALID_ARG", -2: "MHD_ERR_NOT_BOUND", -3: "MHD_ERR_NO_FIELDS", -4: "MHD_ERR_CUDA",
           -5: "MHD_ERR_NOMEM"}
 

@@ -14,22 +14,35 @@ struct Phys {
     double gamma, mu, eta;
 };
 
-// ---- strided (y / z) complex passes on [kz][ky][kx] half-spectrum arrays with row pitch `hx` ------------
+// ---- strided (y / z) complex passes on half-spectrum arrays ------------------------------------------------
+// The transformed axis ("rows") and one outer axis are addressed by strides, so the same kernel serves the
+// in-place in-core sweeps on [kz][ky][kx] arrays (pitch N/2) and the bricks / slabs of the out-of-core
+// pipeline (compact layouts, separate input and output views).
+// Row storage modes: 0 = all N rows stored; 1 = all N rows stored, rows outside the 2/3 mask are not touched
+// (read as zero / not written); 2 = compact: only the 2kc+1 rows inside the mask are stored, consecutively
+// (row r <= kc at r, row r >= N-kc at r - (N - 2kc - 1)).
 struct StridedArgs {
     const cd* in[MAXF];
     cd* out[MAXF];
     const cd* tw;          // exp(-2 pi i m / N), m < N
-    long long row_stride;  // complex elements between consecutive points of the transformed axis
-    long long outer_stride;// complex elements between consecutive outer indices
+    long long in_row_stride, out_row_stride;      // complex elements between consecutive stored rows
+    long long in_outer_stride, out_outer_stride;  // complex elements between consecutive outer indices
     int nchunks;           // column chunks (of C columns) to process
     int ncols;             // valid columns (guards the last chunk)
     int n_outer;           // number of outer indices processed
-    int outer_split;       // outer index o maps to o (o < split) or o + outer_skip
+    int outer_split;       // in-core: outer index o maps to o (o < split) or o + outer_skip
     int outer_skip;
     int kc;                // 2/3 cut-off
-    int in_pruned;         // rows outside the mask are not read (taken as zero)
-    int out_pruned;        // rows outside the mask are not written
+    int in_rows;           // row storage mode of the input (0, 1, 2)
+    int out_rows;          // row storage mode of the output
     int nfields;
+    int general;           // 0: in-core fast path (out strides = in strides, row modes 0/1); 1: general views
+    // Fused current (sweep S1): fields f >= jfirst are not read from in[f]; they are built on load as
+    // J^_c = M (i k x B^)_c from in[bfirst .. bfirst+2] (rows = kz, outer = ky, columns = kx).  jfirst < 0: off.
+    int jfirst, bfirst;
+    int outer_compact;     // 1: outer index (+ outer_base) is a compact ky index; 0: a full array index
+    int outer_base;
+    double k0;             // 2 pi / L
 };
 // dir = -1 forward, +1 inverse (unnormalised both ways)
 void launch_strided(int N, int dir, const StridedArgs& a, cudaStream_t st);
@@ -77,6 +90,11 @@ void launch_cons_to_prim(long long n, double* const f[8], double gamma, cudaStre
 struct SpecGeom {
     int N, hx, kc;     // hx = row pitch in complex elements (N/2)
     int pruned;        // visit only modes inside the mask (1) or all stored modes (0; masked ones get zero)
+    // Compact bricks (out-of-core pipeline): the arrays hold only rows inside the mask.  Thread (ix, oy, oz) with
+    // oy < ny, oz < 2kc+1 addresses "work" arrays at oz*wsz + oy*wsy + ix and "state" arrays at oz*ssz + oy*ssy + ix;
+    // its ky mode follows from the compact index oy + y0.  compact = 0: both are the full [kz][ky][kx] index.
+    int compact, y0, ny;
+    long long wsy, wsz, ssy, ssz;
 };
 // J^ = M i k x B^
 void launch_build_current(const SpecGeom& g, const cd* const B[3], cd* const J[3], Phys ph, cudaStream_t st);

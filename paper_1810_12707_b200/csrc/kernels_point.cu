@@ -11,16 +11,29 @@ namespace mhd {
 
 // ---- mode geometry -----------------------------------------------------------------------------------------
 struct ModeIt {
-    int ix, iy, iz;          // array indices
+    int ix, iy, iz;          // array indices (full layout) / compact indices (bricks)
     int nx, ny, nz;          // integer modes
     bool inside;             // inside the 2/3 mask
-    long long idx;           // linear index
+    long long idx;           // linear index into "work" arrays
+    long long sidx;          // linear index into "state" arrays (same as idx in the full layout)
 };
 // grid: x over kx (blockDim.x threads), y over the (possibly pruned) ky count, z over the kz count
 __device__ __forceinline__ bool mode_of_thread(const SpecGeom& g, ModeIt& m) {
     const int N = g.N, kc = g.kc;
     m.ix = blockIdx.x * blockDim.x + threadIdx.x;
     int oy = blockIdx.y, oz = blockIdx.z;
+    if (g.compact) {
+        if (m.ix > kc) return false;
+        const int cy = oy + g.y0;
+        m.iy = oy; m.iz = oz;
+        m.nx = m.ix;
+        m.ny = cy <= kc ? cy : cy - (2 * kc + 1);
+        m.nz = oz <= kc ? oz : oz - (2 * kc + 1);
+        m.inside = true;
+        m.idx = (long long)oz * g.wsz + (long long)oy * g.wsy + m.ix;
+        m.sidx = (long long)oz * g.ssz + (long long)oy * g.ssy + m.ix;
+        return true;
+    }
     if (g.pruned) {
         if (m.ix > kc) return false;
         m.iy = oy <= kc ? oy : N - (2 * kc + 1) + oy;
@@ -34,9 +47,11 @@ __device__ __forceinline__ bool mode_of_thread(const SpecGeom& g, ModeIt& m) {
     m.nz = m.iz <= N / 2 ? m.iz : m.iz - N;
     m.inside = m.nx <= kc && abs(m.ny) <= kc && abs(m.nz) <= kc;
     m.idx = ((long long)m.iz * N + m.iy) * g.hx + m.ix;
+    m.sidx = m.idx;
     return true;
 }
 static dim3 mode_grid(const SpecGeom& g, int threads) {
+    if (g.compact) return dim3((g.kc + 1 + threads - 1) / threads, g.ny, 2 * g.kc + 1);
     const int nxv = g.pruned ? g.kc + 1 : g.hx;
     const int nyv = g.pruned ? 2 * g.kc + 1 : g.N;
     return dim3((nxv + threads - 1) / threads, nyv, nyv);
@@ -57,7 +72,7 @@ __global__ void build_current_kernel(SpecGeom g, Ptr3 B, PtrW3 J, Phys ph) {
     cd jx = mk(0, 0), jy = jx, jz = jx;
     if (m.inside) {
         const double kx = ph.k0 * m.nx, ky = ph.k0 * m.ny, kz = ph.k0 * m.nz;
-        const cd bx = B.p[0][m.idx], by = B.p[1][m.idx], bz = B.p[2][m.idx];
+        const cd bx = B.p[0][m.sidx], by = B.p[1][m.sidx], bz = B.p[2][m.sidx];
         jx = imul(ky, bz) - imul(kz, by);
         jy = imul(kz, bx) - imul(kx, bz);
         jz = imul(kx, by) - imul(ky, bx);
@@ -77,7 +92,7 @@ __global__ void divergence_kernel(SpecGeom g, Ptr3 B, cd* out, Phys ph) {
     cd d = mk(0, 0);
     if (m.inside) {
         const double kx = ph.k0 * m.nx, ky = ph.k0 * m.ny, kz = ph.k0 * m.nz;
-        d = imul(kx, B.p[0][m.idx]) + imul(ky, B.p[1][m.idx]) + imul(kz, B.p[2][m.idx]);
+        d = imul(kx, B.p[0][m.sidx]) + imul(ky, B.p[1][m.sidx]) + imul(kz, B.p[2][m.sidx]);
     }
     out[m.idx] = d;
 }
@@ -92,14 +107,14 @@ void launch_divergence(const SpecGeom& g, const cd* const B[3], cd* out, Phys ph
 __global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 rout, int mode, double dt, Phys ph) {
     ModeIt m;
     if (!mode_of_thread(g, m)) return;
-    const long long i = m.idx;
+    const long long i = m.idx, j = m.sidx;     // products / state
     cd R[8];
     if (m.inside) {
         const double kx = ph.k0 * m.nx, ky = ph.k0 * m.ny, kz = ph.k0 * m.nz;
         const double k2 = kx * kx + ky * ky + kz * kz;
         cd u[8];
 #pragma unroll
-        for (int f = 0; f < 8; ++f) u[f] = U.p[f][i];
+        for (int f = 0; f < 8; ++f) u[f] = U.p[f][j];
         const cd txx = pr.p[P_TXX][i], txy = pr.p[P_TXY][i], txz = pr.p[P_TXZ][i];
         const cd tyy = pr.p[P_TYY][i], tyz = pr.p[P_TYZ][i], tzz = pr.p[P_TZZ][i];
         const cd ex = pr.p[P_EX][i], ey = pr.p[P_EY][i], ez = pr.p[P_EZ][i];
@@ -115,20 +130,20 @@ __global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 r
         R[7] = imul(kx, ey) - imul(ky, ex) - (ph.eta * k2) * u[7];
         if (mode == 0) {
 #pragma unroll
-            for (int f = 0; f < 8; ++f) rout.p[f][i] = R[f];
+            for (int f = 0; f < 8; ++f) rout.p[f][j] = R[f];
         } else {
 #pragma unroll
             for (int f = 0; f < 8; ++f) {
                 cd inc;
                 if (mode == 1) inc = R[f];
-                else { const cd ro = Rold.p[f][i]; inc = mk(1.5 * R[f].x - 0.5 * ro.x, 1.5 * R[f].y - 0.5 * ro.y); }
-                U.p[f][i] = mk(u[f].x + dt * inc.x, u[f].y + dt * inc.y);
-                Rold.p[f][i] = R[f];
+                else { const cd ro = Rold.p[f][j]; inc = mk(1.5 * R[f].x - 0.5 * ro.x, 1.5 * R[f].y - 0.5 * ro.y); }
+                U.p[f][j] = mk(u[f].x + dt * inc.x, u[f].y + dt * inc.y);
+                Rold.p[f][j] = R[f];
             }
         }
     } else if (mode == 0) {      // unpruned sweep: make the masked-out modes explicit zeros
 #pragma unroll
-        for (int f = 0; f < 8; ++f) rout.p[f][i] = mk(0, 0);
+        for (int f = 0; f < 8; ++f) rout.p[f][j] = mk(0, 0);
     }
 }
 void launch_assemble(const SpecGeom& g, const cd* const prod[16], cd* const U[8], cd* const Rold[8],
@@ -146,8 +161,8 @@ __global__ void axpby_kernel(SpecGeom g, int nf, double a, PtrN y, double b, Ptr
     for (int f = 0; f < nf; ++f) {
         const cd xv = x.p[f][m.idx];
         cd yv = mk(0, 0);
-        if (a != 0.0) { yv = y.p[f][m.idx]; yv = mk(a * yv.x, a * yv.y); }
-        y.p[f][m.idx] = mk(yv.x + b * xv.x, yv.y + b * xv.y);
+        if (a != 0.0) { yv = y.p[f][m.sidx]; yv = mk(a * yv.x, a * yv.y); }
+        y.p[f][m.sidx] = mk(yv.x + b * xv.x, yv.y + b * xv.y);
     }
 }
 void launch_axpby(const SpecGeom& g, int nf, double a, cd* const y[], double b, const cd* const x[], cudaStream_t st) {

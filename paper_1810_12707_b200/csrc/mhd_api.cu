@@ -61,7 +61,7 @@ struct mhd_ctx {
     bool bound = false, have_fields = false, have_old = false;
     cudaStream_t st = nullptr;
     unsigned flags = 0;
-    int opt_fused = 1, opt_prune = 1, integrator = 0;
+    int opt_fused = 1, opt_prune = 1, opt_fuse_current = 1, integrator = 0;
     long long step = 0;
     long long launches = 0;
     std::string err;
@@ -121,7 +121,7 @@ int check_cuda(mhd_ctx* c, const char* what) {
 // ---- sweeps --------------------------------------------------------------------------------------------------
 // strided pass over nf arrays; axis 1 = y, 2 = z; hx = row pitch of the arrays (N/2, or 8 for the Nyquist planes)
 void strided_pass(mhd_ctx* c, int dir, int axis, int nf, const cd* const in[], cd* const out[], int hx, int ncols_full,
-                  bool prune) {
+                  bool prune, int jfirst = -1, int bfirst = 0) {
     const int N = c->N, kc = c->kc();
     int done = 0;
     while (done < nf) {
@@ -132,19 +132,20 @@ void strided_pass(mhd_ctx* c, int dir, int axis, int nf, const cd* const in[], c
         a.tw = c->tw;
         a.kc = kc;
         a.nfields = nb;
+        a.jfirst = jfirst; a.bfirst = bfirst; a.k0 = 2.0 * M_PI / c->L;   // fused current: only with nf <= MAXF
         const int C = N >= 1024 ? 4 : 8;
         a.ncols = prune ? std::min(kc + 1, ncols_full) : ncols_full;
         a.nchunks = (a.ncols + C - 1) / C;
         if (axis == 1) {            // y pass: rows along y, outer = z (all planes)
-            a.row_stride = hx; a.outer_stride = (long long)N * hx;
+            a.in_row_stride = a.out_row_stride = hx; a.in_outer_stride = a.out_outer_stride = (long long)N * hx;
             a.n_outer = N; a.outer_split = N; a.outer_skip = 0;
         } else {                    // z pass: rows along z, outer = ky (pruned to the mask)
-            a.row_stride = (long long)N * hx; a.outer_stride = hx;
+            a.in_row_stride = a.out_row_stride = (long long)N * hx; a.in_outer_stride = a.out_outer_stride = hx;
             if (prune) { a.n_outer = 2 * kc + 1; a.outer_split = kc + 1; a.outer_skip = N - (2 * kc + 1); }
             else { a.n_outer = N; a.outer_split = N; a.outer_skip = 0; }
         }
-        a.in_pruned = (prune && dir > 0) ? 1 : 0;     // inverse: input rows outside the mask are zero
-        a.out_pruned = (prune && dir < 0) ? 1 : 0;    // forward: output rows outside the mask are not needed
+        a.in_rows = (prune && dir > 0) ? 1 : 0;     // inverse: input rows outside the mask are zero
+        a.out_rows = (prune && dir < 0) ? 1 : 0;    // forward: output rows outside the mask are not needed
         mhd_ctx::Scope s(c, dir > 0 ? F_STRIDED_INV : F_STRIDED_FWD);
         launch_strided(N, dir, a, c->st);
         done += nb;
@@ -202,14 +203,19 @@ void products(mhd_ctx* c, cd* const Uin[8]) {
     const bool prune = c->opt_prune != 0;
     const SpecGeom g = c->geom();
     const Phys ph = c->phys();
-    {   // S1a: J^ = M i k x B^ -> W[8..10]
-        mhd_ctx::Scope s(c, F_CURRENT);
-        launch_build_current(g, Uin + 5, c->W + 8, ph, c->st);
-    }
     const cd* in[11];
     for (int f = 0; f < 8; ++f) in[f] = Uin[f];
     for (int f = 8; f < 11; ++f) in[f] = c->W[f];
-    strided_pass(c, +1, 2, 11, in, c->W, c->hx(), c->hx(), prune);        // S1b
+    if (c->opt_fused && c->opt_fuse_current) {
+        // S1: inverse z pass of U^ with J^ = M i k x B^ built on load (fields 8..10 come from in[5..7])
+        strided_pass(c, +1, 2, 11, in, c->W, c->hx(), c->hx(), prune, 8, 5);
+    } else {
+        {   // S1a: J^ = M i k x B^ -> W[8..10]
+            mhd_ctx::Scope s(c, F_CURRENT);
+            launch_build_current(g, Uin + 5, c->W + 8, ph, c->st);
+        }
+        strided_pass(c, +1, 2, 11, in, c->W, c->hx(), c->hx(), prune);    // S1b
+    }
     strided_pass(c, +1, 1, 11, c->W, c->W, c->hx(), c->hx(), prune);      // S2
     const int kmax = prune ? c->kc() : c->hx() - 1;
     const double scale = 1.0 / ((double)N * N * N);
@@ -334,6 +340,7 @@ int mhd_set_option(mhd_ctx* c, int option, int value) {
             if (value < 0 || value > 2) return c->fail(MHD_ERR_INVALID_ARG, "fused must be 0, 1 or 2");
             c->opt_fused = value; return MHD_OK;
         case MHD_OPT_PRUNE: c->opt_prune = value ? 1 : 0; return MHD_OK;
+        case MHD_OPT_FUSE_CURRENT: c->opt_fuse_current = value ? 1 : 0; return MHD_OK;
         case MHD_OPT_INTEGRATOR:
             if (value < 0 || value > 2) return c->fail(MHD_ERR_INVALID_ARG, "integrator must be 0, 1 or 2");
             c->integrator = value; c->have_old = false; return MHD_OK;
