@@ -50,7 +50,15 @@ extern "C" {
 
 /* workspace flags */
 #define MHD_FLAG_DEFAULT 0u
-#define MHD_FLAG_OUT_OF_CORE 1u /* field storage in pinned host memory, slabs streamed (Sec. VII-C) */
+/* The chunked ("out-of-core") pipeline, Sec. VII-C (L333-343, L375-379): the paper pages a working set larger
+ * than device memory through CUDA unified memory; here storage is compact (only the modes inside the 2/3 mask), each
+ * class of arrays is placed explicitly, and bricks / slabs of the host-resident classes are streamed through device
+ * staging buffers on side streams.  Placement flags need MHD_FLAG_OUT_OF_CORE.           */
+#define MHD_FLAG_OUT_OF_CORE 1u   /* chunked pipeline on compact storage; with no placement flag everything stays in HBM */
+#define MHD_FLAG_STATE_ON_HOST 2u /* U^ and the Adams-Bashforth history live in pinned host memory                      */
+#define MHD_FLAG_WORK_ON_HOST 4u  /* the 16 work fields between the z and y passes live in pinned host memory           */
+#define MHD_FLAG_BUDGET_MIB(m) ((unsigned)(m) << 8) /* cap on the device workspace in MiB (0 = none): bounds the staging
+                                     buffers; mhd_workspace_bytes() returns 0 if the placement cannot fit the budget     */
 
 /* options for mhd_set_option() */
 #define MHD_OPT_FUSED 1      /* 1 (default): fused kernels; 2: first-generation fused x sweep;
@@ -61,6 +69,9 @@ extern "C" {
 
 #define MHD_OPT_FUSE_CURRENT 4 /* 1 (default): J^ = M i k x B^ is built on load inside the inverse z pass (sweep S1);
                                 0: separate kernel                                                            */
+
+#define MHD_OPT_OOC_BRICK 5 /* chunked pipeline: largest number of ky columns per brick (0 = what the staging allows) */
+#define MHD_OPT_OOC_SLAB 6  /* chunked pipeline: largest number of z planes per slab  (0 = what the staging allows) */
 
 typedef struct mhd_ctx mhd_ctx; /* opaque, owned by the library */
 
@@ -85,12 +96,15 @@ int mhd_init(mhd_ctx **out, int N, double L, double gamma, double mu, double eta
 
 /* Device bytes the caller must provide to mhd_bind() for grid size N and the given flags. */
 size_t mhd_workspace_bytes(int N, unsigned flags);
-/* Pinned host bytes needed by the out-of-core path (0 for the in-core path). */
+/* Page-locked host bytes mhd_bind() needs for the placement flags (0 if nothing lives on the host). */
 size_t mhd_pinned_bytes(int N, unsigned flags);
 
 /* Attach storage.  dev_workspace: device pointer, 256-byte aligned, >= mhd_workspace_bytes(N, flags);
  * cuda_stream: a cudaStream_t (NULL = legacy default stream); pinned_host/pinned_bytes: page-locked host
- * memory for the out-of-core path (NULL/0 otherwise).  Builds the twiddle tables (device work). */
+ * memory, 256-byte aligned, >= mhd_pinned_bytes(N, flags), for the host-resident classes of the chunked pipeline
+ * (NULL/0 otherwise); the caller keeps it alive like the workspace.  Builds the twiddle tables (device work).
+ * A context bound with MHD_FLAG_OUT_OF_CORE implements every call except mhd_fft3d_*, the kinetic spectrum of
+ * mhd_diagnostics (needs an unpruned transform) and the RK4 / predictor-corrector integrators. */
 int mhd_bind(mhd_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream, unsigned flags,
              void *pinned_host, size_t pinned_bytes);
 
@@ -127,6 +141,9 @@ int mhd_nspec(int N);
 int mhd_fft3d_r2c(mhd_ctx *ctx, int nfields, const double *const real[], double *const spec[],
                   double *const nyq[], int prune);
 int mhd_fft3d_c2r(mhd_ctx *ctx, int nfields, double *const spec[], double *const real[], int prune);
+
+/* Bytes the chunked pipeline has copied host->device / device->host so far (0 for an in-core context). */
+int mhd_transfer_bytes(const mhd_ctx *ctx, long long *h2d, long long *d2h);
 
 /* Number of kernels this context has launched so far (for the bench's gpu_launches claim). */
 long long mhd_launch_count(const mhd_ctx *ctx);

@@ -19,14 +19,21 @@ LIB_PATH = os.path.join(_HERE, "libmhd.so")
 MHD_OK = 0
 MHD_HOST, MHD_DEVICE = 0, 1
 MHD_CONSERVATIVE, MHD_PRIMITIVE = 0, 1
-MHD_OPT_FUSED, MHD_OPT_PRUNE, MHD_OPT_INTEGRATOR, MHD_OPT_FUSE_CURRENT = 1, 2, 3, 4
+MHD_OPT_FUSED, MHD_OPT_PRUNE, MHD_OPT_INTEGRATOR, MHD_OPT_FUSE_CURRENT, MHD_OPT_OOC_BRICK, MHD_OPT_OOC_SLAB = 1, 2, 3, 4, 5, 6
+MHD_FLAG_OUT_OF_CORE, MHD_FLAG_STATE_ON_HOST, MHD_FLAG_WORK_ON_HOST = 1, 2, 4
+
+
+def MHD_FLAG_BUDGET_MIB(m):
+    return int(m) << 8
+
+
 ERRORS = {-1: "MHD_ERR_INVALID_ARG", -2: "MHD_ERR_NOT_BOUND", -3: "MHD_ERR_NO_FIELDS", -4: "MHD_ERR_CUDA",
           -5: "MHD_ERR_NOMEM"}
 
 # every symbol include/mhd.h declares (checked by tests/test_abi.py)
 SYMBOLS = ["mhd_init", "mhd_workspace_bytes", "mhd_pinned_bytes", "mhd_bind", "mhd_set_option", "mhd_set_fields",
            "mhd_rhs", "mhd_step", "mhd_get_fields", "mhd_diagnostics", "mhd_nspec", "mhd_fft3d_r2c",
-           "mhd_fft3d_c2r", "mhd_launch_count", "mhd_profile_enable", "mhd_profile_get", "mhd_last_error",
+           "mhd_fft3d_c2r", "mhd_launch_count", "mhd_transfer_bytes", "mhd_profile_enable", "mhd_profile_get", "mhd_last_error",
            "mhd_destroy"]
 
 
@@ -66,6 +73,7 @@ def lib():
     L.mhd_fft3d_c2r.argtypes = [C.c_void_p, C.c_int, P8, P8, C.c_int]
     L.mhd_launch_count.argtypes = [C.c_void_p]
     L.mhd_launch_count.restype = C.c_longlong
+    L.mhd_transfer_bytes.argtypes = [C.c_void_p, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
     L.mhd_profile_enable.argtypes = [C.c_void_p, C.c_int]
     L.mhd_profile_get.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_char_p), C.POINTER(C.c_double),
                                   C.POINTER(C.c_longlong)]
@@ -86,7 +94,10 @@ def _ptr_array(ptrs):
 class MHD:
     """One solver context on the current CUDA device; torch owns the workspace and the stream."""
 
-    def __init__(self, N, L=2 * math.pi, gamma=5.0 / 3.0, mu=0.0, eta=0.0, dt=1e-3, device="cuda:0", stream=None):
+    def __init__(self, N, L=2 * math.pi, gamma=5.0 / 3.0, mu=0.0, eta=0.0, dt=1e-3, device="cuda:0", stream=None,
+                 flags=0):
+        """flags: 0 = in-core; MHD_FLAG_OUT_OF_CORE [| MHD_FLAG_STATE_ON_HOST | MHD_FLAG_WORK_ON_HOST |
+        MHD_FLAG_BUDGET_MIB(m)] = the chunked pipeline (include/mhd.h); torch then also owns the pinned host block."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: the product path has no CPU fallback")
@@ -98,13 +109,24 @@ class MHD:
         rc = self._L.mhd_init(C.byref(self._h), self.N, L, gamma, mu, eta, dt)
         if rc != MHD_OK:
             raise ValueError("mhd_init: %s" % ERRORS.get(rc, rc))
-        nbytes = int(self._L.mhd_workspace_bytes(self.N, 0))
+        self.flags = int(flags)
+        nbytes = int(self._L.mhd_workspace_bytes(self.N, self.flags))
+        if nbytes == 0:
+            self.close()
+            raise ValueError("mhd_workspace_bytes: flags 0x%x / device budget not usable for N = %d" % (self.flags, self.N))
+        npinned = int(self._L.mhd_pinned_bytes(self.N, self.flags))
+        self.workspace_bytes, self.pinned_bytes = nbytes, npinned
         with torch.cuda.device(self.device):
             self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
             base = self.workspace.data_ptr()
             self._base = (base + 255) // 256 * 256
+            self.pinned = None
+            hbase = None
+            if npinned:
+                self.pinned = torch.empty(npinned + 256, dtype=torch.uint8, pin_memory=True)
+                hbase = (self.pinned.data_ptr() + 255) // 256 * 256
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-            self._check(self._L.mhd_bind(self._h, self._base, nbytes, self.stream.cuda_stream, 0, None, 0))
+            self._check(self._L.mhd_bind(self._h, self._base, nbytes, self.stream.cuda_stream, self.flags, hbase, npinned))
 
     # -- helpers ----------------------------------------------------------------------------------------
     def _check(self, rc):
@@ -203,6 +225,12 @@ class MHD:
         r = _ptr_array([t.data_ptr() for t in real])
         s = _ptr_array([t.data_ptr() for t in spec])
         self._check(self._L.mhd_fft3d_c2r(self._h, n, s, r, int(prune)))
+
+    def transfer_bytes(self):
+        """(host->device, device->host) bytes the chunked pipeline has copied so far."""
+        a, b = C.c_longlong(0), C.c_longlong(0)
+        self._check(self._L.mhd_transfer_bytes(self._h, C.byref(a), C.byref(b)))
+        return int(a.value), int(b.value)
 
     def launch_count(self):
         return int(self._L.mhd_launch_count(self._h))

@@ -121,6 +121,17 @@ void launch_sqrt_rho_u(long long n, const double* const U[8], double* const w[3]
 void launch_shell_spectrum(int N, const cd* const spec[3], const cd* const nyq[3], double* scratch, double* out,
                            int nspec, cudaStream_t st);
 int diag_scratch_doubles(int nspec);
+// slab-after-slab / brick-after-brick variants for the chunked pipeline: partials accumulate in a fixed order
+void launch_diag_partial(long long n, const double* const U[8], double gamma, double* part, int accumulate, cudaStream_t st);
+void launch_diag_final(const double* part, double* out, double inv_n, cudaStream_t st);
+void launch_absmax_partial(long long n, const double* f, double* part, int accumulate, cudaStream_t st);
+void launch_absmax_final(const double* part, double* out, cudaStream_t st);
+void launch_shell_spectrum_compact(const SpecGeom& g, const cd* const spec[3], double* part, int nspec, int accumulate,
+                                   cudaStream_t st);
+void launch_shell_spectrum_final(const double* part, double* out, int nspec, cudaStream_t st);
+int diag_partial_doubles();
+int absmax_partial_doubles();
+int spectrum_partial_doubles(int nspec);
 
 void launch_twiddle_table(int N, cd* tw, cudaStream_t st);
 

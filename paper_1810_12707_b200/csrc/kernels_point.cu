@@ -130,7 +130,7 @@ __global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 r
         R[7] = imul(kx, ey) - imul(ky, ex) - (ph.eta * k2) * u[7];
         if (mode == 0) {
 #pragma unroll
-            for (int f = 0; f < 8; ++f) rout.p[f][j] = R[f];
+            for (int f = 0; f < 8; ++f) rout.p[f][i] = R[f];     // work-array geometry (may alias the products)
         } else {
 #pragma unroll
             for (int f = 0; f < 8; ++f) {
@@ -143,7 +143,7 @@ __global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 r
         }
     } else if (mode == 0) {      // unpruned sweep: make the masked-out modes explicit zeros
 #pragma unroll
-        for (int f = 0; f < 8; ++f) rout.p[f][j] = mk(0, 0);
+        for (int f = 0; f < 8; ++f) rout.p[f][i] = mk(0, 0);
     }
 }
 void launch_assemble(const SpecGeom& g, const cd* const prod[16], cd* const U[8], cd* const Rold[8],
@@ -281,7 +281,7 @@ __device__ __forceinline__ void block_reduce(double (&v)[NRED], double* sh /*[NR
     for (int q = 0; q < NRED; ++q) v[q] = sh[q * RT];
 }
 
-__global__ void __launch_bounds__(RT) diag_stage1(long long n, PtrRC8 U, double gamma, double* part /*[RB][NRED]*/) {
+__global__ void __launch_bounds__(RT) diag_stage1(long long n, PtrRC8 U, double gamma, double* part /*[RB][NRED]*/, int accumulate) {
     __shared__ double sh[NRED * RT];
     double v[NRED];
 #pragma unroll
@@ -298,7 +298,10 @@ __global__ void __launch_bounds__(RT) diag_stage1(long long n, PtrRC8 U, double 
     }
     block_reduce(v, sh);
     if (threadIdx.x == 0)
-        for (int q = 0; q < NRED; ++q) part[blockIdx.x * NRED + q] = v[q];
+        for (int q = 0; q < NRED; ++q) {
+            double* p = &part[blockIdx.x * NRED + q];
+            *p = !accumulate ? v[q] : (q < 8 ? *p + v[q] : fmin(*p, v[q]));     // slab after slab, fixed order
+        }
 }
 __global__ void __launch_bounds__(RT) diag_stage2(const double* part, double* out, double inv_n) {
     __shared__ double sh[NRED * RT];
@@ -319,11 +322,21 @@ void launch_diag_reduce(long long n, const double* const U[8], double gamma, dou
                         cudaStream_t st) {
     PtrRC8 a;
     for (int c = 0; c < 8; ++c) a.p[c] = U[c];
-    diag_stage1<<<RB, RT, 0, st>>>(n, a, gamma, scratch);
+    diag_stage1<<<RB, RT, 0, st>>>(n, a, gamma, scratch, 0);
     diag_stage2<<<1, RT, 0, st>>>(scratch, out, 1.0 / (double)n);
 }
+void launch_diag_partial(long long n, const double* const U[8], double gamma, double* part, int accumulate, cudaStream_t st) {
+    PtrRC8 a;
+    for (int c = 0; c < 8; ++c) a.p[c] = U[c];
+    diag_stage1<<<RB, RT, 0, st>>>(n, a, gamma, part, accumulate);
+}
+void launch_diag_final(const double* part, double* out, double inv_n, cudaStream_t st) {
+    diag_stage2<<<1, RT, 0, st>>>(part, out, inv_n);
+}
+int diag_partial_doubles() { return RB * NRED; }
+int absmax_partial_doubles() { return RB; }
 
-__global__ void __launch_bounds__(RT) absmax_stage1(long long n, const double* f, double* part) {
+__global__ void __launch_bounds__(RT) absmax_stage1(long long n, const double* f, double* part, int accumulate) {
     __shared__ double sh[RT];
     double v = 0.0;
     for (long long i = blockIdx.x * (long long)RT + threadIdx.x; i < n; i += (long long)RB * RT) v = fmax(v, fabs(f[i]));
@@ -333,7 +346,7 @@ __global__ void __launch_bounds__(RT) absmax_stage1(long long n, const double* f
         if (threadIdx.x < s) sh[threadIdx.x] = fmax(sh[threadIdx.x], sh[threadIdx.x + s]);
         __syncthreads();
     }
-    if (threadIdx.x == 0) part[blockIdx.x] = sh[0];
+    if (threadIdx.x == 0) part[blockIdx.x] = accumulate ? fmax(part[blockIdx.x], sh[0]) : sh[0];
 }
 __global__ void __launch_bounds__(RT) absmax_stage2(const double* part, double* out) {
     __shared__ double sh[RT];
@@ -348,9 +361,13 @@ __global__ void __launch_bounds__(RT) absmax_stage2(const double* part, double* 
     if (threadIdx.x == 0) out[0] = sh[0];
 }
 void launch_absmax(long long n, const double* f, double* scratch, double* out, cudaStream_t st) {
-    absmax_stage1<<<RB, RT, 0, st>>>(n, f, scratch);
+    absmax_stage1<<<RB, RT, 0, st>>>(n, f, scratch, 0);
     absmax_stage2<<<1, RT, 0, st>>>(scratch, out);
 }
+void launch_absmax_partial(long long n, const double* f, double* part, int accumulate, cudaStream_t st) {
+    absmax_stage1<<<RB, RT, 0, st>>>(n, f, part, accumulate);
+}
+void launch_absmax_final(const double* part, double* out, cudaStream_t st) { absmax_stage2<<<1, RT, 0, st>>>(part, out); }
 
 // ---- shell spectra ---------------------------------------------------------------------------------------
 // S(K) = sum over the FULL mode cube with floor(|n|+1/2) = K of 1/2 sum_c |w^_c(n)|^2 / N^6.  The stored half
@@ -392,6 +409,41 @@ __global__ void spectrum_stage2(const double* part, double* out, int nspec) {
     for (int b = 0; b < SB; ++b) s += part[(long long)b * nspec + k];
     out[k] = s;
 }
+// compact bricks (chunked pipeline): only modes inside the mask are stored; partial sums accumulate brick after brick
+__global__ void __launch_bounds__(256) spectrum_compact_stage1(SpecGeom g, Ptr3 spec, double* part, int nspec, int accumulate) {
+    __shared__ double hist[MAXSPEC];
+    for (int k = threadIdx.x; k < nspec; k += blockDim.x) hist[k] = 0.0;
+    __syncthreads();
+    const int kc = g.kc, nxv = kc + 1, nzc = 2 * kc + 1;
+    const long long total = (long long)nxv * g.ny * nzc;
+    const double n3 = (double)g.N * g.N * g.N, norm = 0.5 / (n3 * n3);
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)SB * blockDim.x) {
+        const int ix = (int)(i % nxv), oy = (int)((i / nxv) % g.ny), oz = (int)(i / ((long long)nxv * g.ny));
+        const int cy = oy + g.y0;
+        const int ny = cy <= kc ? cy : cy - nzc, nz = oz <= kc ? oz : oz - nzc;
+        const long long j = (long long)oz * g.ssz + (long long)oy * g.ssy + ix;
+        double e = 0.0;
+        for (int c = 0; c < 3; ++c) { const cd a = spec.p[c][j]; e += a.x * a.x + a.y * a.y; }
+        const int K = (int)floor(sqrt((double)(ix * ix + ny * ny + nz * nz)) + 0.5);
+        if (e != 0.0) atomicAdd(&hist[K], (ix == 0 ? 1.0 : 2.0) * norm * e);
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < nspec; k += blockDim.x) {
+        double* p = &part[(long long)blockIdx.x * nspec + k];
+        *p = accumulate ? *p + hist[k] : hist[k];
+    }
+}
+void launch_shell_spectrum_compact(const SpecGeom& g, const cd* const spec[3], double* part, int nspec, int accumulate,
+                                   cudaStream_t st) {
+    Ptr3 a;
+    for (int c = 0; c < 3; ++c) a.p[c] = spec[c];
+    spectrum_compact_stage1<<<SB, 256, 0, st>>>(g, a, part, nspec, accumulate);
+}
+void launch_shell_spectrum_final(const double* part, double* out, int nspec, cudaStream_t st) {
+    spectrum_stage2<<<(nspec + 127) / 128, 128, 0, st>>>(part, out, nspec);
+}
+int spectrum_partial_doubles(int nspec) { return SB * nspec; }
+
 void launch_shell_spectrum(int N, const cd* const spec[3], const cd* const nyq[3], double* scratch, double* out,
                            int nspec, cudaStream_t st) {
     Ptr3 a, b;

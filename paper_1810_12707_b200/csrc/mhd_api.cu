@@ -8,115 +8,11 @@
 //   S4  forward y pass, in place
 //   S5  forward z pass ; assembly of R^ (i k, -k^2, mask) and the explicit update
 // No host round trip inside mhd_step: only kernel launches on the bound stream.
-#include "../../include/mhd.h"
-#include "kernels.h"
-
-#include <algorithm>
-#include <cmath>
-#include <cstdio>
-#include <cstring>
-#include <new>
-#include <string>
-#include <vector>
+#include "ctx.h"
 
 using namespace mhd;
 
 namespace {
-
-enum Family { F_STRIDED_INV = 0, F_STRIDED_FWD, F_X_FUSED, F_X_C2R, F_X_R2C, F_FLUX, F_CURRENT, F_ASSEMBLE, F_AXPBY,
-              F_POINT, F_DIAG, F_COUNT };
-const char* kFamilyNames[F_COUNT] = {"strided_inverse", "strided_forward", "x_fused", "x_c2r", "x_r2c", "flux_real",
-                                     "build_current", "assemble", "axpby", "pointwise_misc", "diagnostics"};
-
-size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
-
-constexpr int NFIELD_BUFS = 48;   // U 8, Rold 8, W 16, X 8, Y 8
-
-struct Layout {
-    size_t field_bytes, tw_off, ftw_off, field_off, nyq_off, nyq_bytes, scratch_off, scratch_bytes, res_off, total;
-};
-int nspec_of(int N) { return (int)std::ceil(std::sqrt(3.0) * N / 2.0) + 1; }
-Layout make_layout(int N) {
-    Layout l;
-    l.field_bytes = (size_t)N * N * N * sizeof(double);
-    size_t off = 0;
-    l.tw_off = off; off += align_up((size_t)N * sizeof(cd));
-    l.ftw_off = off; off += align_up((size_t)(4 * N + 64) * sizeof(cd));
-    l.field_off = off; off += (size_t)NFIELD_BUFS * align_up(l.field_bytes);
-    l.nyq_bytes = align_up((size_t)N * N * 8 * sizeof(cd));
-    l.nyq_off = off; off += 3 * l.nyq_bytes;
-    l.scratch_bytes = align_up((size_t)diag_scratch_doubles(nspec_of(N)) * sizeof(double));
-    l.scratch_off = off; off += l.scratch_bytes;
-    l.res_off = off; off += align_up((size_t)(64 + 2 * nspec_of(N)) * sizeof(double));
-    l.total = off;
-    return l;
-}
-bool valid_N(int N) { return N >= 16 && N <= 1024 && (N & (N - 1)) == 0; }
-
-}  // namespace
-
-struct mhd_ctx {
-    int N = 0;
-    double L = 0, gamma = 0, mu = 0, eta = 0, dt = 0;
-    bool bound = false, have_fields = false, have_old = false;
-    cudaStream_t st = nullptr;
-    unsigned flags = 0;
-    int opt_fused = 1, opt_prune = 1, opt_fuse_current = 1, integrator = 0;
-    long long step = 0;
-    long long launches = 0;
-    std::string err;
-    // device storage (inside the caller's workspace)
-    cd* tw = nullptr;
-    cd* ftw = nullptr;     // lane-contiguous tables of the fused x sweep
-    cd *U[8], *Rold[8], *W[16], *X[8], *Y[8], *nyq[3];
-    double *scratch = nullptr, *res = nullptr;
-    // profiling
-    bool prof = false;
-    struct Rec { int fam; cudaEvent_t a, b; };
-    std::vector<Rec> recs;
-    std::vector<cudaEvent_t> pool;
-    double fam_ms[F_COUNT] = {0};
-    long long fam_n[F_COUNT] = {0};
-
-    int fail(int code, const std::string& m) { err = m; return code; }
-    int hx() const { return N / 2; }
-    int kc() const { return N / 3; }
-    long long n3() const { return (long long)N * N * N; }
-    Phys phys() const { return Phys{2.0 * M_PI / L, gamma, mu, eta}; }
-    SpecGeom geom() const { return SpecGeom{N, N / 2, N / 3, opt_prune}; }
-
-    cudaEvent_t get_event() {
-        if (!pool.empty()) { cudaEvent_t e = pool.back(); pool.pop_back(); return e; }
-        cudaEvent_t e; cudaEventCreate(&e); return e;
-    }
-    struct Scope {
-        mhd_ctx* c; int fam; cudaEvent_t a = nullptr;
-        Scope(mhd_ctx* c_, int fam_, int nlaunch = 1) : c(c_), fam(fam_) {
-            c->launches += nlaunch; c->fam_n[fam] += nlaunch;
-            if (c->prof) { a = c->get_event(); cudaEventRecord(a, c->st); }
-        }
-        ~Scope() {
-            if (a) { cudaEvent_t b = c->get_event(); cudaEventRecord(b, c->st); c->recs.push_back({fam, a, b}); }
-        }
-    };
-    void drain_profile() {
-        if (recs.empty()) return;
-        cudaStreamSynchronize(st);
-        for (auto& r : recs) {
-            float ms = 0; cudaEventElapsedTime(&ms, r.a, r.b);
-            fam_ms[r.fam] += ms; pool.push_back(r.a); pool.push_back(r.b);
-        }
-        recs.clear();
-    }
-};
-
-namespace {
-
-int check_cuda(mhd_ctx* c, const char* what) {
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return c->fail(MHD_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
-    return MHD_OK;
-}
 
 // ---- sweeps --------------------------------------------------------------------------------------------------
 // strided pass over nf arrays; axis 1 = y, 2 = z; hx = row pitch of the arrays (N/2, or 8 for the Nyquist planes)
@@ -197,6 +93,24 @@ void forward3d(mhd_ctx* c, int nf, const double* const real_in[], cd* const spec
     }
 }
 
+}  // namespace
+
+void run_x_fused(mhd_ctx* c, cd* const in[11], cd* const out[16], long long nlines) {
+    const int N = c->N;
+    const bool prune = c->opt_prune != 0 || c->ooc.on;
+    const int kmax = prune ? c->kc() : c->hx() - 1;
+    FusedXArgs a; std::memset(&a, 0, sizeof(a));
+    for (int f = 0; f < 11; ++f) a.in[f] = in[f];
+    for (int f = 0; f < 16; ++f) a.out[f] = out[f];
+    a.tw = c->tw; a.nlines = nlines; a.kmax_in = kmax; a.kmax_out = kmax;
+    a.scale = 1.0 / ((double)N * N * N); a.ph = c->phys();
+    mhd_ctx::Scope s(c, F_X_FUSED);
+    if (c->opt_fused != 2 && x_fused2_supported(N)) { a.tw = c->ftw; launch_x_fused2(N, a, c->st); }
+    else launch_x_fused(N, a, c->st);
+}
+
+namespace {
+
 // products W[0..15] <- state Uin (k-space); sweeps S1-S4 and the forward z pass of S5
 void products(mhd_ctx* c, cd* const Uin[8]) {
     const int N = c->N;
@@ -220,13 +134,7 @@ void products(mhd_ctx* c, cd* const Uin[8]) {
     const int kmax = prune ? c->kc() : c->hx() - 1;
     const double scale = 1.0 / ((double)N * N * N);
     if (c->opt_fused) {                                                   // S3
-        FusedXArgs a; std::memset(&a, 0, sizeof(a));
-        for (int f = 0; f < 11; ++f) a.in[f] = c->W[f];
-        for (int f = 0; f < 16; ++f) a.out[f] = c->W[f];
-        a.tw = c->tw; a.nlines = (long long)N * N; a.kmax_in = kmax; a.kmax_out = kmax; a.scale = scale; a.ph = ph;
-        mhd_ctx::Scope s(c, F_X_FUSED);
-        if (c->opt_fused == 1 && x_fused2_supported(N)) { a.tw = c->ftw; launch_x_fused2(N, a, c->st); }
-        else launch_x_fused(N, a, c->st);
+        run_x_fused(c, c->W, c->W, (long long)N * N);
     } else {
         XArgs a; std::memset(&a, 0, sizeof(a));
         for (int f = 0; f < 11; ++f) { a.spec_in[f] = c->W[f]; a.real_out[f] = reinterpret_cast<double*>(c->W[f]); }
@@ -287,22 +195,29 @@ int mhd_init(mhd_ctx** out, int N, double L, double gamma, double mu, double eta
     return MHD_OK;
 }
 
+static bool flags_valid(unsigned flags) {
+    if ((flags & 0xF8u) != 0) return false;                                 // unknown bits
+    if (!(flags & MHD_FLAG_OUT_OF_CORE)) return flags == 0;                 // placement / budget need the chunked pipeline
+    return true;
+}
 size_t mhd_workspace_bytes(int N, unsigned flags) {
-    (void)flags;
-    if (!valid_N(N)) return 0;
+    if (!valid_N(N) || !flags_valid(flags)) return 0;
+    if (flags & MHD_FLAG_OUT_OF_CORE) return ooc_workspace_bytes(N, flags);
     return make_layout(N).total;
 }
-size_t mhd_pinned_bytes(int N, unsigned flags) { (void)N; (void)flags; return 0; }
+size_t mhd_pinned_bytes(int N, unsigned flags) {
+    if (!valid_N(N) || !flags_valid(flags) || !(flags & MHD_FLAG_OUT_OF_CORE)) return 0;
+    return ooc_pinned_bytes(N, flags);
+}
 int mhd_nspec(int N) { return nspec_of(N); }
 
 int mhd_bind(mhd_ctx* c, void* dev_workspace, size_t bytes, void* cuda_stream, unsigned flags, void* pinned_host,
              size_t pinned_bytes) {
     if (!c) return MHD_ERR_INVALID_ARG;
-    (void)pinned_host; (void)pinned_bytes;
-    if (flags & MHD_FLAG_OUT_OF_CORE) return c->fail(MHD_ERR_INVALID_ARG, "out-of-core path not available in this build");
-    const Layout l = make_layout(c->N);
+    if (!flags_valid(flags)) return c->fail(MHD_ERR_INVALID_ARG, "invalid flags");
     if (!dev_workspace || ((uintptr_t)dev_workspace & 255) != 0) return c->fail(MHD_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
-    if (bytes < l.total) return c->fail(MHD_ERR_NOMEM, "workspace too small");
+    const Layout l = make_layout(c->N);
+    if (!(flags & MHD_FLAG_OUT_OF_CORE) && bytes < l.total) return c->fail(MHD_ERR_NOMEM, "workspace too small");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
         cudaGetLastError();
@@ -311,6 +226,13 @@ int mhd_bind(mhd_ctx* c, void* dev_workspace, size_t bytes, void* cuda_stream, u
     char* base = static_cast<char*>(dev_workspace);
     c->st = static_cast<cudaStream_t>(cuda_stream);
     c->flags = flags;
+    if (flags & MHD_FLAG_OUT_OF_CORE) {
+        int rc = ooc_bind(c, base, bytes, static_cast<char*>(pinned_host), pinned_bytes);
+        if (rc) return rc;
+        c->bound = true; c->have_fields = false; c->have_old = false; c->step = 0;
+        return MHD_OK;
+    }
+    c->ooc.on = false;
     c->tw = reinterpret_cast<cd*>(base + l.tw_off);
     c->ftw = reinterpret_cast<cd*>(base + l.ftw_off);
     const size_t fb = align_up(l.field_bytes);
@@ -344,6 +266,12 @@ int mhd_set_option(mhd_ctx* c, int option, int value) {
         case MHD_OPT_INTEGRATOR:
             if (value < 0 || value > 2) return c->fail(MHD_ERR_INVALID_ARG, "integrator must be 0, 1 or 2");
             c->integrator = value; c->have_old = false; return MHD_OK;
+        case MHD_OPT_OOC_BRICK:
+            if (value < 0) return c->fail(MHD_ERR_INVALID_ARG, "brick size must be >= 0");
+            c->ooc.brick_max = value; return MHD_OK;
+        case MHD_OPT_OOC_SLAB:
+            if (value < 0) return c->fail(MHD_ERR_INVALID_ARG, "slab size must be >= 0");
+            c->ooc.slab_max = value; return MHD_OK;
         default: return c->fail(MHD_ERR_INVALID_ARG, "unknown option");
     }
 }
@@ -352,6 +280,12 @@ int mhd_set_fields(mhd_ctx* c, int kind, int where, const double* const f[8]) {
     if (!c || !f) return MHD_ERR_INVALID_ARG;
     if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
     if ((kind != 0 && kind != 1) || (where != 0 && where != 1)) return c->fail(MHD_ERR_INVALID_ARG, "kind/where");
+    if (c->ooc.on) {
+        int rc = ooc_set_fields(c, kind, where, f);
+        if (rc) return rc;
+        c->have_fields = true; c->have_old = false; c->step = 0;
+        return MHD_OK;
+    }
     double* real[8];
     for (int i = 0; i < 8; ++i) real[i] = reinterpret_cast<double*>(c->W[i]);
     int rc = copy_in(c, where, f, real);
@@ -382,6 +316,7 @@ int mhd_rhs(mhd_ctx* c, int where, double* const out[8]) {
     if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
     if (!c->have_fields) return c->fail(MHD_ERR_NO_FIELDS, "mhd_set_fields has not been called");
     if (where != 0 && where != 1) return c->fail(MHD_ERR_INVALID_ARG, "where");
+    if (c->ooc.on) return ooc_rhs(c, where, out);
     rhs_spectral(c, c->U, c->X, 0);
     double* real[8];
     for (int i = 0; i < 8; ++i) real[i] = (where == MHD_DEVICE) ? out[i] : reinterpret_cast<double*>(c->X[i]);
@@ -394,6 +329,7 @@ int mhd_step(mhd_ctx* c, int nsteps) {
     if (!c || nsteps < 0) return MHD_ERR_INVALID_ARG;
     if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
     if (!c->have_fields) return c->fail(MHD_ERR_NO_FIELDS, "mhd_set_fields has not been called");
+    if (c->ooc.on) return ooc_step(c, nsteps);
     const SpecGeom g = c->geom();
     SpecGeom gp = g; gp.pruned = 1;
     for (int s = 0; s < nsteps; ++s) {
@@ -442,6 +378,7 @@ int mhd_get_fields(mhd_ctx* c, int kind, int where, double* const out[8]) {
     if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
     if (!c->have_fields) return c->fail(MHD_ERR_NO_FIELDS, "mhd_set_fields has not been called");
     if ((kind != 0 && kind != 1) || (where != 0 && where != 1)) return c->fail(MHD_ERR_INVALID_ARG, "kind/where");
+    if (c->ooc.on) return ooc_get_fields(c, kind, where, out);
     double* real[8];
     for (int i = 0; i < 8; ++i) real[i] = (where == MHD_DEVICE) ? out[i] : reinterpret_cast<double*>(c->W[i]);
     inverse3d(c, 8, c->U, c->W, real, true);
@@ -455,6 +392,7 @@ int mhd_diagnostics(mhd_ctx* c, mhd_diag* d, double* spec_kin, double* spec_mag,
     if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
     if (!c->have_fields) return c->fail(MHD_ERR_NO_FIELDS, "mhd_set_fields has not been called");
     const int ns = nspec_of(c->N);
+    if (c->ooc.on) return ooc_diagnostics(c, d, spec_kin, spec_mag, nspec);
     if ((spec_kin || spec_mag) && nspec != ns) return c->fail(MHD_ERR_INVALID_ARG, "nspec must equal mhd_nspec(N)");
     const long long n3 = c->n3();
     double* real[8];
@@ -504,6 +442,7 @@ int mhd_diagnostics(mhd_ctx* c, mhd_diag* d, double* spec_kin, double* spec_mag,
 int mhd_fft3d_r2c(mhd_ctx* c, int nfields, const double* const real[], double* const spec[], double* const nyq[], int prune) {
     if (!c || !real || !spec || nfields < 1) return MHD_ERR_INVALID_ARG;
     if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
+    if (c->ooc.on) return c->fail(MHD_ERR_INVALID_ARG, "mhd_fft3d_* needs an in-core context");
     std::vector<cd*> sp(nfields), nq(nfields);
     for (int f = 0; f < nfields; ++f) { sp[f] = reinterpret_cast<cd*>(spec[f]); nq[f] = nyq ? reinterpret_cast<cd*>(nyq[f]) : nullptr; }
     forward3d(c, nfields, real, sp.data(), (nyq && !prune) ? nq.data() : nullptr, prune != 0);
@@ -512,6 +451,7 @@ int mhd_fft3d_r2c(mhd_ctx* c, int nfields, const double* const real[], double* c
 int mhd_fft3d_c2r(mhd_ctx* c, int nfields, double* const spec[], double* const real[], int prune) {
     if (!c || !real || !spec || nfields < 1) return MHD_ERR_INVALID_ARG;
     if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
+    if (c->ooc.on) return c->fail(MHD_ERR_INVALID_ARG, "mhd_fft3d_* needs an in-core context");
     std::vector<cd*> sp(nfields); std::vector<const cd*> spc(nfields);
     for (int f = 0; f < nfields; ++f) { sp[f] = reinterpret_cast<cd*>(spec[f]); spc[f] = sp[f]; }
     inverse3d(c, nfields, spc.data(), sp.data(), real, prune != 0);
@@ -519,6 +459,13 @@ int mhd_fft3d_c2r(mhd_ctx* c, int nfields, double* const spec[], double* const r
 }
 
 long long mhd_launch_count(const mhd_ctx* c) { return c ? c->launches : 0; }
+
+int mhd_transfer_bytes(const mhd_ctx* c, long long* h2d, long long* d2h) {
+    if (!c) return MHD_ERR_INVALID_ARG;
+    if (h2d) *h2d = c->ooc.h2d_bytes;
+    if (d2h) *d2h = c->ooc.d2h_bytes;
+    return MHD_OK;
+}
 
 int mhd_profile_enable(mhd_ctx* c, int on) {
     if (!c) return MHD_ERR_INVALID_ARG;
@@ -532,7 +479,7 @@ int mhd_profile_get(mhd_ctx* c, int max_entries, const char** names, double* ms,
     c->drain_profile();
     int n = 0;
     for (int i = 0; i < F_COUNT && n < max_entries; ++i, ++n) {
-        if (names) names[n] = kFamilyNames[i];
+        if (names) names[n] = family_name(i);
         if (ms) ms[n] = c->fam_ms[i];
         if (launches) launches[n] = c->fam_n[i];
     }
@@ -544,6 +491,7 @@ const char* mhd_last_error(const mhd_ctx* c) { return c ? c->err.c_str() : "null
 int mhd_destroy(mhd_ctx* c) {
     if (!c) return MHD_OK;
     if (c->bound) c->drain_profile();
+    ooc_destroy(c);
     for (auto e : c->pool) cudaEventDestroy(e);
     delete c;
     return MHD_OK;

@@ -61,6 +61,26 @@ def test_workspace_sizes(lib):
     assert lib.mhd_nspec(32) == 29 and lib.mhd_nspec(256) == 223
 
 
+def test_chunked_pipeline_sizes(lib):
+    """Placement arithmetic of the out-of-core path (config 6, 1024^3): compact storage fits one B200 entirely;
+    with the state and the work fields in pinned host memory the device part is a few GB of staging."""
+    OOC, STATE, WORK = 1, 2, 4
+    kc = 1024 // 3
+    compact = (2 * kc + 1) ** 2 * ((kc + 1 + 7) // 8 * 8) * 16
+    zfull = 1024 * (2 * kc + 1) * ((kc + 1 + 7) // 8 * 8) * 16
+    all_dev = lib.mhd_workspace_bytes(1024, OOC)
+    assert 16 * compact + 16 * zfull < all_dev < 120e9 and lib.mhd_pinned_bytes(1024, OOC) == 0
+    t1 = lib.mhd_workspace_bytes(1024, OOC | STATE)
+    assert 16 * zfull < t1 < all_dev and 16 * compact <= lib.mhd_pinned_bytes(1024, OOC | STATE) < 16 * compact + 16 * 256
+    t2 = lib.mhd_workspace_bytes(1024, OOC | STATE | WORK)
+    assert 0 < t2 < 16e9
+    assert lib.mhd_pinned_bytes(1024, OOC | STATE | WORK) >= 16 * (compact + zfull)
+    # the paper's scenario (PAPER.md L375: 512^3 on a 16 GB P100): fits a 16 GiB budget with everything on the host
+    assert 0 < lib.mhd_workspace_bytes(512, OOC | STATE | WORK | (16384 << 8)) <= 16384 << 20
+    assert lib.mhd_workspace_bytes(512, OOC | 0x80) == 0      # unknown flag bit
+    assert lib.mhd_workspace_bytes(512, STATE) == 0           # placement without the chunked pipeline
+
+
 def test_bind_without_device_fails_loudly(lib):
     import torch
     if torch.cuda.is_available():
