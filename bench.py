@@ -138,7 +138,7 @@ def run_reference(args):
         return 0
     import oracle
     from paper_1810_12707_b200 import inputs
-    n = 64
+    n = 128
     cfg = inputs.config45(n)
     o = oracle.Oracle(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
     o.set_fields(cfg.prim, "primitive")
@@ -150,7 +150,7 @@ def run_reference(args):
     dt = time.perf_counter() - t0
     value = n ** 3 * args.steps / dt
     cores = oracle.get_threads()
-    sample = "config 4/5 initial condition on a 64^3 grid, %d AB2 steps (bounded sample of the %d^3 workload)" % (args.steps, args.size)
+    sample = "config 4/5 initial condition on a %d^3 grid, %d AB2 steps (bounded sample of the %d^3 workload)" % (n, args.steps, args.size)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -165,7 +165,7 @@ def run_reference(args):
 def cpu_baseline(size):
     import oracle
     from paper_1810_12707_b200 import inputs
-    n, steps = 64, 12
+    n, steps = 128, 12
     cfg = inputs.config45(n)
     o = oracle.Oracle(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
     o.set_fields(cfg.prim, "primitive")
@@ -174,8 +174,8 @@ def cpu_baseline(size):
     o.step(steps)
     dt = time.perf_counter() - t0
     return {"value": n ** 3 * steps / dt, "unit": UNIT, "cores": oracle.get_threads(), "kind": "oracle",
-            "sample": "config 4/5 initial condition on a 64^3 grid, %d AB2 steps, %.1f s (bounded sample of the %d^3 workload)"
-                      % (steps, dt, size)}
+            "sample": "config 4/5 initial condition on a %d^3 grid, %d AB2 steps, %.1f s (bounded sample of the %d^3 workload)"
+                      % (n, steps, dt, size)}
 
 
 def time_steps(g, torch, nsteps, dist):
@@ -247,9 +247,18 @@ def run_ours(args):
     from paper_1810_12707_b200 import MHD, inputs
 
     N = args.size
-    cfg = inputs.config45(N)
-    g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, device="cuda:%d" % local_rank)
-    host = [torch.from_numpy(p).pin_memory() for p in cfg.prim]      # pinned host inputs
+    from paper_1810_12707_b200 import binding as B
+    flags = {"incore": 0, "device": B.MHD_FLAG_OUT_OF_CORE, "state_host": B.MHD_FLAG_OUT_OF_CORE | B.MHD_FLAG_STATE_ON_HOST,
+             "all_host": B.MHD_FLAG_OUT_OF_CORE | B.MHD_FLAG_STATE_ON_HOST | B.MHD_FLAG_WORK_ON_HOST}[args.placement]
+    if args.budget_mib:
+        flags |= B.MHD_FLAG_BUDGET_MIB(args.budget_mib)
+    if N == 1024 and not flags:
+        print(json.dumps({"error": "1024^3 does not fit in core (48 full fields = 412 GB): use --placement device|state_host|all_host"}))
+        return 2
+    cfg = inputs.config6(N) if N == 1024 else inputs.config45(N)     # config 6 = the out-of-core workload of BASELINE.json
+    g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, device="cuda:%d" % local_rank, flags=flags)
+    pin_inputs = N < 1024        # 8 x 8.6 GB of inputs stay pageable at 1024^3 (the pinned budget goes to the solver's arrays)
+    host = [torch.from_numpy(p).pin_memory() if pin_inputs else torch.from_numpy(p) for p in cfg.prim]
     cfg.prim = None
     opts = {}
     for kv in args.option:
@@ -257,6 +266,8 @@ def run_ours(args):
         opts[int(k)] = int(v)
         g.set_option(int(k), int(v))
     g.set_fields(host, "primitive")
+    if args.no_e2e:
+        host = None          # frees the input copies (matters at 1024^3: 69 GB)
     K, W = args.steps, max(args.warmup, 3)
 
     # ---- device-resident timing -----------------------------------------------------------------------------
@@ -267,6 +278,18 @@ def run_ours(args):
     ms = time_steps(g, torch, K, dist)
     launches = g.launch_count() - l0
     prof = g.profile_get()
+    ooc = None
+    if flags:
+        g.profile_enable(False)
+        x0 = g.transfer_bytes()
+        ms_np = time_steps(g, torch, K, dist)          # without the per-family events (they serialise nothing, but to be sure)
+        x1 = g.transfer_bytes()
+        ms = ms_np
+        ooc = {"placement": args.placement, "budget_mib": args.budget_mib, "device_workspace_gb": g.workspace_bytes / 1e9,
+               "pinned_host_gb": g.pinned_bytes / 1e9, "in_core_workspace_gb": 48 * 8.0 * N ** 3 / 1e9,
+               "h2d_bytes_per_step": (x1[0] - x0[0]) / K, "d2h_bytes_per_step": (x1[1] - x0[1]) / K,
+               "h2d_gbs": (x1[0] - x0[0]) / ms_np / 1e6, "d2h_gbs": (x1[1] - x0[1]) / ms_np / 1e6,
+               "s_per_step": ms_np / K / 1e3}
     g.profile_enable(False)
     clocks = sampler.stop()
     ms_max, units = aggregate(ms, float(N) ** 3 * K, dist)
@@ -327,11 +350,12 @@ def run_ours(args):
         ms_e, units_e = aggregate(t_e2e, float(N) ** 3 * K, dist)
         fb = 8.0 * N ** 3 * 8
         e2e = {"value": units_e / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": fb / K, "d2h_bytes_per_step": fb / K,
-               "what": "mhd_set_fields(pinned host) + mhd_step(%d) + mhd_get_fields(pinned host), wall clock" % K}
+               "what": "mhd_set_fields(%s host) + mhd_step(%d) + mhd_get_fields(%s host), wall clock"
+                       % ("pinned" if pin_inputs else "pageable", K, "pinned" if pin_inputs else "pageable")}
 
     extra = {}
-    if rank == 0 and not args.no_fft:
-        del host
+    if rank == 0 and not args.no_fft and not flags:
+        host = None
         extra["fft3d"] = fft_metric(g, torch, N)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
@@ -341,11 +365,12 @@ def run_ours(args):
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
                 "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
-                "config": {"workload": "config%d_abc_dynamo_%d^3" % (5 if N == 512 else 4, N), "N": N, "dt": cfg.dt,
+                "config": {"workload": ("config6_turbulence_out_of_core_%d^3" % N) if N == 1024 else
+                           "config%d_abc_dynamo_%d^3" % (5 if N == 512 else 4, N), "N": N, "dt": cfg.dt, "placement": args.placement,
                            "mu": cfg.mu, "eta": cfg.eta, "integrator": "AB2", "fused": 1, "pruned": 1,
                            "parallelism": "replicas x%d" % world,
                            "l2": "no flush: one step streams %.1f GB, far beyond the 126 MB L2" % (alg_pruned / 1e9)},
-                "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
+                "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "out_of_core": ooc,
                 "paper_context": {"256^3 s/step P100/V100": [0.32, 0.22], "512^3 s/step P100/V100 (out-of-core)": [80.97, 92.81],
                                   "source": "PAPER.md Table III L368-375; other hardware, context only"}}
         line.update(extra)
@@ -361,7 +386,11 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--size", type=int, default=512, choices=[64, 128, 256, 512])
+    ap.add_argument("--size", type=int, default=512, choices=[64, 128, 256, 512, 1024])
+    ap.add_argument("--placement", default="incore", choices=["incore", "device", "state_host", "all_host"],
+                    help="incore: the tuned in-core path; others: the chunked pipeline (include/mhd.h MHD_FLAG_OUT_OF_CORE) with "
+                         "everything in HBM / U^ and R^old in pinned host memory / the work fields there too")
+    ap.add_argument("--budget-mib", type=int, default=0, help="cap on the device workspace of the chunked pipeline")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-fft", action="store_true")

@@ -355,8 +355,10 @@ int stage_slabs(mhd_ctx* c, SlabKind kind, const SlabIO& io) {
 }
 
 // ---- stage C: forward z pass of the 16 products, assembly of R^ and the explicit update (mode 1 Euler, 2 AB2);
-//      mode 0 (mhd_rhs): R^ replaces the first 8 work fields and is inverse-z-transformed on the spot --------------------
-int stage_forward_z_assemble(mhd_ctx* c, int mode) {
+//      mode 0 (mhd_rhs): R^ replaces the first 8 work fields and is inverse-z-transformed on the spot.
+//      next_inverse (modes 1, 2): stage A of the NEXT step runs on the freshly updated brick while it is still on the
+//      device (the z pass is local to a brick), which saves one host->device pass over U^ per step ----------------------
+int stage_forward_z_assemble(mhd_ctx* c, int mode, bool next_inverse) {
     Ooc& o = c->ooc;
     stage_begin(c);
     const auto chunks = brick_chunks(c);
@@ -377,11 +379,19 @@ int stage_forward_z_assemble(mhd_ctx* c, int mode) {
             launch_assemble(g, w.p, u.p, mode != 0 ? r.p : nullptr, mode == 0 ? w.p : nullptr, mode, c->dt, c->phys(), c->st);
         }
         if (mode == 0) gen_pass(c, +1, 8, w.p, w.p, w.rs, o.nxp, 2, w.rs, o.nxp, 0, ny);
-        const bool d2h = mode == 0 ? o.work_host : o.state_host;
+        if (mode != 0 && next_inverse) {
+            const cd* in[11];
+            for (int f = 0; f < 11; ++f) in[f] = u.p[f < 8 ? f : 5];
+            gen_pass(c, +1, 11, in, w.p, u.rs, o.nxp, 2, w.rs, o.nxp, 0, ny, 8, 5, y0);
+        }
+        const bool d2h = mode == 0 ? o.work_host : (o.state_host || (next_inverse && o.work_host));
         chunk_comp_done(c, ch, d2h);
         if (d2h) {
             if (mode == 0) work_store(c, w, 8, y0);
-            else { state_store(c, u, o.Uc, 8, y0); state_store(c, r, o.Rc, 8, y0); }
+            else {
+                state_store(c, u, o.Uc, 8, y0); state_store(c, r, o.Rc, 8, y0);
+                if (next_inverse) work_store(c, w, 11, y0);
+            }
             chunk_d2h_done(c, ch);
         }
     }
@@ -538,9 +548,11 @@ int ooc_get_fields(mhd_ctx* c, int kind, int where, double* const out[8]) {
     return check_cuda(c, "get_fields (chunked)");
 }
 
-static int ooc_products(mhd_ctx* c) {
-    int rc = stage_inverse_z(c, c->ooc.Uc, true);
-    if (rc) return rc;
+static int ooc_products(mhd_ctx* c, bool have_inverse_z = false) {
+    if (!have_inverse_z) {
+        int rc = stage_inverse_z(c, c->ooc.Uc, true);
+        if (rc) return rc;
+    }
     SlabIO io; io.nin = 11; io.nout = 16;
     return stage_slabs(c, SLAB_FLUX, io);
 }
@@ -549,7 +561,7 @@ int ooc_rhs(mhd_ctx* c, int where, double* const out[8]) {
     for (int i = 0; i < 8; ++i) if (!out[i]) return c->fail(MHD_ERR_INVALID_ARG, "null field pointer");
     int rc = ooc_products(c);
     if (rc) return rc;
-    rc = stage_forward_z_assemble(c, 0);
+    rc = stage_forward_z_assemble(c, 0, false);
     if (rc) return rc;
     SlabIO io; io.nin = 8; io.nout = 0; io.kind = MHD_CONSERVATIVE; io.where = where; io.user_out = out;
     rc = stage_slabs(c, SLAB_TO_REAL, io);
@@ -561,9 +573,9 @@ int ooc_rhs(mhd_ctx* c, int where, double* const out[8]) {
 int ooc_step(mhd_ctx* c, int nsteps) {
     if (c->integrator != 0) return c->fail(MHD_ERR_INVALID_ARG, "the chunked pipeline implements Adams-Bashforth only");
     for (int s = 0; s < nsteps; ++s) {
-        int rc = ooc_products(c);
+        int rc = ooc_products(c, s > 0);
         if (rc) return rc;
-        rc = stage_forward_z_assemble(c, c->have_old ? 2 : 1);
+        rc = stage_forward_z_assemble(c, c->have_old ? 2 : 1, s + 1 < nsteps);
         if (rc) return rc;
         c->have_old = true;
         ++c->step;

@@ -69,8 +69,8 @@ def random_solenoidal(N: int, kmin: float, kmax: float, p: float, seed: int, str
         raise ValueError("kmax must stay below the Nyquist mode")
     modes = half_space_modes(kmin, kmax)
     nh = N // 2 + 1
-    Vh = [np.zeros((N, N, nh), dtype=np.complex128) for _ in range(3)]
-    scale = 0.5 * float(N) ** 3  # cos(n.x+phi) = (e^{i(n.x+phi)} + c.c.)/2 ; numpy irfftn divides by N^3
+    scale = 0.5 * float(N) ** 3  # cos(n.x+phi) = (e^{i(n.x+phi)} + c.c.)/2 ; the inverse FFT divides by N^3
+    entries = [[], [], []]       # per component: ((iz, iy, ix), value) of the half spectrum
     for (nx, ny, nz) in modes:
         amp = (nx * nx + ny * ny + nz * nz) ** (0.5 * p)
         a = [amp * complex(math.cos(ph), math.sin(ph)) * scale
@@ -78,13 +78,40 @@ def random_solenoidal(N: int, kmin: float, kmax: float, p: float, seed: int, str
         # V^ = i n x A^
         v = (1j * (ny * a[2] - nz * a[1]), 1j * (nz * a[0] - nx * a[2]), 1j * (nx * a[1] - ny * a[0]))
         for c in range(3):
-            Vh[c][nz % N, ny % N, nx] += v[c]
+            entries[c].append(((nz % N, ny % N, nx), v[c]))
             if nx == 0:  # the kx = 0 plane holds both members of the pair
-                Vh[c][(-nz) % N, (-ny) % N, 0] += np.conj(v[c])
-    V = [np.fft.irfftn(Vh[c], s=(N, N, N), axes=(0, 1, 2)) for c in range(3)]
-    ms = float(np.mean(V[0] ** 2 + V[1] ** 2 + V[2] ** 2))
+                entries[c].append((((-nz) % N, (-ny) % N, 0), v[c].conjugate()))
+    V = [_synthesise(N, nh, entries[c]) for c in range(3)]
+    ms = float(np.mean(V[0] ** 2) + np.mean(V[1] ** 2) + np.mean(V[2] ** 2))
     f = rms / math.sqrt(ms)
-    return tuple(np.ascontiguousarray(v * f) for v in V)
+    for v in V:
+        v *= f
+    return tuple(V)
+
+
+def _synthesise(N: int, nh: int, entries):
+    """Real field [N][N][N] from a sparse list of half-spectrum entries (inverse real FFT, input synthesis only).
+    Large grids use torch's FFT on the GPU when one is present (minutes -> seconds at 1024^3); the harness may use
+    a library FFT, the product path never does."""
+    if N >= 512:
+        try:
+            import torch
+            if torch.cuda.is_available():
+                Vh = torch.zeros((N, N, nh), dtype=torch.complex128, device="cuda")
+                for (iz, iy, ix), val in entries:
+                    Vh[iz, iy, ix] += val
+                out = torch.fft.irfftn(Vh, s=(N, N, N), dim=(0, 1, 2))
+                del Vh
+                res = out.cpu().numpy()
+                del out
+                torch.cuda.empty_cache()
+                return res
+        except ImportError:
+            pass
+    Vh = np.zeros((N, N, nh), dtype=np.complex128)
+    for (iz, iy, ix), val in entries:
+        Vh[iz, iy, ix] += val
+    return np.ascontiguousarray(np.fft.irfftn(Vh, s=(N, N, N), axes=(0, 1, 2)))
 
 
 # ----------------------------------------------------------------------------------------------------
