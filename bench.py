@@ -227,6 +227,32 @@ def fft_metric(g, torch, N, nf=8, reps=5):
     return out
 
 
+def pcie_peaks(torch, device, nbytes=1 << 30, reps=4):
+    """Measured pinned-memory copy bandwidth of this box (GB/s): host->device alone, device->host alone, and both
+    directions at once on two streams — the ceiling of the chunked pipeline when arrays live on the host."""
+    h_in = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
+    h_out = torch.empty(nbytes, dtype=torch.uint8, pin_memory=True)
+    d_in = torch.empty(nbytes, dtype=torch.uint8, device=device)
+    d_out = torch.empty(nbytes, dtype=torch.uint8, device=device)
+    s1, s2 = torch.cuda.Stream(device), torch.cuda.Stream(device)
+
+    def run(do_in, do_out):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(reps):
+            if do_in:
+                with torch.cuda.stream(s1):
+                    d_in.copy_(h_in, non_blocking=True)
+            if do_out:
+                with torch.cuda.stream(s2):
+                    h_out.copy_(d_out, non_blocking=True)
+        torch.cuda.synchronize()
+        return nbytes * reps / (time.perf_counter() - t0) / 1e9
+
+    run(True, True)
+    return {"h2d_alone_gbs": run(True, False), "d2h_alone_gbs": run(False, True), "each_direction_when_both_gbs": run(True, True)}
+
+
 def run_ours(args):
     rank, local_rank, world = dist_env()
     import torch
@@ -290,6 +316,10 @@ def run_ours(args):
                "h2d_bytes_per_step": (x1[0] - x0[0]) / K, "d2h_bytes_per_step": (x1[1] - x0[1]) / K,
                "h2d_gbs": (x1[0] - x0[0]) / ms_np / 1e6, "d2h_gbs": (x1[1] - x0[1]) / ms_np / 1e6,
                "s_per_step": ms_np / K / 1e3}
+        if g.pinned_bytes:
+            ooc["pcie_measured"] = pcie_peaks(torch, g.device)
+            ooc["bound"] = "pcie"
+            ooc["frac_of_duplex_pcie"] = max(ooc["h2d_gbs"], ooc["d2h_gbs"]) / ooc["pcie_measured"]["each_direction_when_both_gbs"]
     g.profile_enable(False)
     clocks = sampler.stop()
     ms_max, units = aggregate(ms, float(N) ** 3 * K, dist)
