@@ -44,6 +44,10 @@ def lib():
         L.orc_apply.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         L.orc_fft3.argtypes = [C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
         L.orc_dft3_direct.argtypes = [C.c_int, C.c_int, C.c_int, C.c_void_p, C.c_void_p]
+        L.orc_cic.argtypes = [C.c_int, C.c_double, C.c_int, PP, C.c_longlong, PP, PP]
+        L.orc_tracers_push.argtypes = [C.c_int, C.c_double, C.c_double, PP, C.c_longlong, PP, PP, C.c_int]
+        L.orc_tracers_set.argtypes = [C.c_void_p, C.c_longlong, PP, PP]
+        L.orc_tracers_get.argtypes = [C.c_void_p, PP, PP]
         _lib = L
     return _lib
 
@@ -81,6 +85,34 @@ def fft3(a: np.ndarray, sign: int = -1, long_double: bool = False, direct: bool 
     fn = lib().orc_dft3_direct if direct else lib().orc_fft3
     _check(fn(N, int(sign), int(long_double), a.ctypes.data, out.ctypes.data))
     return out
+
+
+def _ptrn(arrs):
+    a = (C.c_void_p * len(arrs))()
+    for i, x in enumerate(arrs):
+        a[i] = x.ctypes.data
+    return a
+
+
+def cic(fields, pos, L=2 * math.pi):
+    """Eq. 20: cloud-in-cell interpolation of the [N][N][N] grid fields to the positions pos (3 arrays of np)."""
+    g = [_c_in(x) for x in fields]
+    N = g[0].shape[0]
+    p = [_c_in(x) for x in pos]
+    n = p[0].size
+    out = [np.empty(n) for _ in g]
+    _check(lib().orc_cic(N, L, len(g), _ptrn(g), n, _ptrn(p), _ptrn(out)))
+    return out
+
+
+def tracers_push(B, pos, vel, dt, nsteps=1, L=2 * math.pi):
+    """nsteps Boris pushes (Eq. 21-22) in the frozen grid field B; returns new (pos, vel)."""
+    g = [_c_in(x) for x in B]
+    N = g[0].shape[0]
+    p = [np.array(x, dtype=np.float64) for x in pos]
+    v = [np.array(x, dtype=np.float64) for x in vel]
+    _check(lib().orc_tracers_push(N, L, dt, _ptrn(g), p[0].size, _ptrn(p), _ptrn(v), int(nsteps)))
+    return p, v
 
 
 class Oracle:
@@ -153,6 +185,18 @@ class Oracle:
         if spectra:
             out["spec_kin"], out["spec_mag"] = sk, sm
         return out
+
+    def tracers_set(self, pos, vel=None):
+        p = [_c_in(x) for x in pos]
+        self._np = p[0].size
+        v = [_c_in(x) for x in vel] if vel is not None else None
+        _check(lib().orc_tracers_set(self._h, self._np, _ptrn(p), _ptrn(v) if v is not None else None))
+
+    def tracers_get(self):
+        p = [np.empty(self._np) for _ in range(3)]
+        v = [np.empty(self._np) for _ in range(3)]
+        _check(lib().orc_tracers_get(self._h, _ptrn(p), _ptrn(v)))
+        return p, v
 
     def apply(self, op, f):
         names = {"dx": 0, "dy": 1, "dz": 2, "lap": 3, "project": 4}

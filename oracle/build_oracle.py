@@ -11,7 +11,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = [os.path.join(HERE, "oracle_capi.cpp")]
-DEPS = SRC + [os.path.join(HERE, "mhd_oracle.hpp"), os.path.join(HERE, "oracle.h")]
+DEPS = SRC + [os.path.join(HERE, f) for f in ("mhd_oracle.hpp", "tracers_oracle.hpp", "oracle.h")]
 OUT = os.path.join(HERE, "liboracle.so")
 
 

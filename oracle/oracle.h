@@ -42,6 +42,18 @@ int orc_apply(orc_ctx *c, int op, const double *in, double *out);
 int orc_fft3(int N, int sign, int precision, const double *in, double *out);
 int orc_dft3_direct(int N, int sign, int precision, const double *in, double *out);
 
+/* ---- tracer particles, Sec. VI (L229-275), oracle/tracers_oracle.hpp ---------------------------------
+ * Stand-alone pieces (fp64): CIC interpolation (Eq. 20) of nf grid fields to np positions; nsteps Boris pushes
+ * (Eq. 21-22) in a FROZEN grid field B[3].  pos / vel are 3 arrays of np doubles (x, y, z components). */
+int orc_cic(int N, double L, int nf, const double *const g[], long long np, const double *const pos[3],
+            double *const out[]);
+int orc_tracers_push(int N, double L, double dt, const double *const B[3], long long np, double *const pos[3],
+                     double *const vel[3], int nsteps);
+/* Tracers attached to a solver: orc_step() then pushes them once per step with the B of the state at the START of
+ * the step (t_n), before the fields advance.  vel == NULL: initial velocity = CIC interpolation of u = m/rho. */
+int orc_tracers_set(orc_ctx *c, long long np, const double *const pos[3], const double *const vel[3]);
+int orc_tracers_get(orc_ctx *c, double *const pos[3], double *const vel[3]);
+
 #ifdef __cplusplus
 }
 #endif
