@@ -73,6 +73,8 @@ extern "C" {
 #define MHD_OPT_OOC_BRICK 5 /* chunked pipeline: largest number of ky columns per brick (0 = what the staging allows) */
 #define MHD_OPT_OOC_SLAB 6  /* chunked pipeline: largest number of z planes per slab  (0 = what the staging allows) */
 
+#define MHD_OPT_STRIDED_COLS 7 /* tuning: kx columns per CTA of the strided (y, z) passes, 0 = default, 4 / 8 / 16 */
+
 typedef struct mhd_ctx mhd_ctx; /* opaque, owned by the library */
 
 /* Diagnostics record ("per grid" = volume means; L71 Eq. 9; R8). */
@@ -141,6 +143,26 @@ int mhd_nspec(int N);
 int mhd_fft3d_r2c(mhd_ctx *ctx, int nfields, const double *const real[], double *const spec[],
                   double *const nyq[], int prune);
 int mhd_fft3d_c2r(mhd_ctx *ctx, int nfields, double *const spec[], double *const real[], int prune);
+
+/* ---- Tracer particles (Sec. VI, readings T1-T4) ----------------
+ * Passive particles with q = M = 1 that feel only the magnetic field of the grid (L241).  One push (L268-272) =
+ *   1) corner index (i,j,k) = floor(x N/L) of the particle's unit cell;
+ *   2) Eq. 20 (L251): cloud-in-cell interpolation of B from the 8 corner grids (weights = opposite sub-cell volumes /
+ *      cell volume, corner indices wrapped periodically, L255);
+ *   3) Eq. 21 (L259-265): t = B_p dt/2, s = 2t/(1+|t|^2), v_d = v + v x t, v(t+dt) = v + v_d x s;
+ *   4) Eq. 22 (L266): x(t+dt) = x + v(t+dt) dt, wrapped into [0, L).
+ * Storage: the caller provides mhd_tracers_bytes(np) device bytes (256-byte aligned) and keeps them alive; pos / vel
+ * arguments are 3 arrays (x, y, z components) of np doubles, host or device as `where` says.
+ * mhd_tracers_set: positions are wrapped into [0, L); vel == NULL sets the initial velocity to the CIC interpolation
+ *   of u = m/rho of the current state (L241; needs mhd_set_fields first).
+ * While tracers are set, every step of mhd_step() first pushes them once with dt and the B of the state at the START
+ * of that step (t_n), then advances the fields.  mhd_tracers_push() pushes nsteps times in the B of the current state
+ * without advancing the fields (one kernel; the gather benchmark).  Not available on an out-of-core context. */
+size_t mhd_tracers_bytes(long long np);
+int mhd_tracers_bind(mhd_ctx *ctx, long long np, void *dev_buffer, size_t bytes);   /* np = 0 detaches */
+int mhd_tracers_set(mhd_ctx *ctx, int where, const double *const pos[3], const double *const vel[3]);
+int mhd_tracers_get(mhd_ctx *ctx, int where, double *const pos[3], double *const vel[3]);
+int mhd_tracers_push(mhd_ctx *ctx, int nsteps);
 
 /* Bytes the chunked pipeline has copied host->device / device->host so far (0 for an in-core context). */
 int mhd_transfer_bytes(const mhd_ctx *ctx, long long *h2d, long long *d2h);

@@ -34,7 +34,8 @@ ERRORS = {-1: "MHD_ERR_INVALID_ARG", -2: "MHD_ERR_NOT_BOUND", -3: "MHD_ERR_NO_FI
 SYMBOLS = ["mhd_init", "mhd_workspace_bytes", "mhd_pinned_bytes", "mhd_bind", "mhd_set_option", "mhd_set_fields",
            "mhd_rhs", "mhd_step", "mhd_get_fields", "mhd_diagnostics", "mhd_nspec", "mhd_fft3d_r2c",
            "mhd_fft3d_c2r", "mhd_launch_count", "mhd_transfer_bytes", "mhd_profile_enable", "mhd_profile_get", "mhd_last_error",
-           "mhd_destroy"]
+           "mhd_destroy", "mhd_tracers_bytes", "mhd_tracers_bind", "mhd_tracers_set", "mhd_tracers_get",
+           "mhd_tracers_push"]
 
 
 class MhdDiag(C.Structure):
@@ -71,6 +72,12 @@ def lib():
     L.mhd_nspec.argtypes = [C.c_int]
     L.mhd_fft3d_r2c.argtypes = [C.c_void_p, C.c_int, P8, P8, P8, C.c_int]
     L.mhd_fft3d_c2r.argtypes = [C.c_void_p, C.c_int, P8, P8, C.c_int]
+    L.mhd_tracers_bytes.argtypes = [C.c_longlong]
+    L.mhd_tracers_bytes.restype = C.c_size_t
+    L.mhd_tracers_bind.argtypes = [C.c_void_p, C.c_longlong, C.c_void_p, C.c_size_t]
+    L.mhd_tracers_set.argtypes = [C.c_void_p, C.c_int, P8, P8]
+    L.mhd_tracers_get.argtypes = [C.c_void_p, C.c_int, P8, P8]
+    L.mhd_tracers_push.argtypes = [C.c_void_p, C.c_int]
     L.mhd_launch_count.argtypes = [C.c_void_p]
     L.mhd_launch_count.restype = C.c_longlong
     L.mhd_transfer_bytes.argtypes = [C.c_void_p, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
@@ -225,6 +232,56 @@ class MHD:
         r = _ptr_array([t.data_ptr() for t in real])
         s = _ptr_array([t.data_ptr() for t in spec])
         self._check(self._L.mhd_fft3d_c2r(self._h, n, s, r, int(prune)))
+
+    # -- tracer particles (Sec. VI) ------------------------------------------------------------
+    def _marshal3(self, arrs, n):
+        torch = self.torch
+        if all(isinstance(a, np.ndarray) for a in arrs):
+            keep = [np.ascontiguousarray(a, dtype=np.float64) for a in arrs]
+            assert all(k.size == n for k in keep)
+            return MHD_HOST, _ptr_array([k.ctypes.data for k in keep]), keep
+        keep = [a.contiguous() for a in arrs]
+        assert all(k.dtype == torch.float64 and k.numel() == n for k in keep)
+        where = MHD_DEVICE if keep[0].is_cuda else MHD_HOST
+        assert all(k.is_cuda == keep[0].is_cuda for k in keep)
+        return where, _ptr_array([k.data_ptr() for k in keep]), keep
+
+    def tracers_set(self, pos, vel=None):
+        """Attach len(pos[0]) tracers (torch owns their device storage); vel=None: v0 = CIC of u = m/rho."""
+        torch = self.torch
+        n = int(pos[0].numel() if isinstance(pos[0], torch.Tensor) else np.asarray(pos[0]).size)
+        if getattr(self, "_ntr", 0) != n:
+            nbytes = int(self._L.mhd_tracers_bytes(n))
+            with torch.cuda.device(self.device):
+                self._trbuf = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = (self._trbuf.data_ptr() + 255) // 256 * 256
+            self._check(self._L.mhd_tracers_bind(self._h, n, base, nbytes))
+            self._ntr = n
+        where, pp, keep_p = self._marshal3(pos, n)
+        if vel is None:
+            self._check(self._L.mhd_tracers_set(self._h, where, pp, None))
+        else:
+            wv, vp, keep_v = self._marshal3(vel, n)
+            assert wv == where
+            self._check(self._L.mhd_tracers_set(self._h, where, pp, vp))
+
+    def tracers_get(self, where="host"):
+        n = self._ntr
+        if where == "host":
+            pos = [np.empty(n) for _ in range(3)]
+            vel = [np.empty(n) for _ in range(3)]
+            pp, vp = _ptr_array([a.ctypes.data for a in pos]), _ptr_array([a.ctypes.data for a in vel])
+            self._check(self._L.mhd_tracers_get(self._h, MHD_HOST, pp, vp))
+        else:
+            pos = [self.torch.empty(n, dtype=self.torch.float64, device=self.device) for _ in range(3)]
+            vel = [self.torch.empty(n, dtype=self.torch.float64, device=self.device) for _ in range(3)]
+            pp, vp = _ptr_array([a.data_ptr() for a in pos]), _ptr_array([a.data_ptr() for a in vel])
+            self._check(self._L.mhd_tracers_get(self._h, MHD_DEVICE, pp, vp))
+        return pos, vel
+
+    def tracers_push(self, nsteps=1):
+        """nsteps Boris pushes in the B of the current state (fields do not advance)."""
+        self._check(self._L.mhd_tracers_push(self._h, int(nsteps)))
 
     def transfer_bytes(self):
         """(host->device, device->host) bytes the chunked pipeline has copied so far."""

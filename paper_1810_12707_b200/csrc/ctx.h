@@ -14,10 +14,10 @@
 using namespace mhd;
 
 enum Family { F_STRIDED_INV = 0, F_STRIDED_FWD, F_X_FUSED, F_X_C2R, F_X_R2C, F_FLUX, F_CURRENT, F_ASSEMBLE, F_AXPBY,
-              F_POINT, F_DIAG, F_COUNT };
+              F_POINT, F_DIAG, F_TRACERS, F_COUNT };
 inline const char* family_name(int f) {
     static const char* names[F_COUNT] = {"strided_inverse", "strided_forward", "x_fused", "x_c2r", "x_r2c", "flux_real",
-                                         "build_current", "assemble", "axpby", "pointwise_misc", "diagnostics"};
+                                         "build_current", "assemble", "axpby", "pointwise_misc", "diagnostics", "tracers"};
     return names[f];
 }
 
@@ -52,7 +52,7 @@ struct mhd_ctx {
     bool bound = false, have_fields = false, have_old = false;
     cudaStream_t st = nullptr;
     unsigned flags = 0;
-    int opt_fused = 1, opt_prune = 1, opt_fuse_current = 1, integrator = 0;
+    int opt_fused = 1, opt_prune = 1, opt_fuse_current = 1, integrator = 0, opt_strided_cols = 0;
     long long step = 0;
     long long launches = 0;
     std::string err;
@@ -76,6 +76,12 @@ struct mhd_ctx {
         double *part_diag = nullptr, *part_max = nullptr, *part_spec = nullptr;
         long long h2d_bytes = 0, d2h_bytes = 0;
     } ooc;
+    // tracer particles (tracers.cu): caller-provided device storage, 6 arrays of np doubles
+    struct Tracers {
+        long long np = 0;
+        bool set = false;
+        double *pos[3] = {nullptr, nullptr, nullptr}, *vel[3] = {nullptr, nullptr, nullptr};
+    } tr;
     // profiling
     bool prof = false;
     struct Rec { int fam; cudaEvent_t a, b; };
@@ -125,7 +131,7 @@ inline int check_cuda(mhd_ctx* c, const char* what) {
 
 // ---- shared between mhd_api.cu and ooc.cu -----------------------------------------------------------------------
 // sweep S3 on `nlines` consecutive lines (in place allowed): C2R of 11 fields, flux products, R2C of 16 products
-void run_x_fused(mhd_ctx* c, cd* const in[11], cd* const out[16], long long nlines);
+void run_x_fused(mhd_ctx* c, cd* const in[11], cd* const out[16], long long nlines, double* const breal[3] = nullptr);
 
 size_t ooc_workspace_bytes(int N, unsigned flags);
 size_t ooc_pinned_bytes(int N, unsigned flags);

@@ -27,7 +27,8 @@ struct StridedArgs {
     const cd* tw;          // exp(-2 pi i m / N), m < N
     long long in_row_stride, out_row_stride;      // complex elements between consecutive stored rows
     long long in_outer_stride, out_outer_stride;  // complex elements between consecutive outer indices
-    int nchunks;           // column chunks (of C columns) to process
+    int nchunks;           // (computed by the launcher from ncols and the columns per CTA)
+    int cols;              // columns per CTA: 0 = default for N (8; 4 at N = 1024); 4 / 16 = tuning variants (in-core path)
     int ncols;             // valid columns (guards the last chunk)
     int n_outer;           // number of outer indices processed
     int outer_split;       // in-core: outer index o maps to o (o < split) or o + outer_skip
@@ -72,6 +73,7 @@ struct FusedXArgs {
     int kmax_in, kmax_out;
     double scale;
     Phys ph;
+    double* breal[3];     // optional (fused2 only): real-space Bx, By, Bz lines are also written here (tracers); or null
 };
 void launch_x_fused(int N, const FusedXArgs& a, cudaStream_t st);
 // second-generation fused sweep (kernels_xfused2.cu): N = 128, 256, 512
@@ -132,6 +134,21 @@ void launch_shell_spectrum_final(const double* part, double* out, int nspec, cud
 int diag_partial_doubles();
 int absmax_partial_doubles();
 int spectrum_partial_doubles(int nspec);
+
+// ---- tracer particles (tracers.cu) ------------------------------------------------------------------------
+struct TracerArgs {
+    const double* B[3];    // real-space grid fields [z][y][x] gathered by the push
+    double* pos[3];
+    double* vel[3];
+    long long np;
+    int N;
+    double L, dt;
+    int nsteps;            // pushes in the frozen field
+};
+void launch_tracer_push(const TracerArgs& a, cudaStream_t st);
+// vel <- CIC interpolation of m/rho (real-space rho, mx, my, mz)
+void launch_tracer_init_velocity(const TracerArgs& a, const double* rho, const double* const m[3], cudaStream_t st);
+void launch_tracer_wrap(const TracerArgs& a, cudaStream_t st);
 
 void launch_twiddle_table(int N, cd* tw, cudaStream_t st);
 

@@ -112,7 +112,7 @@ template <int N, int DIR, int C, bool GEN, bool FJ> static void launch_one(const
         cudaFuncSetAttribute(strided_kernel<N, DIR, C, GEN, FJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         configured = true;
     }
-    dim3 grid(a.nchunks, a.n_outer, a.nfields);
+    dim3 grid((a.ncols + C - 1) / C, a.n_outer, a.nfields);
     strided_kernel<N, DIR, C, GEN, FJ><<<grid, threads, smem, st>>>(a);
 }
 
@@ -131,8 +131,15 @@ void launch_strided(int N, int dir, const StridedArgs& a, cudaStream_t st) {
         case 32: launch_dir<32, 8>(dir, a, st); break;
         case 64: launch_dir<64, 8>(dir, a, st); break;
         case 128: launch_dir<128, 8>(dir, a, st); break;
-        case 256: launch_dir<256, 8>(dir, a, st); break;
-        case 512: launch_dir<512, 8>(dir, a, st); break;
+        case 256:
+            if (a.cols == 4 && !a.general) launch_dir<256, 4>(dir, a, st);
+            else if (a.cols == 16 && !a.general) launch_dir<256, 16>(dir, a, st);
+            else launch_dir<256, 8>(dir, a, st);
+            break;
+        case 512:
+            if (a.cols == 4 && !a.general) launch_dir<512, 4>(dir, a, st);
+            else launch_dir<512, 8>(dir, a, st);
+            break;
         case 1024: launch_dir<1024, 4>(dir, a, st); break;
         default: break;
     }

@@ -191,6 +191,11 @@ x_fused2_kernel(const __grid_constant__ FusedXArgs a) {
             const cd z = sm[tidx<H>(n, f)];
             s0[f] = z.x; s1[f] = z.y;
         }
+        if (a.breal[0]) {           // tracers: the real-space B of this line also goes to HBM (block-uniform branch)
+#pragma unroll
+            for (int d = 0; d < 3; ++d)
+                reinterpret_cast<cd*>(a.breal[d])[off + n] = mk(s0[S_BX + d], s1[S_BX + d]);
+        }
         flux_point(s0, o0, a.ph);
         flux_point(s1, o1, a.ph);
 #pragma unroll

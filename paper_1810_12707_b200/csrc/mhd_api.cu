@@ -29,9 +29,8 @@ void strided_pass(mhd_ctx* c, int dir, int axis, int nf, const cd* const in[], c
         a.kc = kc;
         a.nfields = nb;
         a.jfirst = jfirst; a.bfirst = bfirst; a.k0 = 2.0 * M_PI / c->L;   // fused current: only with nf <= MAXF
-        const int C = N >= 1024 ? 4 : 8;
         a.ncols = prune ? std::min(kc + 1, ncols_full) : ncols_full;
-        a.nchunks = (a.ncols + C - 1) / C;
+        a.cols = c->opt_strided_cols;
         if (axis == 1) {            // y pass: rows along y, outer = z (all planes)
             a.in_row_stride = a.out_row_stride = hx; a.in_outer_stride = a.out_outer_stride = (long long)N * hx;
             a.n_outer = N; a.outer_split = N; a.outer_skip = 0;
@@ -95,7 +94,7 @@ void forward3d(mhd_ctx* c, int nf, const double* const real_in[], cd* const spec
 
 }  // namespace
 
-void run_x_fused(mhd_ctx* c, cd* const in[11], cd* const out[16], long long nlines) {
+void run_x_fused(mhd_ctx* c, cd* const in[11], cd* const out[16], long long nlines, double* const breal[3]) {
     const int N = c->N;
     const bool prune = c->opt_prune != 0 || c->ooc.on;
     const int kmax = prune ? c->kc() : c->hx() - 1;
@@ -104,15 +103,18 @@ void run_x_fused(mhd_ctx* c, cd* const in[11], cd* const out[16], long long nlin
     for (int f = 0; f < 16; ++f) a.out[f] = out[f];
     a.tw = c->tw; a.nlines = nlines; a.kmax_in = kmax; a.kmax_out = kmax;
     a.scale = 1.0 / ((double)N * N * N); a.ph = c->phys();
+    const bool gen2 = c->opt_fused != 2 && x_fused2_supported(N);
+    if (breal && gen2) for (int d = 0; d < 3; ++d) a.breal[d] = breal[d];   // only the second-generation kernel emits B
     mhd_ctx::Scope s(c, F_X_FUSED);
-    if (c->opt_fused != 2 && x_fused2_supported(N)) { a.tw = c->ftw; launch_x_fused2(N, a, c->st); }
+    if (gen2) { a.tw = c->ftw; launch_x_fused2(N, a, c->st); }
     else launch_x_fused(N, a, c->st);
 }
 
 namespace {
 
 // products W[0..15] <- state Uin (k-space); sweeps S1-S4 and the forward z pass of S5
-void products(mhd_ctx* c, cd* const Uin[8]) {
+// breal != null (tracers, fused sweep only): the real-space B of Uin is also written there by sweep S3
+void products(mhd_ctx* c, cd* const Uin[8], double* const breal[3] = nullptr) {
     const int N = c->N;
     const bool prune = c->opt_prune != 0;
     const SpecGeom g = c->geom();
@@ -134,7 +136,7 @@ void products(mhd_ctx* c, cd* const Uin[8]) {
     const int kmax = prune ? c->kc() : c->hx() - 1;
     const double scale = 1.0 / ((double)N * N * N);
     if (c->opt_fused) {                                                   // S3
-        run_x_fused(c, c->W, c->W, (long long)N * N);
+        run_x_fused(c, c->W, c->W, (long long)N * N, breal);
     } else {
         XArgs a; std::memset(&a, 0, sizeof(a));
         for (int f = 0; f < 11; ++f) { a.spec_in[f] = c->W[f]; a.real_out[f] = reinterpret_cast<double*>(c->W[f]); }
@@ -154,10 +156,33 @@ void products(mhd_ctx* c, cd* const Uin[8]) {
 }
 
 // R^(Uin) -> rout (mode 0) or explicit update of Uin / Rold (mode 1 Euler, 2 AB2)
-void rhs_spectral(mhd_ctx* c, cd* const Uin[8], cd* const rout[8], int mode) {
-    products(c, Uin);
+void rhs_spectral(mhd_ctx* c, cd* const Uin[8], cd* const rout[8], int mode, double* const breal[3] = nullptr) {
+    products(c, Uin, breal);
     mhd_ctx::Scope s(c, F_ASSEMBLE);
     launch_assemble(c->geom(), c->W, Uin, c->Rold, rout, mode, c->dt, c->phys(), c->st);
+}
+
+// ---- tracer particles (Sec. VI) ----------------------------------------------------------------------
+TracerArgs tracer_args(mhd_ctx* c, const double* const B[3], int nsteps) {
+    TracerArgs a; std::memset(&a, 0, sizeof(a));
+    for (int d = 0; d < 3; ++d) { a.B[d] = B ? B[d] : nullptr; a.pos[d] = c->tr.pos[d]; a.vel[d] = c->tr.vel[d]; }
+    a.np = c->tr.np; a.N = c->N; a.L = c->L; a.dt = c->dt; a.nsteps = nsteps;
+    return a;
+}
+bool tracers_active(const mhd_ctx* c) { return c->tr.np > 0 && c->tr.set; }
+// sweep S3 of the second-generation fused kernel can write the real-space B as a by-product
+bool tracers_fused_emit(const mhd_ctx* c) { return c->opt_fused == 1 && x_fused2_supported(c->N) && c->integrator == 0; }
+// real-space B of the current state -> X[0..2] by a separate pruned inverse transform (U^ is left intact)
+void tracers_real_B(mhd_ctx* c, double* Breal[3]) {
+    const cd* spec[3] = {c->U[5], c->U[6], c->U[7]};
+    cd* work[3] = {c->X[0], c->X[1], c->X[2]};
+    for (int d = 0; d < 3; ++d) Breal[d] = reinterpret_cast<double*>(c->X[d]);
+    inverse3d(c, 3, spec, work, Breal, true);
+}
+void tracers_push_with(mhd_ctx* c, double* const Breal[3], int nsteps) {
+    const double* B[3] = {Breal[0], Breal[1], Breal[2]};
+    mhd_ctx::Scope s(c, F_TRACERS);
+    launch_tracer_push(tracer_args(c, B, nsteps), c->st);
 }
 
 int copy_in(mhd_ctx* c, int where, const double* const src[8], double* const dst[8]) {
@@ -266,6 +291,9 @@ int mhd_set_option(mhd_ctx* c, int option, int value) {
         case MHD_OPT_INTEGRATOR:
             if (value < 0 || value > 2) return c->fail(MHD_ERR_INVALID_ARG, "integrator must be 0, 1 or 2");
             c->integrator = value; c->have_old = false; return MHD_OK;
+        case MHD_OPT_STRIDED_COLS:
+            if (value != 0 && value != 4 && value != 8 && value != 16) return c->fail(MHD_ERR_INVALID_ARG, "strided columns must be 0, 4, 8 or 16");
+            c->opt_strided_cols = value; return MHD_OK;
         case MHD_OPT_OOC_BRICK:
             if (value < 0) return c->fail(MHD_ERR_INVALID_ARG, "brick size must be >= 0");
             c->ooc.brick_max = value; return MHD_OK;
@@ -332,9 +360,15 @@ int mhd_step(mhd_ctx* c, int nsteps) {
     if (c->ooc.on) return ooc_step(c, nsteps);
     const SpecGeom g = c->geom();
     SpecGeom gp = g; gp.pruned = 1;
+    const bool tracers = tracers_active(c), emit = tracers && tracers_fused_emit(c);
+    double* Breal[3] = {reinterpret_cast<double*>(c->X[0]), reinterpret_cast<double*>(c->X[1]), reinterpret_cast<double*>(c->X[2])};
     for (int s = 0; s < nsteps; ++s) {
+        // tracers feel the B of the state at the start of the step (t_n): either a separate inverse transform now, or
+        // (AB2 + fused sweep) the real-space B that sweep S3 of this step's right-hand side produces anyway
+        if (tracers && !emit) { tracers_real_B(c, Breal); tracers_push_with(c, Breal, 1); }
         if (c->integrator == 0) {                       // Adams-Bashforth 2, Euler start (R6)
-            rhs_spectral(c, c->U, nullptr, c->have_old ? 2 : 1);
+            rhs_spectral(c, c->U, nullptr, c->have_old ? 2 : 1, emit ? Breal : nullptr);
+            if (emit) tracers_push_with(c, Breal, 1);
             c->have_old = true;
         } else if (c->integrator == 1) {                // classical RK4
             // U0 = Rold, acc = Y, k = X, stage state in U
@@ -456,6 +490,83 @@ int mhd_fft3d_c2r(mhd_ctx* c, int nfields, double* const spec[], double* const r
     for (int f = 0; f < nfields; ++f) { sp[f] = reinterpret_cast<cd*>(spec[f]); spc[f] = sp[f]; }
     inverse3d(c, nfields, spc.data(), sp.data(), real, prune != 0);
     return check_cuda(c, "fft3d_c2r");
+}
+
+size_t mhd_tracers_bytes(long long np) { return np <= 0 ? 0 : 6 * align_up((size_t)np * sizeof(double)); }
+
+int mhd_tracers_bind(mhd_ctx* c, long long np, void* dev_buffer, size_t bytes) {
+    if (!c || np < 0) return MHD_ERR_INVALID_ARG;
+    if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
+    if (c->ooc.on) return c->fail(MHD_ERR_INVALID_ARG, "tracers need an in-core context");
+    c->tr = mhd_ctx::Tracers();
+    if (np == 0) return MHD_OK;
+    if (!dev_buffer || ((uintptr_t)dev_buffer & 255) != 0) return c->fail(MHD_ERR_INVALID_ARG, "tracer buffer must be 256-byte aligned");
+    if (bytes < mhd_tracers_bytes(np)) return c->fail(MHD_ERR_NOMEM, "tracer buffer too small");
+    const size_t stride = align_up((size_t)np * sizeof(double));
+    char* b = static_cast<char*>(dev_buffer);
+    for (int d = 0; d < 3; ++d) {
+        c->tr.pos[d] = reinterpret_cast<double*>(b + (size_t)d * stride);
+        c->tr.vel[d] = reinterpret_cast<double*>(b + (size_t)(3 + d) * stride);
+    }
+    c->tr.np = np;
+    return MHD_OK;
+}
+
+int mhd_tracers_set(mhd_ctx* c, int where, const double* const pos[3], const double* const vel[3]) {
+    if (!c || !pos) return MHD_ERR_INVALID_ARG;
+    if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
+    if (c->tr.np <= 0) return c->fail(MHD_ERR_NOT_BOUND, "mhd_tracers_bind has not been called");
+    if (where != 0 && where != 1) return c->fail(MHD_ERR_INVALID_ARG, "where");
+    if (!vel && !c->have_fields) return c->fail(MHD_ERR_NO_FIELDS, "initial tracer velocity needs mhd_set_fields first");
+    const size_t bytes = (size_t)c->tr.np * sizeof(double);
+    const cudaMemcpyKind kind = where == MHD_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+    for (int d = 0; d < 3; ++d) {
+        if (!pos[d] || (vel && !vel[d])) return c->fail(MHD_ERR_INVALID_ARG, "null tracer array");
+        cudaMemcpyAsync(c->tr.pos[d], pos[d], bytes, kind, c->st);
+        if (vel) cudaMemcpyAsync(c->tr.vel[d], vel[d], bytes, kind, c->st);
+    }
+    { mhd_ctx::Scope s(c, F_TRACERS); launch_tracer_wrap(tracer_args(c, nullptr, 0), c->st); }
+    if (!vel) {      // v0 = CIC of u = m/rho (L241): real-space rho, m of the current state -> X[0..3]
+        const cd* spec[4] = {c->U[0], c->U[1], c->U[2], c->U[3]};
+        cd* work[4] = {c->X[0], c->X[1], c->X[2], c->X[3]};
+        double* real[4];
+        for (int f = 0; f < 4; ++f) real[f] = reinterpret_cast<double*>(c->X[f]);
+        inverse3d(c, 4, spec, work, real, true);
+        const double* m[3] = {real[1], real[2], real[3]};
+        mhd_ctx::Scope s(c, F_TRACERS);
+        launch_tracer_init_velocity(tracer_args(c, nullptr, 0), real[0], m, c->st);
+    }
+    if (where == MHD_HOST) cudaStreamSynchronize(c->st);
+    int rc = check_cuda(c, "tracers_set");
+    if (rc) return rc;
+    c->tr.set = true;
+    return MHD_OK;
+}
+
+int mhd_tracers_get(mhd_ctx* c, int where, double* const pos[3], double* const vel[3]) {
+    if (!c) return MHD_ERR_INVALID_ARG;
+    if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
+    if (!tracers_active(c)) return c->fail(MHD_ERR_NO_FIELDS, "mhd_tracers_set has not been called");
+    if (where != 0 && where != 1) return c->fail(MHD_ERR_INVALID_ARG, "where");
+    const size_t bytes = (size_t)c->tr.np * sizeof(double);
+    const cudaMemcpyKind kind = where == MHD_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
+    for (int d = 0; d < 3; ++d) {
+        if (pos && pos[d]) cudaMemcpyAsync(pos[d], c->tr.pos[d], bytes, kind, c->st);
+        if (vel && vel[d]) cudaMemcpyAsync(vel[d], c->tr.vel[d], bytes, kind, c->st);
+    }
+    if (where == MHD_HOST) cudaStreamSynchronize(c->st);
+    return check_cuda(c, "tracers_get");
+}
+
+int mhd_tracers_push(mhd_ctx* c, int nsteps) {
+    if (!c || nsteps < 0) return MHD_ERR_INVALID_ARG;
+    if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
+    if (!c->have_fields) return c->fail(MHD_ERR_NO_FIELDS, "mhd_set_fields has not been called");
+    if (!tracers_active(c)) return c->fail(MHD_ERR_NO_FIELDS, "mhd_tracers_set has not been called");
+    double* Breal[3];
+    tracers_real_B(c, Breal);
+    tracers_push_with(c, Breal, nsteps);
+    return check_cuda(c, "tracers_push");
 }
 
 long long mhd_launch_count(const mhd_ctx* c) { return c ? c->launches : 0; }

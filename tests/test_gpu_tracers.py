@@ -1,0 +1,165 @@
+"""GPU parity of the tracer particles (Sec. VI, Eq. 20-22) against the CPU oracle, through the C ABI.
+
+Tolerances: the cell index floor(x N/L) is an integer decided in fp64 on both sides from the same expression; the
+push itself is ~150 fp64 operations, so positions and velocities agree to a few ulp per step: after n steps the
+bound used is 1e-13 * (1 + n) relative to L resp. |v| (round-off grows linearly at worst; a flipped cell decision at
+an exact cell boundary changes nothing because CIC is continuous across cells)."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1810_12707_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+L = 2 * math.pi
+
+
+@pytest.fixture(scope="module")
+def MHD():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1810_12707_b200 import build, binding
+    build.build()
+    return binding.MHD
+
+
+def particles(n, seed, vscale=1.0):
+    rng = np.random.default_rng(seed)
+    pos = [rng.uniform(0, L, n) for _ in range(3)]
+    vel = [rng.standard_normal(n) * vscale for _ in range(3)]
+    return pos, vel
+
+
+def close(a, b, tol):
+    return all(np.max(np.abs(x - y)) <= tol for x, y in zip(a, b))
+
+
+def wrapped_diff(a, b):
+    d = np.abs(a - b)
+    return np.minimum(d, L - d)
+
+
+@pytest.mark.parametrize("N", [16, 32, 64, 128])
+def test_frozen_field_push_matches_oracle(orc, MHD, N):
+    """mhd_tracers_push (one launch, nsteps pushes in the frozen B of the state) vs the oracle's loop; 5003 particles
+    (ragged tail of the 128-thread blocks), velocities large enough to cross the periodic boundary many times."""
+    cfg = inputs.config3(N, kmax=4) if N >= 32 else inputs.config1(N)
+    g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, 0.05)
+    g.set_fields(cfg.prim, "primitive")
+    pos, vel = particles(5003, N, vscale=3.0)
+    g.tracers_set(pos, vel)
+    nsteps = 40
+    g.tracers_push(nsteps)
+    pg, vg = g.tracers_get()
+    B = g.get_fields("conservative")[5:8]            # the projected state the GPU holds (identical input for both)
+    po, vo = orc.tracers_push(B, pos, vel, 0.05, nsteps, L=cfg.L)
+    tol = 1e-13 * (1 + nsteps)
+    for c in range(3):
+        assert np.max(wrapped_diff(pg[c], po[c])) <= tol * L
+        assert np.max(np.abs(vg[c] - vo[c])) <= tol * 10.0
+        assert np.all(pg[c] >= 0) and np.all(pg[c] < L)
+
+
+def test_initial_velocity_is_cic_of_u(orc, MHD):
+    cfg = inputs.config3(32, kmax=4)
+    rho = 1.0 + 0.3 * np.sin(inputs.grid(32)[0])           # non-uniform density: u = m/rho at the grid points
+    prim = list(cfg.prim)
+    prim[0] = rho * np.ones_like(prim[0])
+    g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+    g.set_fields(prim, "primitive")
+    pos, _ = particles(777, 5)
+    g.tracers_set(pos)
+    pg, vg = g.tracers_get()
+    U = g.get_fields("conservative")
+    u = [U[1 + c] / U[0] for c in range(3)]
+    vo = orc.cic(u, pos, L=cfg.L)
+    for c in range(3):
+        assert np.max(np.abs(vg[c] - vo[c])) <= 1e-13
+        assert np.array_equal(pg[c], pos[c])
+
+
+@pytest.mark.parametrize("N,fused", [(32, 1), (128, 1), (128, 0), (128, 2)])
+def test_tracers_advance_with_the_fields(orc, MHD, N, fused):
+    """mhd_step with tracers attached vs the oracle with tracers attached: the push of step n uses B(t_n).  N = 128 with
+    fused = 1 takes B from the by-product of the fused x sweep, the other cases from a separate inverse transform."""
+    cfg = inputs.config3(N, kmax=4) if N > 32 else inputs.config2(N)
+    dt = 2e-3
+    o = orc.Oracle(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, dt)
+    o.set_fields(cfg.prim, "primitive")
+    g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, dt)
+    g.set_option(1, fused)
+    g.set_fields(cfg.prim, "primitive")
+    pos, vel = particles(1000, 11 + N, vscale=2.0)
+    o.tracers_set(pos, vel)
+    g.tracers_set(pos, vel)
+    nsteps = 6
+    o.step(nsteps)
+    g.step(3)
+    g.step(nsteps - 3)                                  # split calls: same result
+    po, vo = o.tracers_get()
+    pg, vg = g.tracers_get()
+    tol = 1e-13 * (1 + nsteps)
+    for c in range(3):
+        assert np.max(wrapped_diff(pg[c], po[c])) <= tol * L, (c, np.max(wrapped_diff(pg[c], po[c])))
+        assert np.max(np.abs(vg[c] - vo[c])) <= tol * 10.0
+    # and the fields are untouched by the presence of tracers
+    Ug, Uo = g.get_fields(), o.get_fields()
+    scale = max(np.linalg.norm(x) for x in Uo)       # some components (m_z, B_z of config 2) are roundoff-small
+    for f in range(8):
+        assert np.linalg.norm(Ug[f] - Uo[f]) <= 1e-12 * scale
+
+
+@pytest.mark.parametrize("integ", [1, 2])
+def test_tracers_with_other_integrators_use_start_of_step_B(orc, MHD, integ):
+    """RK4 / predictor-corrector: the tracers still see B(t_n) of the step's initial state (separate transform)."""
+    cfg = inputs.config2(32)
+    g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, 1e-3)
+    g.set_option(3, integ)
+    g.set_fields(cfg.prim, "primitive")
+    pos, vel = particles(300, 2)
+    g.tracers_set(pos, vel)
+    p, v = pos, vel
+    for s in range(3):
+        B = g.get_fields("conservative")[5:8]
+        p, v = orc.tracers_push(B, p, v, 1e-3, 1, L=cfg.L)
+        g.step(1)
+    pg, vg = g.tracers_get()
+    for c in range(3):
+        assert np.max(wrapped_diff(pg[c], p[c])) <= 1e-12 and np.max(np.abs(vg[c] - v[c])) <= 1e-12
+
+
+def test_device_pointers_and_errors(MHD):
+    import torch
+    cfg = inputs.config1(32)
+    g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+    pos, vel = particles(100, 3)
+    with pytest.raises(RuntimeError):
+        g.tracers_set(pos)                               # CIC of u needs fields
+    g.set_fields(cfg.prim, "primitive")
+    with pytest.raises(RuntimeError):
+        g.tracers_push(1)                                # no tracers yet
+    dp = [torch.from_numpy(x).cuda() for x in pos]
+    dv = [torch.from_numpy(x).cuda() for x in vel]
+    g.tracers_set(dp, dv)
+    g.tracers_push(3)
+    pd, vd = g.tracers_get("device")
+    g.tracers_set(pos, vel)
+    g.tracers_push(3)
+    ph, vh = g.tracers_get()
+    for c in range(3):
+        assert np.array_equal(pd[c].cpu().numpy(), ph[c]) and np.array_equal(vd[c].cpu().numpy(), vh[c])
+    # speed is conserved by the rotation
+    s0 = np.sqrt(sum(x ** 2 for x in vel))
+    s1 = np.sqrt(sum(x ** 2 for x in vh))
+    assert np.max(np.abs(s1 - s0) / s0) <= 1e-14
+    # positions outside [0, L) are wrapped on input
+    far = [x + 3 * L for x in pos]
+    g.tracers_set(far, vel)
+    pw, _ = g.tracers_get()
+    for c in range(3):
+        assert np.max(wrapped_diff(pw[c], pos[c])) <= 1e-14 * 4 * L and np.all(pw[c] < L)
+    from paper_1810_12707_b200 import binding
+    ooc = MHD(32, flags=binding.MHD_FLAG_OUT_OF_CORE)
+    with pytest.raises(RuntimeError):
+        ooc.tracers_set(pos, vel)
