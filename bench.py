@@ -227,6 +227,38 @@ def fft_metric(g, torch, N, nf=8, reps=5):
     return out
 
 
+def tracer_metric(g, torch, N, L, np_, K, ms_step_plain):
+    """Tracer particles (Sec. VI): particle-pushes/s of the gather + Boris kernel in a frozen field (two
+    launches of different length, so that the 3-field inverse transform of mhd_tracers_push cancels), and the cost of
+    carrying the tracers through mhd_step (B taken from the fused x sweep)."""
+    gen = torch.Generator(device=g.device).manual_seed(7)
+    pos = [torch.rand(np_, dtype=torch.float64, device=g.device, generator=gen) * L for _ in range(3)]
+    g.tracers_set(pos)                      # v0 = CIC of u
+
+    def timed(fn):
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(g.stream); fn(); e1.record(g.stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1)
+
+    g.tracers_push(1)
+    n1, n2 = 2, 22
+    t1 = min(timed(lambda: g.tracers_push(n1)) for _ in range(3))
+    t2 = min(timed(lambda: g.tracers_push(n2)) for _ in range(3))
+    per_push_ms = (t2 - t1) / (n2 - n1)
+    g.step(2)
+    ms_with = timed(lambda: g.step(K)) / K
+    # sector model of the gather: 3 fields x 4 (y,z) corner rows x 1-2 32-byte sectors + 6 x 8 B particle state r/w
+    sector_bytes = 3 * 4 * 1.25 * 32 + 96
+    return {"particles": np_, "pushes_per_s_frozen_field": np_ / (per_push_ms * 1e-3), "ms_per_push_launch": per_push_ms,
+            "gather_sector_bytes_per_push_model": sector_bytes,
+            "gather_gbs_model": sector_bytes * np_ / per_push_ms / 1e6,
+            "ms_per_step_with_tracers": ms_with, "ms_per_step_without": ms_step_plain,
+            "step_overhead_frac": ms_with / ms_step_plain - 1.0,
+            "positions": "uniform random (seeded) in the box; v0 = CIC of u"}
+
+
 def pcie_peaks(torch, device, nbytes=1 << 30, reps=4):
     """Measured pinned-memory copy bandwidth of this box (GB/s): host->device alone, device->host alone, and both
     directions at once on two streams — the ceiling of the chunked pipeline when arrays live on the host."""
@@ -387,6 +419,8 @@ def run_ours(args):
     if rank == 0 and not args.no_fft and not flags:
         host = None
         extra["fft3d"] = fft_metric(g, torch, N)
+    if rank == 0 and args.tracers > 0 and not flags:
+        extra["tracers"] = tracer_metric(g, torch, N, cfg.L, args.tracers, K, ms / K)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
         cpu = cpu_baseline(N)
@@ -425,6 +459,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-fft", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--tracers", type=int, default=0, metavar="NP",
+                    help="also measure NP tracer particles (PAPER.md Sec. VI): frozen-field pushes/s and the step overhead")
     ap.add_argument("--option", action="append", default=[], metavar="ID=VALUE",
                     help="mhd_set_option(ID, VALUE) before the run (include/mhd.h MHD_OPT_*), for A/B measurements")
     args = ap.parse_args()

@@ -34,6 +34,7 @@ def lib():
         L.orc_set_threads.argtypes = [C.c_int]
         L.orc_get_threads.restype = C.c_int
         L.orc_use_direct_dft.argtypes = [C.c_void_p, C.c_int]
+        L.orc_set_variant.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int]
         L.orc_set_fields.argtypes = [C.c_void_p, C.c_int, PP]
         L.orc_get_fields.argtypes = [C.c_void_p, C.c_int, PP]
         L.orc_rhs.argtypes = [C.c_void_p, PP]
@@ -139,6 +140,10 @@ class Oracle:
 
     def use_direct_dft(self, on=True):
         _check(lib().orc_use_direct_dft(self._h, int(on)))
+
+    def set_variant(self, cs2=0.0, f0=0.0, kf=1, evolve=3):
+        """Equation-set variants: barotropic closure (cs2 > 0), ABC forcing (f0, kf), switched-off equations."""
+        _check(lib().orc_set_variant(self._h, float(cs2), float(f0), int(kf), int(evolve)))
 
     def set_fields(self, fields, kind="primitive"):
         f = [_c_in(x) for x in fields]

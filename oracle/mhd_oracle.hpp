@@ -167,6 +167,11 @@ public:
     T L, gamma, mu, eta, dt, k0;
     T time = T(0);
     long long nstep = 0;
+    // Equation-set variants of the paper (readings V1-V3):
+    T cs2 = T(0);      // > 0: barotropic closure P = C_s^2 rho of Eq. 5 / Eq. 18 (L63, L192); E is then not evolved
+    T f0 = T(0);       // amplitude of the ABC forcing rho f of Eq. 18 / L215, f = f0 (sin kz + cos ky, sin kx + cos kz, sin ky + cos kx)
+    int kf = 1;        // its integer mode number k_f (k = k_f 2 pi/L)
+    int evolve = 3;    // bit 0: Eq. 17-18 (+ energy) evolve; bit 1: Eq. 19 evolves ("turn off" of L199 / L205)
     bool use_direct_dft = false;   // P13: substitute the O(N^6) definition for the FFT
     bool have_fields = false;
     rfield<T> U[NF];        // conservative state in real space
@@ -268,7 +273,7 @@ public:
             for (int c = 0; c < 3; ++c) u[c][i] = (*m[c])[i] / rho[i];
             const T b2 = (*B[0])[i] * (*B[0])[i] + (*B[1])[i] * (*B[1])[i] + (*B[2])[i] * (*B[2])[i];
             const T mu_dot = mx[i] * u[0][i] + my[i] * u[1][i] + mz[i] * u[2][i];
-            const T P = (gamma - T(1)) * (E[i] - T(0.5) * mu_dot - T(0.5) * b2);
+            const T P = cs2 > T(0) ? cs2 * rho[i] : (gamma - T(1)) * (E[i] - T(0.5) * mu_dot - T(0.5) * b2);
             Pt[i] = P + T(0.5) * b2;
             q[i] = T(0.5) * (u[0][i] * u[0][i] + u[1][i] * u[1][i] + u[2][i] * u[2][i]);
         }
@@ -368,6 +373,35 @@ public:
             accum_phi(BY, exy); accum_phi(BY, eyz);
             accum_phi(BZ, exz); accum_phi(BZ, eyz);
         }
+
+        // Eq. 18 forcing rho f (L192, L215) and its work m.f in the energy equation (reading V1); like every product
+        // it is dealias-projected (operator family O1, op 4)
+        if (f0 != T(0)) {
+            rfield<T> f[3];
+            for (auto& c : f) c.resize(N3);
+            const T kk = k0 * T(kf), dx = L / T(N);
+            for (int iz = 0; iz < N; ++iz)
+                for (int iy = 0; iy < N; ++iy)
+                    for (int ix = 0; ix < N; ++ix) {
+                        const std::int64_t i = (std::int64_t(iz) * N + iy) * N + ix;
+                        const T x = dx * T(ix), y = dx * T(iy), z = dx * T(iz);
+                        f[0][i] = f0 * (std::sin(kk * z) + std::cos(kk * y));
+                        f[1][i] = f0 * (std::sin(kk * x) + std::cos(kk * z));
+                        f[2][i] = f0 * (std::sin(kk * y) + std::cos(kk * x));
+                    }
+            rfield<T> work(N3, T(0));
+            for (int c = 0; c < 3; ++c) {
+                rfield<T> prod(N3);
+                for (std::int64_t i = 0; i < N3; ++i) { prod[i] = rho[i] * f[c][i]; work[i] += (*m[c])[i] * f[c][i]; }
+                const rfield<T> pr = project(prod);
+                for (std::int64_t i = 0; i < N3; ++i) R[MX + c][i] += pr[i];
+            }
+            const rfield<T> pw = project(work);
+            for (std::int64_t i = 0; i < N3; ++i) R[EN][i] += pw[i];
+        }
+        if (cs2 > T(0)) R[EN].assign(N3, T(0));                              // barotropic: no energy equation
+        if (!(evolve & 1)) for (int c = RHO; c <= EN; ++c) R[c].assign(N3, T(0));
+        if (!(evolve & 2)) for (int c = BX; c <= BZ; ++c) R[c].assign(N3, T(0));
 
         if (phi) for (int f = 0; f < NF; ++f) phi[f] = std::sqrt(phi2[f]);
         if (dsc) {

@@ -27,6 +27,10 @@ void orc_set_threads(int n);               /* OpenMP threads used by the pencil 
 int orc_get_threads(void);
 int orc_use_direct_dft(orc_ctx *c, int on); /* substitute the O(N^6) DFT for the FFT (pin P13)        */
 
+/* equation-set variants (Eq. 5/18 barotropic closure, Eq. 18 + L215 ABC forcing, L199/L205 switched-off
+ * equations): cs2 > 0 selects P = cs2*rho; f0, kf = forcing amplitude and integer mode; evolve bit 0 = Eq. 17-18 (+E),
+ * bit 1 = Eq. 19 */
+int orc_set_variant(orc_ctx *c, double cs2, double f0, int kf, int evolve);
 int orc_set_fields(orc_ctx *c, int kind, const double *const f[8]);  /* 0 conservative, 1 primitive  */
 int orc_get_fields(orc_ctx *c, int kind, double *const out[8]);
 int orc_rhs(orc_ctx *c, double *const out[8]);                       /* dU/dt of the current state    */

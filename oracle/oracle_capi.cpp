@@ -123,6 +123,12 @@ int orc_get_threads(void) {
 
 int orc_use_direct_dft(orc_ctx* c, int on) { return guarded([&] { DISPATCH(c, S.use_direct_dft = (on != 0)); }); }
 
+int orc_set_variant(orc_ctx* c, double cs2, double f0, int kf, int evolve) {
+    return guarded([&] {
+        if (cs2 < 0 || kf < 0 || evolve < 0 || evolve > 3) throw std::invalid_argument("variant");
+        DISPATCH(c, { S.cs2 = cs2; S.f0 = f0; S.kf = kf; S.evolve = evolve; S.have_old = false; });
+    });
+}
 int orc_set_fields(orc_ctx* c, int kind, const double* const f[8]) {
     return guarded([&] { if (kind != 0 && kind != 1) throw std::invalid_argument("kind"); DISPATCH(c, S.set_fields(kind, f)); });
 }
