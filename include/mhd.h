@@ -75,6 +75,17 @@ extern "C" {
 
 #define MHD_OPT_STRIDED_COLS 7 /* tuning: kx columns per CTA of the strided (y, z) passes, 0 = default, 4 / 8 / 16 */
 
+/* Equation-set variants of the paper (readings V1-V3).  Changing one resets the integrator history. */
+#define MHD_OPT_EVOLVE 8  /* bit 0: Eq. 17-18 and the energy equation evolve, bit 1: Eq. 19 evolves (default 3).  2 = the
+                             kinematic dynamo of PAPER.md L205 ("turn off Eq. 17 and 18"), 1 = hydrodynamic (L199)      */
+#define MHD_OPT_FORCE_K 9 /* integer mode number k_f >= 1 of the ABC forcing (default 1)                               */
+/* parameters for mhd_set_param() */
+#define MHD_PARAM_CS2 1       /* C_s^2 > 0: barotropic closure P = C_s^2 rho (Eq. 5, Eq. 18): E is carried
+                                 but not evolved (R_E = 0); 0 (default): ideal gas, P from E (R1)             */
+#define MHD_PARAM_FORCE_AMP 2 /* f0: external force rho f in the momentum equation (Eq. 18) with the ABC profile of
+                                 L215, f = f0 (sin k z + cos k y, sin k x + cos k z, sin k y + cos k x), k = k_f 2 pi/L,
+                                 and its work m.f in the energy equation; 0 (default): unforced.  In-core contexts only */
+
 typedef struct mhd_ctx mhd_ctx; /* opaque, owned by the library */
 
 /* Diagnostics record ("per grid" = volume means; L71 Eq. 9; R8). */
@@ -111,6 +122,7 @@ int mhd_bind(mhd_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream,
              void *pinned_host, size_t pinned_bytes);
 
 int mhd_set_option(mhd_ctx *ctx, int option, int value);
+int mhd_set_param(mhd_ctx *ctx, int param, double value);
 
 /* Load a state.  f[i]: N^3 doubles each.  Primitive input is converted point-wise to conservative; each of the
  * 8 conservative fields is then dealias-projected, U <- IFFT(M FFT U) (R5).  Resets t = 0, step = 0

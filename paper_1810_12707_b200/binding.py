@@ -35,7 +35,7 @@ SYMBOLS = ["mhd_init", "mhd_workspace_bytes", "mhd_pinned_bytes", "mhd_bind", "m
            "mhd_rhs", "mhd_step", "mhd_get_fields", "mhd_diagnostics", "mhd_nspec", "mhd_fft3d_r2c",
            "mhd_fft3d_c2r", "mhd_launch_count", "mhd_transfer_bytes", "mhd_profile_enable", "mhd_profile_get", "mhd_last_error",
            "mhd_destroy", "mhd_tracers_bytes", "mhd_tracers_bind", "mhd_tracers_set", "mhd_tracers_get",
-           "mhd_tracers_push"]
+           "mhd_tracers_push", "mhd_set_param"]
 
 
 class MhdDiag(C.Structure):
@@ -64,6 +64,7 @@ def lib():
     L.mhd_pinned_bytes.restype = C.c_size_t
     L.mhd_bind.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p, C.c_uint, C.c_void_p, C.c_size_t]
     L.mhd_set_option.argtypes = [C.c_void_p, C.c_int, C.c_int]
+    L.mhd_set_param.argtypes = [C.c_void_p, C.c_int, C.c_double]
     L.mhd_set_fields.argtypes = [C.c_void_p, C.c_int, C.c_int, P8]
     L.mhd_rhs.argtypes = [C.c_void_p, C.c_int, P8]
     L.mhd_step.argtypes = [C.c_void_p, C.c_int]
@@ -181,6 +182,16 @@ class MHD:
     # -- the ABI calls ------------------------------------------------------------------------------------
     def set_option(self, option, value):
         self._check(self._L.mhd_set_option(self._h, int(option), int(value)))
+
+    def set_param(self, param, value):
+        self._check(self._L.mhd_set_param(self._h, int(param), float(value)))
+
+    def set_variant(self, cs2=0.0, f0=0.0, kf=1, evolve=3):
+        """Equation-set variants (include/mhd.h MHD_PARAM_CS2, MHD_PARAM_FORCE_AMP, MHD_OPT_FORCE_K, MHD_OPT_EVOLVE)."""
+        self.set_param(1, cs2)
+        self.set_option(9, kf)
+        self.set_param(2, f0)
+        self.set_option(8, evolve)
 
     def set_fields(self, fields, kind="primitive"):
         where, ptrs, keep = self._marshal(fields)

@@ -49,6 +49,8 @@ inline bool valid_N(int N) { return N >= 16 && N <= 1024 && (N & (N - 1)) == 0; 
 struct mhd_ctx {
     int N = 0;
     double L = 0, gamma = 0, mu = 0, eta = 0, dt = 0;
+    double cs2 = 0, f0 = 0;          // variants: barotropic sound speed squared, ABC forcing amplitude
+    int kf = 1, evolve = 3;          // forcing mode number, evolved equation subsets
     bool bound = false, have_fields = false, have_old = false;
     cudaStream_t st = nullptr;
     unsigned flags = 0;
@@ -94,7 +96,7 @@ struct mhd_ctx {
     int hx() const { return N / 2; }
     int kc() const { return N / 3; }
     long long n3() const { return (long long)N * N * N; }
-    Phys phys() const { return Phys{2.0 * M_PI / L, gamma, mu, eta}; }
+    Phys phys() const { return Phys{2.0 * M_PI / L, gamma, mu, eta, cs2, f0, kf, evolve}; }
     SpecGeom geom() const { return SpecGeom{N, N / 2, N / 3, opt_prune}; }
 
     cudaEvent_t get_event() {

@@ -12,6 +12,11 @@ constexpr int MAXF = 16;   // largest batch of fields one launch handles
 struct Phys {
     double k0;       // 2*pi/L : wavenumber of integer mode 1
     double gamma, mu, eta;
+    // equation-set variants (Eq. 5/18, L192, L199, L205, L215)
+    double cs2;      // > 0: barotropic closure P = cs2 * rho, the energy equation is not evolved
+    double f0;       // amplitude of the ABC forcing rho f (0 = unforced)
+    int kf;          // its integer mode number
+    int evolve;      // bit 0: Eq. 17-18 (+ energy) evolve; bit 1: Eq. 19 evolves
 };
 
 // ---- strided (y / z) complex passes on half-spectrum arrays ------------------------------------------------
@@ -102,8 +107,12 @@ struct SpecGeom {
 void launch_build_current(const SpecGeom& g, const cd* const B[3], cd* const J[3], Phys ph, cudaStream_t st);
 // R^ from the 16 transformed product fields and the state; mode 0: write R^ to rout only;
 // mode 1: Euler update U += dt R, Rold = R; mode 2: AB2 update U += dt(1.5 R - 0.5 Rold), Rold = R
+// force (or null): 4 arrays F^_x, F^_y, F^_z, (m.f)^ added to R_m and R_E (launch_forcing below)
 void launch_assemble(const SpecGeom& g, const cd* const prod[16], cd* const U[8], cd* const Rold[8],
-                     cd* const rout[8], int mode, double dt, Phys ph, cudaStream_t st);
+                     cd* const rout[8], int mode, double dt, Phys ph, cudaStream_t st, const cd* const force[4] = nullptr);
+// ABC forcing in k-space (full layout only): F^ = M (rho f)^ and M (m.f)^ as +-kf shifts of rho^, m^ (exact: the
+// state is band-limited to the mask).  add = 0: out[0..3] = F ; add = 1: out[1..4] += F (out = an 8-field R^ array)
+void launch_forcing(const SpecGeom& g, const cd* const U[8], cd* const out[], int add, Phys ph, cudaStream_t st);
 // generic linear update on masked modes: y[f] = a*y[f] + b*x[f] ... used by RK4 / predictor-corrector
 void launch_axpby(const SpecGeom& g, int nf, double a, cd* const y[], double b, const cd* const x[], cudaStream_t st);
 void launch_copy_masked(const SpecGeom& g, int nf, cd* const dst[], const cd* const src[], cudaStream_t st);

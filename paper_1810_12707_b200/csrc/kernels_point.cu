@@ -104,7 +104,8 @@ void launch_divergence(const SpecGeom& g, const cd* const B[3], cd* out, Phys ph
 
 // ---- R^ assembly (+ explicit update) -------------------------------------------------------------------
 // mode 0: rout = R ; 1: U += dt R, Rold = R ; 2: U += dt (1.5 R - 0.5 Rold), Rold = R
-__global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 rout, int mode, double dt, Phys ph) {
+struct PtrC4 { const cd* p[4]; };
+__global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 rout, int mode, double dt, Phys ph, PtrC4 force) {
     ModeIt m;
     if (!mode_of_thread(g, m)) return;
     const long long i = m.idx, j = m.sidx;     // products / state
@@ -128,6 +129,13 @@ __global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 r
         R[5] = imul(ky, ez) - imul(kz, ey) - (ph.eta * k2) * u[5];
         R[6] = imul(kz, ex) - imul(kx, ez) - (ph.eta * k2) * u[6];
         R[7] = imul(kx, ey) - imul(ky, ex) - (ph.eta * k2) * u[7];
+        if (force.p[0]) {        // variants: rho f and its work m.f (launch_forcing), state geometry
+#pragma unroll
+            for (int f = 0; f < 4; ++f) R[1 + f] = R[1 + f] + force.p[f][j];
+        }
+        if (ph.cs2 > 0.0) R[4] = mk(0, 0);                      // barotropic: no energy equation
+        if (!(ph.evolve & 1)) { R[0] = R[1] = R[2] = R[3] = R[4] = mk(0, 0); }
+        if (!(ph.evolve & 2)) { R[5] = R[6] = R[7] = mk(0, 0); }
         if (mode == 0) {
 #pragma unroll
             for (int f = 0; f < 8; ++f) rout.p[f][i] = R[f];     // work-array geometry (may alias the products)
@@ -147,11 +155,64 @@ __global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 r
     }
 }
 void launch_assemble(const SpecGeom& g, const cd* const prod[16], cd* const U[8], cd* const Rold[8],
-                     cd* const rout[8], int mode, double dt, Phys ph, cudaStream_t st) {
-    PtrC16 p; Ptr8 u, ro, rr;
+                     cd* const rout[8], int mode, double dt, Phys ph, cudaStream_t st, const cd* const force[4]) {
+    PtrC16 p; Ptr8 u, ro, rr; PtrC4 fc;
+    for (int f = 0; f < 4; ++f) fc.p[f] = force ? force[f] : nullptr;
     for (int f = 0; f < 16; ++f) p.p[f] = prod[f];
     for (int f = 0; f < 8; ++f) { u.p[f] = U[f]; ro.p[f] = Rold ? Rold[f] : nullptr; rr.p[f] = rout ? rout[f] : nullptr; }
-    assemble_kernel<<<mode_grid(g, KT), KT, 0, st>>>(g, p, u, ro, rr, mode, dt, ph);
+    assemble_kernel<<<mode_grid(g, KT), KT, 0, st>>>(g, p, u, ro, rr, mode, dt, ph, fc);
+}
+
+// ---- ABC forcing in k-space ------------------------------------------------------------------------------
+// a^(n) of a real field from its half spectrum (nx >= 0 stored; Hermitian symmetry for nx < 0); zero outside the mask
+__device__ __forceinline__ cd spec_at(const cd* __restrict__ a, int N, int hx, int kc, int nx, int ny, int nz) {
+    if (abs(nx) > kc || abs(ny) > kc || abs(nz) > kc) return mk(0, 0);
+    const bool neg = nx < 0;
+    if (neg) { nx = -nx; ny = -ny; nz = -nz; }
+    const int iy = ny >= 0 ? ny : ny + N, iz = nz >= 0 ? nz : nz + N;
+    const cd v = a[((long long)iz * N + iy) * hx + nx];
+    return neg ? cconj(v) : v;
+}
+// (a sin(kf x_d))^(n) = (a^(n - kf e_d) - a^(n + kf e_d)) / (2i) ;  (a cos(kf x_d))^(n) = (a^(n - kf e_d) + a^(n + kf e_d)) / 2
+__device__ __forceinline__ void shifted(const cd* __restrict__ a, const SpecGeom& g, const ModeIt& m, int d, int kf, cd& lo, cd& hi) {
+    const int dx = d == 0 ? kf : 0, dy = d == 1 ? kf : 0, dz = d == 2 ? kf : 0;
+    lo = spec_at(a, g.N, g.hx, g.kc, m.nx - dx, m.ny - dy, m.nz - dz);
+    hi = spec_at(a, g.N, g.hx, g.kc, m.nx + dx, m.ny + dy, m.nz + dz);
+}
+__device__ __forceinline__ cd times_sin(const cd* a, const SpecGeom& g, const ModeIt& m, int d, int kf) {
+    cd lo, hi; shifted(a, g, m, d, kf, lo, hi);
+    const cd df = lo - hi;
+    return mk(0.5 * df.y, -0.5 * df.x);      // / (2i)
+}
+__device__ __forceinline__ cd times_cos(const cd* a, const SpecGeom& g, const ModeIt& m, int d, int kf) {
+    cd lo, hi; shifted(a, g, m, d, kf, lo, hi);
+    return 0.5 * (lo + hi);
+}
+__global__ void forcing_kernel(SpecGeom g, Ptr8 U, Ptr8 out, int add, Phys ph) {
+    ModeIt m;
+    if (!mode_of_thread(g, m) || !m.inside) return;
+    const int kf = ph.kf;
+    // f = f0 (sin kz + cos ky, sin kx + cos kz, sin ky + cos kx)    (A = B = C = 1)
+    cd F[4];
+    F[0] = ph.f0 * (times_sin(U.p[0], g, m, 2, kf) + times_cos(U.p[0], g, m, 1, kf));
+    F[1] = ph.f0 * (times_sin(U.p[0], g, m, 0, kf) + times_cos(U.p[0], g, m, 2, kf));
+    F[2] = ph.f0 * (times_sin(U.p[0], g, m, 1, kf) + times_cos(U.p[0], g, m, 0, kf));
+    F[3] = ph.f0 * (times_sin(U.p[1], g, m, 2, kf) + times_cos(U.p[1], g, m, 1, kf)
+                    + times_sin(U.p[2], g, m, 0, kf) + times_cos(U.p[2], g, m, 2, kf)
+                    + times_sin(U.p[3], g, m, 1, kf) + times_cos(U.p[3], g, m, 0, kf));
+    if (ph.cs2 > 0.0) F[3] = mk(0, 0);
+    if (!(ph.evolve & 1)) F[0] = F[1] = F[2] = F[3] = mk(0, 0);
+#pragma unroll
+    for (int f = 0; f < 4; ++f) {
+        if (add) out.p[1 + f][m.idx] = out.p[1 + f][m.idx] + F[f];
+        else out.p[f][m.idx] = F[f];
+    }
+}
+void launch_forcing(const SpecGeom& g, const cd* const U[8], cd* const out[], int add, Phys ph, cudaStream_t st) {
+    Ptr8 u, o;
+    for (int f = 0; f < 8; ++f) { u.p[f] = const_cast<cd*>(U[f]); o.p[f] = nullptr; }
+    for (int f = 0; f < (add ? 8 : 4); ++f) o.p[f] = out[f];
+    forcing_kernel<<<mode_grid(g, KT), KT, 0, st>>>(g, u, o, add, ph);
 }
 
 // ---- y = a y + b x on the masked modes (integrator stages) -----------------------------------------------

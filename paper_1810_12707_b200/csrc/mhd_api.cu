@@ -158,8 +158,23 @@ void products(mhd_ctx* c, cd* const Uin[8], double* const breal[3] = nullptr) {
 // R^(Uin) -> rout (mode 0) or explicit update of Uin / Rold (mode 1 Euler, 2 AB2)
 void rhs_spectral(mhd_ctx* c, cd* const Uin[8], cd* const rout[8], int mode, double* const breal[3] = nullptr) {
     products(c, Uin, breal);
-    mhd_ctx::Scope s(c, F_ASSEMBLE);
-    launch_assemble(c->geom(), c->W, Uin, c->Rold, rout, mode, c->dt, c->phys(), c->st);
+    const bool forced = c->f0 != 0.0;
+    SpecGeom gp = c->geom(); gp.pruned = 1;
+    const cd* Uc[8];
+    for (int f = 0; f < 8; ++f) Uc[f] = Uin[f];
+    const cd* force[4] = {c->Y[0], c->Y[1], c->Y[2], c->Y[3]};
+    if (forced && mode != 0) {      // the update is in place: the +-k_f neighbours of U^ must be read before it starts
+        mhd_ctx::Scope s(c, F_POINT);
+        launch_forcing(gp, Uc, c->Y, 0, c->phys(), c->st);
+    }
+    {
+        mhd_ctx::Scope s(c, F_ASSEMBLE);
+        launch_assemble(c->geom(), c->W, Uin, c->Rold, rout, mode, c->dt, c->phys(), c->st, (forced && mode != 0) ? force : nullptr);
+    }
+    if (forced && mode == 0) {      // U^ is not modified: add F^ to the assembled R^ (Y may hold integrator stages)
+        mhd_ctx::Scope s(c, F_POINT);
+        launch_forcing(gp, Uc, rout, 1, c->phys(), c->st);
+    }
 }
 
 // ---- tracer particles (Sec. VI) ----------------------------------------------------------------------
@@ -294,6 +309,12 @@ int mhd_set_option(mhd_ctx* c, int option, int value) {
         case MHD_OPT_STRIDED_COLS:
             if (value != 0 && value != 4 && value != 8 && value != 16) return c->fail(MHD_ERR_INVALID_ARG, "strided columns must be 0, 4, 8 or 16");
             c->opt_strided_cols = value; return MHD_OK;
+        case MHD_OPT_EVOLVE:
+            if (value < 0 || value > 3) return c->fail(MHD_ERR_INVALID_ARG, "evolve must be 0..3");
+            c->evolve = value; c->have_old = false; return MHD_OK;
+        case MHD_OPT_FORCE_K:
+            if (value < 1 || value > c->kc()) return c->fail(MHD_ERR_INVALID_ARG, "forcing mode must be in 1..kc");
+            c->kf = value; c->have_old = false; return MHD_OK;
         case MHD_OPT_OOC_BRICK:
             if (value < 0) return c->fail(MHD_ERR_INVALID_ARG, "brick size must be >= 0");
             c->ooc.brick_max = value; return MHD_OK;
@@ -301,6 +322,20 @@ int mhd_set_option(mhd_ctx* c, int option, int value) {
             if (value < 0) return c->fail(MHD_ERR_INVALID_ARG, "slab size must be >= 0");
             c->ooc.slab_max = value; return MHD_OK;
         default: return c->fail(MHD_ERR_INVALID_ARG, "unknown option");
+    }
+}
+
+int mhd_set_param(mhd_ctx* c, int param, double value) {
+    if (!c) return MHD_ERR_INVALID_ARG;
+    switch (param) {
+        case MHD_PARAM_CS2:
+            if (!(value >= 0.0)) return c->fail(MHD_ERR_INVALID_ARG, "C_s^2 must be >= 0");
+            c->cs2 = value; c->have_old = false; return MHD_OK;
+        case MHD_PARAM_FORCE_AMP:
+            if (value != value) return c->fail(MHD_ERR_INVALID_ARG, "forcing amplitude is NaN");
+            if (value != 0.0 && c->ooc.on) return c->fail(MHD_ERR_INVALID_ARG, "forcing needs an in-core context");
+            c->f0 = value; c->have_old = false; return MHD_OK;
+        default: return c->fail(MHD_ERR_INVALID_ARG, "unknown parameter");
     }
 }
 

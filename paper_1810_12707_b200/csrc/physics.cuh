@@ -25,7 +25,8 @@ __device__ __forceinline__ void flux_point(const double (&s)[S_NIN], double (&o)
     const double bx = s[S_BX], by = s[S_BY], bz = s[S_BZ];
     const double b2 = bx * bx + by * by + bz * bz;
     const double mu_dot = s[S_MX] * ux + s[S_MY] * uy + s[S_MZ] * uz;
-    const double P = (ph.gamma - 1.0) * (s[S_E] - 0.5 * mu_dot - 0.5 * b2);
+    const double P = ph.cs2 > 0.0 ? ph.cs2 * s[S_RHO]                                   // barotropic closure (Eq. 5 / 18)
+                                  : (ph.gamma - 1.0) * (s[S_E] - 0.5 * mu_dot - 0.5 * b2);
     const double Pt = P + 0.5 * b2;
     o[P_TXX] = s[S_MX] * ux + Pt - bx * bx;
     o[P_TXY] = s[S_MX] * uy - bx * by;
