@@ -249,11 +249,10 @@ def tracer_metric(g, torch, N, L, np_, K, ms_step_plain):
     per_push_ms = (t2 - t1) / (n2 - n1)
     g.step(2)
     ms_with = timed(lambda: g.step(K)) / K
-    # sector model of the gather: 3 fields x 4 (y,z) corner rows x 1-2 32-byte sectors + 6 x 8 B particle state r/w
-    sector_bytes = 3 * 4 * 1.25 * 32 + 96
+    # bytes that must move per push: 6 x 8 B of particle state read + written; the grid rows come from L1 / L2 once the
+    # storage is sorted by grid row (MHD_OPT_TRACER_SORT), from DRAM at sector granularity (~670 B per push) if it is not
     return {"particles": np_, "pushes_per_s_frozen_field": np_ / (per_push_ms * 1e-3), "ms_per_push_launch": per_push_ms,
-            "gather_sector_bytes_per_push_model": sector_bytes,
-            "gather_gbs_model": sector_bytes * np_ / per_push_ms / 1e6,
+            "particle_state_bytes_per_push": 96, "particle_state_gbs": 96.0 * np_ / per_push_ms / 1e6,
             "ms_per_step_with_tracers": ms_with, "ms_per_step_without": ms_step_plain,
             "step_overhead_frac": ms_with / ms_step_plain - 1.0,
             "positions": "uniform random (seeded) in the box; v0 = CIC of u"}

@@ -75,6 +75,11 @@ extern "C" {
 
 #define MHD_OPT_STRIDED_COLS 7 /* tuning: kx columns per CTA of the strided (y, z) passes, 0 = default, 4 / 8 / 16 */
 
+#define MHD_OPT_L2_SLAB 10 /* z planes per slab of the in-core L2 slab loop over sweeps S2-S4 (0 = whole volume per launch) */
+
+#define MHD_OPT_TRACER_SORT 11 /* re-sort the tracer storage by grid row every this many pushes (default 32; 0 = never):
+                                  gather locality only, results do not depend on it (mhd_tracers_get returns id order) */
+
 /* Equation-set variants of the paper (readings V1-V3).  Changing one resets the integrator history. */
 #define MHD_OPT_EVOLVE 8  /* bit 0: Eq. 17-18 and the energy equation evolve, bit 1: Eq. 19 evolves (default 3).  2 = the
                              kinematic dynamo of PAPER.md L205 ("turn off Eq. 17 and 18"), 1 = hydrodynamic (L199)      */
@@ -163,7 +168,8 @@ int mhd_fft3d_c2r(mhd_ctx *ctx, int nfields, double *const spec[], double *const
  *      cell volume, corner indices wrapped periodically, L255);
  *   3) Eq. 21 (L259-265): t = B_p dt/2, s = 2t/(1+|t|^2), v_d = v + v x t, v(t+dt) = v + v_d x s;
  *   4) Eq. 22 (L266): x(t+dt) = x + v(t+dt) dt, wrapped into [0, L).
- * Storage: the caller provides mhd_tracers_bytes(np) device bytes (256-byte aligned) and keeps them alive; pos / vel
+ * Storage: the caller provides mhd_tracers_bytes(np) device bytes (256-byte aligned; two sets of particle arrays, ids
+ * and the scratch of the spatial sort, ~130 B per particle + 4 MB) and keeps them alive; pos / vel
  * arguments are 3 arrays (x, y, z components) of np doubles, host or device as `where` says.
  * mhd_tracers_set: positions are wrapped into [0, L); vel == NULL sets the initial velocity to the CIC interpolation
  *   of u = m/rho of the current state (L241; needs mhd_set_fields first).

@@ -54,7 +54,7 @@ struct mhd_ctx {
     bool bound = false, have_fields = false, have_old = false;
     cudaStream_t st = nullptr;
     unsigned flags = 0;
-    int opt_fused = 1, opt_prune = 1, opt_fuse_current = 1, integrator = 0, opt_strided_cols = 0;
+    int opt_fused = 1, opt_prune = 1, opt_fuse_current = 1, integrator = 0, opt_strided_cols = 0, opt_slab = 0;
     long long step = 0;
     long long launches = 0;
     std::string err;
@@ -83,7 +83,14 @@ struct mhd_ctx {
         long long np = 0;
         bool set = false;
         double *pos[3] = {nullptr, nullptr, nullptr}, *vel[3] = {nullptr, nullptr, nullptr};
+        // spatial sort: second set of arrays (ping-pong), particle ids, counting-sort scratch
+        double* alt[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+        long long *id = nullptr, *alt_id = nullptr;
+        unsigned *hist = nullptr, *key = nullptr, *rank = nullptr;
+        bool sorted = false;           // storage order != id order
+        int since_sort = 0;            // pushes since the last sort
     } tr;
+    int opt_tracer_sort = 32;          // re-sort the tracers every this many pushes (0 = never sort)
     // profiling
     bool prof = false;
     struct Rec { int fam; cudaEvent_t a, b; };

@@ -158,6 +158,11 @@ void launch_tracer_push(const TracerArgs& a, cudaStream_t st);
 // vel <- CIC interpolation of m/rho (real-space rho, mx, my, mz)
 void launch_tracer_init_velocity(const TracerArgs& a, const double* rho, const double* const m[3], cudaStream_t st);
 void launch_tracer_wrap(const TracerArgs& a, cudaStream_t st);
+// spatial sort by grid row (see tracers.cu): (pos, vel, id) -> (alt[0..5], alt_id); hist holds N*N bins
+void launch_tracer_sort(const TracerArgs& a, const long long* id, double* const alt[6], long long* alt_id, unsigned* hist,
+                        unsigned* key, unsigned* rank, cudaStream_t st);
+void launch_tracer_iota(long long np, long long* id, cudaStream_t st);
+void launch_tracer_unpermute(long long np, const long long* id, const double* in, double* out, cudaStream_t st);
 
 void launch_twiddle_table(int N, cd* tw, cudaStream_t st);
 

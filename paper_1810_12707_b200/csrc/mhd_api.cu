@@ -16,15 +16,17 @@ namespace {
 
 // ---- sweeps --------------------------------------------------------------------------------------------------
 // strided pass over nf arrays; axis 1 = y, 2 = z; hx = row pitch of the arrays (N/2, or 8 for the Nyquist planes)
+// axis 1 only: z0 / nz restrict the pass to the z planes [z0, z0 + nz) (nz = 0: all planes) — the L2 slab loop
 void strided_pass(mhd_ctx* c, int dir, int axis, int nf, const cd* const in[], cd* const out[], int hx, int ncols_full,
-                  bool prune, int jfirst = -1, int bfirst = 0) {
+                  bool prune, int jfirst = -1, int bfirst = 0, int z0 = 0, int nz = 0) {
     const int N = c->N, kc = c->kc();
     int done = 0;
     while (done < nf) {
         const int nb = std::min(nf - done, MAXF);
         StridedArgs a;
         std::memset(&a, 0, sizeof(a));
-        for (int f = 0; f < nb; ++f) { a.in[f] = in[done + f]; a.out[f] = out[done + f]; }
+        const long long zoff = (axis == 1 && nz > 0) ? (long long)z0 * N * hx : 0;
+        for (int f = 0; f < nb; ++f) { a.in[f] = in[done + f] + zoff; a.out[f] = out[done + f] + zoff; }
         a.tw = c->tw;
         a.kc = kc;
         a.nfields = nb;
@@ -33,7 +35,7 @@ void strided_pass(mhd_ctx* c, int dir, int axis, int nf, const cd* const in[], c
         a.cols = c->opt_strided_cols;
         if (axis == 1) {            // y pass: rows along y, outer = z (all planes)
             a.in_row_stride = a.out_row_stride = hx; a.in_outer_stride = a.out_outer_stride = (long long)N * hx;
-            a.n_outer = N; a.outer_split = N; a.outer_skip = 0;
+            a.n_outer = nz > 0 ? nz : N; a.outer_split = N; a.outer_skip = 0;
         } else {                    // z pass: rows along z, outer = ky (pruned to the mask)
             a.in_row_stride = a.out_row_stride = (long long)N * hx; a.in_outer_stride = a.out_outer_stride = hx;
             if (prune) { a.n_outer = 2 * kc + 1; a.outer_split = kc + 1; a.outer_skip = N - (2 * kc + 1); }
@@ -132,26 +134,38 @@ void products(mhd_ctx* c, cd* const Uin[8], double* const breal[3] = nullptr) {
         }
         strided_pass(c, +1, 2, 11, in, c->W, c->hx(), c->hx(), prune);    // S1b
     }
-    strided_pass(c, +1, 1, 11, c->W, c->W, c->hx(), c->hx(), prune);      // S2
+    // S2-S4 work inside z planes.  They run slab after slab (a few planes at a time) so that what the inverse y pass
+    // writes is still in the 126 MB L2 when the fused x sweep reads it, and what that writes when the forward y pass reads
+    // it: the 27 intermediate field sweeps between S1 and S5 then never reach HBM.
     const int kmax = prune ? c->kc() : c->hx() - 1;
     const double scale = 1.0 / ((double)N * N * N);
-    if (c->opt_fused) {                                                   // S3
-        run_x_fused(c, c->W, c->W, (long long)N * N, breal);
-    } else {
-        XArgs a; std::memset(&a, 0, sizeof(a));
-        for (int f = 0; f < 11; ++f) { a.spec_in[f] = c->W[f]; a.real_out[f] = reinterpret_cast<double*>(c->W[f]); }
-        a.tw = c->tw; a.nlines = (long long)N * N; a.nfields = 11; a.kmax = kmax; a.scale = scale;
-        { mhd_ctx::Scope s(c, F_X_C2R); launch_x_c2r(N, a, c->st); }
-        const double* rin[11]; double* rout[16];
-        for (int f = 0; f < 11; ++f) rin[f] = reinterpret_cast<const double*>(c->W[f]);
-        for (int f = 0; f < 16; ++f) rout[f] = reinterpret_cast<double*>(c->W[f]);
-        { mhd_ctx::Scope s(c, F_FLUX); launch_flux_real(c->n3(), rin, rout, ph, c->st); }
-        XArgs b; std::memset(&b, 0, sizeof(b));
-        for (int f = 0; f < 16; ++f) { b.real_in[f] = rout[f]; b.spec_out[f] = c->W[f]; }
-        b.tw = c->tw; b.nlines = (long long)N * N; b.nfields = 16; b.kmax = kmax; b.scale = 1.0;
-        { mhd_ctx::Scope s(c, F_X_R2C); launch_x_r2c(N, b, c->st); }
+    const int slab = (c->opt_fused && c->opt_slab > 0) ? std::min(c->opt_slab, N) : N;
+    for (int z0 = 0; z0 < N; z0 += slab) {
+        const int nz = std::min(slab, N - z0);
+        strided_pass(c, +1, 1, 11, c->W, c->W, c->hx(), c->hx(), prune, -1, 0, z0, nz);      // S2
+        if (c->opt_fused) {                                                                 // S3
+            const long long off = (long long)z0 * N * c->hx();
+            cd* w[16];
+            for (int f = 0; f < 16; ++f) w[f] = c->W[f] + off;
+            double* br[3] = {nullptr, nullptr, nullptr};
+            if (breal) for (int d = 0; d < 3; ++d) br[d] = breal[d] + 2 * off;
+            run_x_fused(c, w, w, (long long)nz * N, breal ? br : nullptr);
+        } else {
+            XArgs a; std::memset(&a, 0, sizeof(a));
+            for (int f = 0; f < 11; ++f) { a.spec_in[f] = c->W[f]; a.real_out[f] = reinterpret_cast<double*>(c->W[f]); }
+            a.tw = c->tw; a.nlines = (long long)N * N; a.nfields = 11; a.kmax = kmax; a.scale = scale;
+            { mhd_ctx::Scope s(c, F_X_C2R); launch_x_c2r(N, a, c->st); }
+            const double* rin[11]; double* rout[16];
+            for (int f = 0; f < 11; ++f) rin[f] = reinterpret_cast<const double*>(c->W[f]);
+            for (int f = 0; f < 16; ++f) rout[f] = reinterpret_cast<double*>(c->W[f]);
+            { mhd_ctx::Scope s(c, F_FLUX); launch_flux_real(c->n3(), rin, rout, ph, c->st); }
+            XArgs b; std::memset(&b, 0, sizeof(b));
+            for (int f = 0; f < 16; ++f) { b.real_in[f] = rout[f]; b.spec_out[f] = c->W[f]; }
+            b.tw = c->tw; b.nlines = (long long)N * N; b.nfields = 16; b.kmax = kmax; b.scale = 1.0;
+            { mhd_ctx::Scope s(c, F_X_R2C); launch_x_r2c(N, b, c->st); }
+        }
+        strided_pass(c, -1, 1, 16, c->W, c->W, c->hx(), c->hx(), prune, -1, 0, z0, nz);      // S4
     }
-    strided_pass(c, -1, 1, 16, c->W, c->W, c->hx(), c->hx(), prune);      // S4
     strided_pass(c, -1, 2, 16, c->W, c->W, c->hx(), c->hx(), prune);      // S5a
 }
 
@@ -194,10 +208,28 @@ void tracers_real_B(mhd_ctx* c, double* Breal[3]) {
     for (int d = 0; d < 3; ++d) Breal[d] = reinterpret_cast<double*>(c->X[d]);
     inverse3d(c, 3, spec, work, Breal, true);
 }
+// spatial sort of the particle storage (tracers.cu); ping-pongs the two sets of arrays
+void tracers_sort(mhd_ctx* c) {
+    auto& t = c->tr;
+    {
+        mhd_ctx::Scope s(c, F_TRACERS, 3);
+        launch_tracer_sort(tracer_args(c, nullptr, 0), t.id, t.alt, t.alt_id, t.hist, t.key, t.rank, c->st);
+    }
+    for (int d = 0; d < 3; ++d) { std::swap(t.pos[d], t.alt[d]); std::swap(t.vel[d], t.alt[3 + d]); }
+    std::swap(t.id, t.alt_id);
+    t.sorted = true; t.since_sort = 0;
+}
+// nsteps pushes in the field Breal; the storage is re-sorted every opt_tracer_sort pushes
 void tracers_push_with(mhd_ctx* c, double* const Breal[3], int nsteps) {
     const double* B[3] = {Breal[0], Breal[1], Breal[2]};
-    mhd_ctx::Scope s(c, F_TRACERS);
-    launch_tracer_push(tracer_args(c, B, nsteps), c->st);
+    const int every = c->opt_tracer_sort;
+    while (nsteps > 0) {
+        if (every > 0 && c->tr.since_sort >= every) tracers_sort(c);
+        const int n = every > 0 ? std::min(nsteps, every - c->tr.since_sort) : nsteps;
+        mhd_ctx::Scope s(c, F_TRACERS);
+        launch_tracer_push(tracer_args(c, B, n), c->st);
+        c->tr.since_sort += n; nsteps -= n;
+    }
 }
 
 int copy_in(mhd_ctx* c, int where, const double* const src[8], double* const dst[8]) {
@@ -309,6 +341,12 @@ int mhd_set_option(mhd_ctx* c, int option, int value) {
         case MHD_OPT_STRIDED_COLS:
             if (value != 0 && value != 4 && value != 8 && value != 16) return c->fail(MHD_ERR_INVALID_ARG, "strided columns must be 0, 4, 8 or 16");
             c->opt_strided_cols = value; return MHD_OK;
+        case MHD_OPT_L2_SLAB:
+            if (value < 0) return c->fail(MHD_ERR_INVALID_ARG, "slab planes must be >= 0");
+            c->opt_slab = value; return MHD_OK;
+        case MHD_OPT_TRACER_SORT:
+            if (value < 0) return c->fail(MHD_ERR_INVALID_ARG, "tracer sort interval must be >= 0");
+            c->opt_tracer_sort = value; return MHD_OK;
         case MHD_OPT_EVOLVE:
             if (value < 0 || value > 3) return c->fail(MHD_ERR_INVALID_ARG, "evolve must be 0..3");
             c->evolve = value; c->have_old = false; return MHD_OK;
@@ -527,7 +565,12 @@ int mhd_fft3d_c2r(mhd_ctx* c, int nfields, double* const spec[], double* const r
     return check_cuda(c, "fft3d_c2r");
 }
 
-size_t mhd_tracers_bytes(long long np) { return np <= 0 ? 0 : 6 * align_up((size_t)np * sizeof(double)); }
+// 12 particle arrays (two sets: the spatial sort ping-pongs), 2 id arrays, key + rank, 2^20 histogram bins
+static size_t tracer_hist_bytes() { return align_up(((size_t)1 << 20) * sizeof(unsigned)); }
+size_t mhd_tracers_bytes(long long np) {
+    if (np <= 0) return 0;
+    return 14 * align_up((size_t)np * sizeof(double)) + 2 * align_up((size_t)np * sizeof(unsigned)) + tracer_hist_bytes();
+}
 
 int mhd_tracers_bind(mhd_ctx* c, long long np, void* dev_buffer, size_t bytes) {
     if (!c || np < 0) return MHD_ERR_INVALID_ARG;
@@ -537,12 +580,19 @@ int mhd_tracers_bind(mhd_ctx* c, long long np, void* dev_buffer, size_t bytes) {
     if (np == 0) return MHD_OK;
     if (!dev_buffer || ((uintptr_t)dev_buffer & 255) != 0) return c->fail(MHD_ERR_INVALID_ARG, "tracer buffer must be 256-byte aligned");
     if (bytes < mhd_tracers_bytes(np)) return c->fail(MHD_ERR_NOMEM, "tracer buffer too small");
-    const size_t stride = align_up((size_t)np * sizeof(double));
+    if (np >= ((long long)1 << 32)) return c->fail(MHD_ERR_INVALID_ARG, "at most 2^32 - 1 tracers");
+    const size_t stride = align_up((size_t)np * sizeof(double)), istride = align_up((size_t)np * sizeof(unsigned));
     char* b = static_cast<char*>(dev_buffer);
     for (int d = 0; d < 3; ++d) {
         c->tr.pos[d] = reinterpret_cast<double*>(b + (size_t)d * stride);
         c->tr.vel[d] = reinterpret_cast<double*>(b + (size_t)(3 + d) * stride);
     }
+    for (int f = 0; f < 6; ++f) c->tr.alt[f] = reinterpret_cast<double*>(b + (size_t)(6 + f) * stride);
+    c->tr.id = reinterpret_cast<long long*>(b + 12 * stride);
+    c->tr.alt_id = reinterpret_cast<long long*>(b + 13 * stride);
+    c->tr.key = reinterpret_cast<unsigned*>(b + 14 * stride);
+    c->tr.rank = reinterpret_cast<unsigned*>(b + 14 * stride + istride);
+    c->tr.hist = reinterpret_cast<unsigned*>(b + 14 * stride + 2 * istride);
     c->tr.np = np;
     return MHD_OK;
 }
@@ -560,7 +610,8 @@ int mhd_tracers_set(mhd_ctx* c, int where, const double* const pos[3], const dou
         cudaMemcpyAsync(c->tr.pos[d], pos[d], bytes, kind, c->st);
         if (vel) cudaMemcpyAsync(c->tr.vel[d], vel[d], bytes, kind, c->st);
     }
-    { mhd_ctx::Scope s(c, F_TRACERS); launch_tracer_wrap(tracer_args(c, nullptr, 0), c->st); }
+    { mhd_ctx::Scope s(c, F_TRACERS, 2); launch_tracer_wrap(tracer_args(c, nullptr, 0), c->st); launch_tracer_iota(c->tr.np, c->tr.id, c->st); }
+    c->tr.sorted = false; c->tr.since_sort = 0;
     if (!vel) {      // v0 = CIC of u = m/rho (L241): real-space rho, m of the current state -> X[0..3]
         const cd* spec[4] = {c->U[0], c->U[1], c->U[2], c->U[3]};
         cd* work[4] = {c->X[0], c->X[1], c->X[2], c->X[3]};
@@ -571,6 +622,7 @@ int mhd_tracers_set(mhd_ctx* c, int where, const double* const pos[3], const dou
         mhd_ctx::Scope s(c, F_TRACERS);
         launch_tracer_init_velocity(tracer_args(c, nullptr, 0), real[0], m, c->st);
     }
+    if (c->opt_tracer_sort > 0) tracers_sort(c);
     if (where == MHD_HOST) cudaStreamSynchronize(c->st);
     int rc = check_cuda(c, "tracers_set");
     if (rc) return rc;
@@ -586,8 +638,16 @@ int mhd_tracers_get(mhd_ctx* c, int where, double* const pos[3], double* const v
     const size_t bytes = (size_t)c->tr.np * sizeof(double);
     const cudaMemcpyKind kind = where == MHD_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
     for (int d = 0; d < 3; ++d) {
-        if (pos && pos[d]) cudaMemcpyAsync(pos[d], c->tr.pos[d], bytes, kind, c->st);
-        if (vel && vel[d]) cudaMemcpyAsync(vel[d], c->tr.vel[d], bytes, kind, c->st);
+        const double* src[2] = {c->tr.pos[d], c->tr.vel[d]};
+        double* dst[2] = {pos ? pos[d] : nullptr, vel ? vel[d] : nullptr};
+        for (int k = 0; k < 2; ++k) {
+            if (!dst[k]) continue;
+            if (!c->tr.sorted) { cudaMemcpyAsync(dst[k], src[k], bytes, kind, c->st); continue; }
+            // storage is in sorted order: out[id[m]] = in[m], straight into device output or through the spare set
+            double* tmp = where == MHD_DEVICE ? dst[k] : c->tr.alt[0];
+            { mhd_ctx::Scope s(c, F_TRACERS); launch_tracer_unpermute(c->tr.np, c->tr.id, src[k], tmp, c->st); }
+            if (where == MHD_HOST) cudaMemcpyAsync(dst[k], tmp, bytes, cudaMemcpyDeviceToHost, c->st);
+        }
     }
     if (where == MHD_HOST) cudaStreamSynchronize(c->st);
     return check_cuda(c, "tracers_get");

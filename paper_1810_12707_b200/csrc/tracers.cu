@@ -117,7 +117,81 @@ __global__ void tracer_wrap_kernel(const __grid_constant__ TracerArgs a) {
 
 unsigned blocks_for(long long np) { return (unsigned)((np + 127) / 128); }
 
+// ---- spatial sort (counting sort by grid row) ------------------------------------------------------------------
+// Random particle order makes the gather DRAM-bound at sector granularity (ncu: ~670 B of DRAM reads per push at 256^3,
+// against 48 B of particle state).  Sorted by the (z, y) row of their cell, consecutive threads read the same few grid
+// rows, which then come from L1 / L2.  key = iz * N + iy (N^2 <= 2^20 bins); three kernels: histogram (the atomic's
+// return value is the particle's rank inside its bin), exclusive scan of the bins, scatter.  The order inside a bin
+// depends on the atomics, but every particle's own trajectory does not depend on where it is stored, and
+// mhd_tracers_get un-permutes by id: results are bitwise independent of the sort.
+__global__ void sort_hist_kernel(const __grid_constant__ TracerArgs a, unsigned* __restrict__ hist, unsigned* __restrict__ key,
+                                 unsigned* __restrict__ rank) {
+    const long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= a.np) return;
+    const CellIdx c = locate(a.N, (double)a.N / a.L, a.pos[0][m], a.pos[1][m], a.pos[2][m]);
+    const unsigned k = (unsigned)c.i0[2] * (unsigned)a.N + (unsigned)c.i0[1];
+    key[m] = k;
+    rank[m] = atomicAdd(&hist[k], 1u);
+}
+// exclusive scan of n <= 2^20 bins by one block of 1024 threads (each thread owns a contiguous run)
+__global__ void __launch_bounds__(1024) sort_scan_kernel(unsigned* __restrict__ hist, int n) {
+    __shared__ unsigned part[1024];
+    const int t = threadIdx.x, per = (n + 1023) / 1024, lo = t * per, hi = min(n, lo + per);
+    unsigned s = 0;
+    for (int i = lo; i < hi; ++i) s += hist[i];
+    part[t] = s;
+    __syncthreads();
+    for (int d = 1; d < 1024; d <<= 1) {
+        const unsigned v = t >= d ? part[t - d] : 0u;
+        __syncthreads();
+        part[t] += v;
+        __syncthreads();
+    }
+    unsigned run = part[t] - s;
+    for (int i = lo; i < hi; ++i) { const unsigned h = hist[i]; hist[i] = run; run += h; }
+}
+struct SortIO { const double* src[6]; double* dst[6]; const long long* id_src; long long* id_dst; };
+__global__ void sort_scatter_kernel(long long np, const unsigned* __restrict__ hist, const unsigned* __restrict__ key,
+                                    const unsigned* __restrict__ rank, const __grid_constant__ SortIO io) {
+    const long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= np) return;
+    const long long d = (long long)hist[key[m]] + rank[m];
+#pragma unroll
+    for (int f = 0; f < 6; ++f) io.dst[f][d] = io.src[f][m];
+    io.id_dst[d] = io.id_src[m];
+}
+__global__ void iota_kernel(long long np, long long* id) {
+    const long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m < np) id[m] = m;
+}
+// out[id[m]] = in[m]
+__global__ void unpermute_kernel(long long np, const long long* __restrict__ id, const double* __restrict__ in, double* __restrict__ out) {
+    const long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (m < np) out[id[m]] = in[m];
+}
+
 }  // namespace
+
+void launch_tracer_iota(long long np, long long* id, cudaStream_t st) {
+    if (np > 0) iota_kernel<<<blocks_for(np), 128, 0, st>>>(np, id);
+}
+void launch_tracer_unpermute(long long np, const long long* id, const double* in, double* out, cudaStream_t st) {
+    if (np > 0) unpermute_kernel<<<blocks_for(np), 128, 0, st>>>(np, id, in, out);
+}
+// sorts (pos, vel, id) into (alt_pos, alt_vel, alt_id); the caller swaps the buffers.  4 launches + one memset.
+void launch_tracer_sort(const TracerArgs& a, const long long* id, double* const alt[6], long long* alt_id, unsigned* hist,
+                        unsigned* key, unsigned* rank, cudaStream_t st) {
+    if (a.np <= 0) return;
+    const int nbins = a.N * a.N;
+    cudaMemsetAsync(hist, 0, (size_t)nbins * sizeof(unsigned), st);
+    sort_hist_kernel<<<blocks_for(a.np), 128, 0, st>>>(a, hist, key, rank);
+    sort_scan_kernel<<<1, 1024, 0, st>>>(hist, nbins);
+    SortIO io;
+    for (int d = 0; d < 3; ++d) { io.src[d] = a.pos[d]; io.src[3 + d] = a.vel[d]; }
+    for (int f = 0; f < 6; ++f) io.dst[f] = alt[f];
+    io.id_src = id; io.id_dst = alt_id;
+    sort_scatter_kernel<<<blocks_for(a.np), 128, 0, st>>>(a.np, hist, key, rank, io);
+}
 
 void launch_tracer_push(const TracerArgs& a, cudaStream_t st) {
     if (a.np > 0) tracer_push_kernel<<<blocks_for(a.np), 128, 0, st>>>(a);
