@@ -30,6 +30,9 @@ if ROOT not in sys.path:
 
 METRIC = "fp64 grid-point-steps/s"
 UNIT = "grid-point-steps/s"
+# fp64 instructions the fused x sweep executes per (y,z) line, from the committed ncu capture (profiles/r01b_ncu_full_*.md:
+# fp64 pipe busy fraction x 2 warp-instructions/clk/SM x active cycles); DESIGN.md section 6 derives the same figure by hand
+X_FUSED_FP64_INSTR_PER_LINE = {512: 312.0e3, 256: 141.3e3}
 FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
 
 
@@ -388,6 +391,14 @@ def run_ours(args):
                                    "frac_vs_1184B": unpruned_reference_bytes(N) / step_ms_local / 1e6 / peak,
                                    "frac_vs_1184B_nominal_8TBs": unpruned_reference_bytes(N) / step_ms_local / 1e6 / 8000.0},
                     "families": fam}
+        if "x_fused" in fam and N in X_FUSED_FP64_INSTR_PER_LINE:
+            # the fused x sweep is bound by fp64 issue, not by HBM: second roofline against the measured DFMA issue rate
+            peak_i = g.probe_fp64()
+            ach_i = X_FUSED_FP64_INSTR_PER_LINE[N] * N * N / (fam["x_fused"]["avg_launch_ms"] * 1e-3)
+            roofline["alu"] = {"bound": "alu", "kernel": "x_fused", "achieved": ach_i / 1e9, "peak": peak_i / 1e9,
+                               "unit": "Ginstr/s (fp64 pipe)", "frac": ach_i / peak_i,
+                               "peak_source": "measured in this run: register-only DFMA kernel (mhd_probe_fp64)",
+                               "nominal_peak": 148 * 64 * 1.965, "instr_per_line": X_FUSED_FP64_INSTR_PER_LINE[N]}
         tpath = os.path.join(ROOT, "profiles", "traffic_r01.json")
         if os.path.exists(tpath):   # DRAM bytes per launch from the committed ncu --set full capture
             try:

@@ -185,6 +185,11 @@ int mhd_tracers_push(mhd_ctx *ctx, int nsteps);
 /* Bytes the chunked pipeline has copied host->device / device->host so far (0 for an in-core context). */
 int mhd_transfer_bytes(const mhd_ctx *ctx, long long *h2d, long long *d2h);
 
+/* Measurement helper for the bench (not part of the method): fp64 instructions per second of a register-only DFMA
+ * kernel on the current device = the issue ceiling of the fp64 pipe ("measure it with an FMA
+ * micro-benchmark"); flop/s of pure-FMA code is twice that. */
+int mhd_probe_fp64(mhd_ctx *ctx, double *instr_per_s);
+
 /* Number of kernels this context has launched so far (for the bench's gpu_launches claim). */
 long long mhd_launch_count(const mhd_ctx *ctx);
 /* Milliseconds and launches accumulated per kernel family since the last reset; names[i] are static strings.

@@ -35,7 +35,7 @@ SYMBOLS = ["mhd_init", "mhd_workspace_bytes", "mhd_pinned_bytes", "mhd_bind", "m
            "mhd_rhs", "mhd_step", "mhd_get_fields", "mhd_diagnostics", "mhd_nspec", "mhd_fft3d_r2c",
            "mhd_fft3d_c2r", "mhd_launch_count", "mhd_transfer_bytes", "mhd_profile_enable", "mhd_profile_get", "mhd_last_error",
            "mhd_destroy", "mhd_tracers_bytes", "mhd_tracers_bind", "mhd_tracers_set", "mhd_tracers_get",
-           "mhd_tracers_push", "mhd_set_param"]
+           "mhd_tracers_push", "mhd_set_param", "mhd_probe_fp64"]
 
 
 class MhdDiag(C.Structure):
@@ -79,6 +79,7 @@ def lib():
     L.mhd_tracers_set.argtypes = [C.c_void_p, C.c_int, P8, P8]
     L.mhd_tracers_get.argtypes = [C.c_void_p, C.c_int, P8, P8]
     L.mhd_tracers_push.argtypes = [C.c_void_p, C.c_int]
+    L.mhd_probe_fp64.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
     L.mhd_launch_count.argtypes = [C.c_void_p]
     L.mhd_launch_count.restype = C.c_longlong
     L.mhd_transfer_bytes.argtypes = [C.c_void_p, C.POINTER(C.c_longlong), C.POINTER(C.c_longlong)]
@@ -293,6 +294,12 @@ class MHD:
     def tracers_push(self, nsteps=1):
         """nsteps Boris pushes in the B of the current state (fields do not advance)."""
         self._check(self._L.mhd_tracers_push(self._h, int(nsteps)))
+
+    def probe_fp64(self):
+        """fp64 instructions / s of a register-only DFMA kernel (the fp64 issue ceiling of this GPU)."""
+        v = C.c_double()
+        self._check(self._L.mhd_probe_fp64(self._h, C.byref(v)))
+        return v.value
 
     def transfer_bytes(self):
         """(host->device, device->host) bytes the chunked pipeline has copied so far."""
