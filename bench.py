@@ -316,7 +316,14 @@ def run_ours(args):
         print(json.dumps({"error": "1024^3 does not fit in core (48 full fields = 412 GB): use --placement device|state_host|all_host"}))
         return 2
     cfg = inputs.config6(N) if N == 1024 else inputs.config45(N)     # config 6 = the out-of-core workload of BASELINE.json
-    g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, device="cuda:%d" % local_rank, flags=flags)
+    if args.decompose:
+        # slab decomposition: ONE problem over all ranks, two all-to-alls per step (strong scaling)
+        from paper_1810_12707_b200.dist import DistMHD
+        flags = B.MHD_FLAG_OUT_OF_CORE
+        g = DistMHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, rank=rank, world=world, device="cuda:%d" % local_rank)
+        args.no_e2e = args.no_fft = True
+    else:
+        g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, device="cuda:%d" % local_rank, flags=flags)
     pin_inputs = N < 1024        # 8 x 8.6 GB of inputs stay pageable at 1024^3 (the pinned budget goes to the solver's arrays)
     host = [torch.from_numpy(p).pin_memory() if pin_inputs else torch.from_numpy(p) for p in cfg.prim]
     cfg.prim = None
@@ -342,7 +349,9 @@ def run_ours(args):
     if flags:
         g.profile_enable(False)
         x0 = g.transfer_bytes()
-        ms_np = time_steps(g, torch, K, dist)          # without the per-family events (they serialise nothing, but to be sure)
+        e0 = getattr(g, "exchanged_bytes", 0)
+        ms_np = time_steps(g, torch, K, dist)
+        e1 = getattr(g, "exchanged_bytes", 0)          # without the per-family events (they serialise nothing, but to be sure)
         x1 = g.transfer_bytes()
         ms = ms_np
         ooc = {"placement": args.placement, "budget_mib": args.budget_mib, "device_workspace_gb": g.workspace_bytes / 1e9,
@@ -356,7 +365,10 @@ def run_ours(args):
             ooc["frac_of_duplex_pcie"] = max(ooc["h2d_gbs"], ooc["d2h_gbs"]) / ooc["pcie_measured"]["each_direction_when_both_gbs"]
     g.profile_enable(False)
     clocks = sampler.stop()
-    ms_max, units = aggregate(ms, float(N) ** 3 * K, dist)
+    if args.decompose:
+        ooc["decomposed"] = {"world": world, "sent_to_peers_bytes_per_step_per_rank": (e1 - e0) / K,
+                             "collective": "torch.distributed.all_to_all_single (NCCL), 2 per step: 11 and 16 work fields"}
+    ms_max, units = aggregate(ms, float(N) ** 3 * K / (world if args.decompose else 1), dist)
     value = units / (ms_max * 1e-3)
 
     # ---- roofline of the dominant kernel family ---------------------------------------------------------------
@@ -437,12 +449,12 @@ def run_ours(args):
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-                "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "strong" if args.decompose else "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
                 "config": {"workload": ("config6_turbulence_out_of_core_%d^3" % N) if N == 1024 else
                            "config%d_abc_dynamo_%d^3" % (5 if N == 512 else 4, N), "N": N, "dt": cfg.dt, "placement": args.placement,
                            "mu": cfg.mu, "eta": cfg.eta, "integrator": "AB2", "fused": 1, "pruned": 1,
-                           "parallelism": "replicas x%d" % world,
+                           "parallelism": ("slab decomposition x%d" if args.decompose else "replicas x%d") % world,
                            "l2": "no flush: one step streams %.1f GB, far beyond the 126 MB L2" % (alg_pruned / 1e9)},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "out_of_core": ooc,
                 "paper_context": {"256^3 s/step P100/V100": [0.32, 0.22], "512^3 s/step P100/V100 (out-of-core)": [80.97, 92.81],
@@ -469,6 +481,9 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-fft", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--decompose", action="store_true",
+                    help="with --gpus N under torchrun: ONE problem decomposed over the N GPUs (ky bricks / z slabs, two NCCL "
+                         "all-to-alls per step) instead of N replicas; with N = 1 it measures the pack / unpack overhead")
     ap.add_argument("--tracers", type=int, default=0, metavar="NP",
                     help="also measure NP tracer particles (PAPER.md Sec. VI): frozen-field pushes/s and the step overhead")
     ap.add_argument("--option", action="append", default=[], metavar="ID=VALUE",

@@ -182,6 +182,30 @@ int mhd_tracers_set(mhd_ctx *ctx, int where, const double *const pos[3], const d
 int mhd_tracers_get(mhd_ctx *ctx, int where, double *const pos[3], double *const vel[3]);
 int mhd_tracers_push(mhd_ctx *ctx, int nsteps);
 
+/* ---- Slab decomposition over several GPUs (not in the paper) -----------------
+ * One process per GPU.  A context bound with MHD_FLAG_OUT_OF_CORE (everything in device memory) becomes rank `rank` of
+ * `world`: it owns a contiguous share of the compact ky axis for the z passes, the assembly and the update (phases A, C)
+ * and a contiguous share of the z planes for the y passes and the fused x sweep (phase B).  Between the phases the work
+ * arrays are transposed across ranks by an all-to-all that THE CALLER performs (torch.distributed over NCCL) on device
+ * buffers packed / unpacked by the library.  One step:
+ *     [phase A]  pack(0,11) -> all-to-all -> unpack(0,11)  phase B  pack(1,16) -> all-to-all -> unpack(1,16)  phase C(next)
+ * phase C with arg != 0 also runs phase A of the next step on the updated bricks (then the next step starts at pack).
+ * mhd_set_fields (every rank passes the full fields; only its z planes are read) must be followed by the exchange
+ * (1, 8) and MHD_DIST_PHASE_STORE; mhd_get_fields (only the rank's z planes of `out` are written) must be preceded by
+ * MHD_DIST_PHASE_STATE_Z and the exchange (0, 8).  mhd_step / mhd_rhs / mhd_diagnostics return MHD_ERR_INVALID_ARG on
+ * a decomposed context.  Counts are in doubles, per peer, in rank order (the split sizes of the all-to-all). */
+#define MHD_DIST_PHASE_A 0        /* U^ -> J^ on load, inverse z pass of own ky bricks -> work[0..10]              */
+#define MHD_DIST_PHASE_B 1        /* inverse y, fused x sweep, forward y on own z planes -> work[0..15]             */
+#define MHD_DIST_PHASE_C 2        /* forward z, assembly, explicit update of own bricks (+ next phase A if arg != 0) */
+#define MHD_DIST_PHASE_STORE 3    /* mhd_set_fields, second half: forward z + projection into the compact state    */
+#define MHD_DIST_PHASE_STATE_Z 4  /* mhd_get_fields, first half: inverse z pass of the state -> work[0..7]          */
+int mhd_dist_config(mhd_ctx *ctx, int rank, int world);
+int mhd_dist_phase(mhd_ctx *ctx, int phase, int arg);
+int mhd_dist_counts(mhd_ctx *ctx, int dir, int nfields, long long *send_counts, long long *recv_counts);
+int mhd_dist_pack(mhd_ctx *ctx, int dir, int nfields, double *dev_sendbuf);
+int mhd_dist_unpack(mhd_ctx *ctx, int dir, int nfields, const double *dev_recvbuf);
+int mhd_dist_ranges(mhd_ctx *ctx, int rank, int *ky_lo, int *ky_hi, int *z_lo, int *z_hi);   /* shares of any rank */
+
 /* Bytes the chunked pipeline has copied host->device / device->host so far (0 for an in-core context). */
 int mhd_transfer_bytes(const mhd_ctx *ctx, long long *h2d, long long *d2h);
 

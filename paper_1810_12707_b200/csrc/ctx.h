@@ -77,6 +77,12 @@ struct mhd_ctx {
         cudaEvent_t ev_h2d[NBUF], ev_comp[NBUF], ev_d2h[NBUF], ev_start = nullptr;
         double *part_diag = nullptr, *part_max = nullptr, *part_spec = nullptr;
         long long h2d_bytes = 0, d2h_bytes = 0;
+        // slab decomposition over `world` GPUs: this rank owns the compact ky
+        // range [ky_lo(rank), ky_lo(rank+1)) for the brick stages and the z planes [z_lo(rank), z_lo(rank+1)) for the slab
+        // stage; the exchange between them is done by the caller (all-to-all) on packed buffers
+        int rank = 0, world = 1;
+        int ky_lo(int r) const { return (int)((long long)nyc * r / world); }
+        int z_lo(int r, int N) const { return (int)((long long)N * r / world); }
     } ooc;
     // tracer particles (tracers.cu): caller-provided device storage, 6 arrays of np doubles
     struct Tracers {
@@ -151,3 +157,7 @@ int ooc_get_fields(mhd_ctx* c, int kind, int where, double* const out[8]);
 int ooc_rhs(mhd_ctx* c, int where, double* const out[8]);
 int ooc_step(mhd_ctx* c, int nsteps);
 int ooc_diagnostics(mhd_ctx* c, mhd_diag* d, double* spec_kin, double* spec_mag, int nspec);
+int ooc_dist_config(mhd_ctx* c, int rank, int world);
+int ooc_dist_phase(mhd_ctx* c, int phase, int arg);
+int ooc_dist_counts(mhd_ctx* c, int dir, int nf, long long* send, long long* recv);
+int ooc_dist_pack(mhd_ctx* c, int dir, int nf, double* buf, int unpack);

@@ -384,7 +384,8 @@ int mhd_set_fields(mhd_ctx* c, int kind, int where, const double* const f[8]) {
     if (c->ooc.on) {
         int rc = ooc_set_fields(c, kind, where, f);
         if (rc) return rc;
-        c->have_fields = true; c->have_old = false; c->step = 0;
+        c->have_fields = c->ooc.world == 1;      // decomposed: only after the exchange and MHD_DIST_PHASE_STORE
+        c->have_old = false; c->step = 0;
         return MHD_OK;
     }
     double* real[8];
@@ -662,6 +663,39 @@ int mhd_tracers_push(mhd_ctx* c, int nsteps) {
     tracers_real_B(c, Breal);
     tracers_push_with(c, Breal, nsteps);
     return check_cuda(c, "tracers_push");
+}
+
+int mhd_dist_config(mhd_ctx* c, int rank, int world) {
+    if (!c) return MHD_ERR_INVALID_ARG;
+    if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
+    return ooc_dist_config(c, rank, world);
+}
+int mhd_dist_phase(mhd_ctx* c, int phase, int arg) {
+    if (!c) return MHD_ERR_INVALID_ARG;
+    if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
+    if (!c->ooc.on) return c->fail(MHD_ERR_INVALID_ARG, "not a chunked-pipeline context");
+    if (phase != MHD_DIST_PHASE_STORE && !c->have_fields) return c->fail(MHD_ERR_NO_FIELDS, "mhd_set_fields has not been called");
+    return ooc_dist_phase(c, phase, arg);
+}
+int mhd_dist_counts(mhd_ctx* c, int dir, int nf, long long* send, long long* recv) {
+    if (!c || !c->bound || !c->ooc.on) return MHD_ERR_INVALID_ARG;
+    return ooc_dist_counts(c, dir, nf, send, recv);
+}
+int mhd_dist_pack(mhd_ctx* c, int dir, int nf, double* buf) {
+    if (!c || !c->bound || !c->ooc.on) return MHD_ERR_INVALID_ARG;
+    return ooc_dist_pack(c, dir, nf, buf, 0);
+}
+int mhd_dist_unpack(mhd_ctx* c, int dir, int nf, const double* buf) {
+    if (!c || !c->bound || !c->ooc.on) return MHD_ERR_INVALID_ARG;
+    return ooc_dist_pack(c, dir, nf, const_cast<double*>(buf), 1);
+}
+int mhd_dist_ranges(mhd_ctx* c, int rank, int* ky_lo, int* ky_hi, int* z_lo, int* z_hi) {
+    if (!c || !c->bound || !c->ooc.on || rank < 0 || rank >= c->ooc.world) return MHD_ERR_INVALID_ARG;
+    if (ky_lo) *ky_lo = c->ooc.ky_lo(rank);
+    if (ky_hi) *ky_hi = c->ooc.ky_lo(rank + 1);
+    if (z_lo) *z_lo = c->ooc.z_lo(rank, c->N);
+    if (z_hi) *z_hi = c->ooc.z_lo(rank + 1, c->N);
+    return MHD_OK;
 }
 
 long long mhd_launch_count(const mhd_ctx* c) { return c ? c->launches : 0; }

@@ -152,8 +152,13 @@ std::vector<std::pair<int, int>> brick_chunks(const mhd_ctx* c) {
     if (o.brick_max > 0) nmax = std::min<long long>(nmax, o.brick_max);
     nmax = std::max<long long>(1, std::min<long long>(nmax, kc + 1));
     std::vector<std::pair<int, int>> v;
-    for (int y = 0; y <= kc; y += (int)nmax) v.push_back({y, (int)std::min<long long>(nmax, kc + 1 - y)});
-    for (int y = kc + 1; y <= 2 * kc; y += (int)nmax) v.push_back({y, (int)std::min<long long>(nmax, 2 * kc + 1 - y)});
+    const int ya = o.ky_lo(o.rank), yb = o.ky_lo(o.rank + 1);     // this rank's share (everything when world = 1)
+    auto add = [&](int lo, int hi) {
+        lo = std::max(lo, ya); hi = std::min(hi, yb);
+        for (int y = lo; y < hi; y += (int)nmax) v.push_back({y, (int)std::min<long long>(nmax, hi - y)});
+    };
+    add(0, kc + 1);
+    add(kc + 1, 2 * kc + 1);
     return v;
 }
 std::vector<std::pair<int, int>> slab_chunks(const mhd_ctx* c) {
@@ -163,7 +168,8 @@ std::vector<std::pair<int, int>> slab_chunks(const mhd_ctx* c) {
     if (o.slab_max > 0) nmax = std::min<long long>(nmax, o.slab_max);
     nmax = std::max<long long>(1, std::min<long long>(nmax, c->N));
     std::vector<std::pair<int, int>> v;
-    for (int z = 0; z < c->N; z += (int)nmax) v.push_back({z, (int)std::min<long long>(nmax, c->N - z)});
+    const int za = o.z_lo(o.rank, c->N), zb = o.z_lo(o.rank + 1, c->N);
+    for (int z = za; z < zb; z += (int)nmax) v.push_back({z, (int)std::min<long long>(nmax, zb - z)});
     return v;
 }
 
@@ -531,6 +537,7 @@ int ooc_set_fields(mhd_ctx* c, int kind, int where, const double* const f[8]) {
     SlabIO io; io.nin = 0; io.nout = 8; io.kind = kind; io.where = where; io.user_in = f;
     int rc = stage_slabs(c, SLAB_FROM_REAL, io);
     if (rc) return rc;
+    if (c->ooc.world > 1) return check_cuda(c, "set_fields (decomposed, slab part)");   // exchange, then MHD_DIST_PHASE_STORE
     rc = stage_forward_z_store(c);
     if (rc) return rc;
     if (where == MHD_HOST) cudaStreamSynchronize(c->st);
@@ -539,7 +546,7 @@ int ooc_set_fields(mhd_ctx* c, int kind, int where, const double* const f[8]) {
 
 int ooc_get_fields(mhd_ctx* c, int kind, int where, double* const out[8]) {
     for (int i = 0; i < 8; ++i) if (!out[i]) return c->fail(MHD_ERR_INVALID_ARG, "null field pointer");
-    int rc = stage_inverse_z(c, c->ooc.Uc, false);
+    int rc = c->ooc.world > 1 ? MHD_OK : stage_inverse_z(c, c->ooc.Uc, false);   // decomposed: MHD_DIST_PHASE_STATE_Z + exchange came first
     if (rc) return rc;
     SlabIO io; io.nin = 8; io.nout = 0; io.kind = kind; io.where = where; io.user_out = out;
     rc = stage_slabs(c, SLAB_TO_REAL, io);
@@ -558,6 +565,7 @@ static int ooc_products(mhd_ctx* c, bool have_inverse_z = false) {
 }
 
 int ooc_rhs(mhd_ctx* c, int where, double* const out[8]) {
+    if (c->ooc.world > 1) return c->fail(MHD_ERR_INVALID_ARG, "mhd_rhs is not available on a decomposed context");
     for (int i = 0; i < 8; ++i) if (!out[i]) return c->fail(MHD_ERR_INVALID_ARG, "null field pointer");
     int rc = ooc_products(c);
     if (rc) return rc;
@@ -571,6 +579,7 @@ int ooc_rhs(mhd_ctx* c, int where, double* const out[8]) {
 }
 
 int ooc_step(mhd_ctx* c, int nsteps) {
+    if (c->ooc.world > 1) return c->fail(MHD_ERR_INVALID_ARG, "decomposed context: drive the step with mhd_dist_phase and the exchanges");
     if (c->integrator != 0) return c->fail(MHD_ERR_INVALID_ARG, "the chunked pipeline implements Adams-Bashforth only");
     for (int s = 0; s < nsteps; ++s) {
         int rc = ooc_products(c, s > 0);
@@ -586,6 +595,7 @@ int ooc_step(mhd_ctx* c, int nsteps) {
 int ooc_diagnostics(mhd_ctx* c, mhd_diag* d, double* spec_kin, double* spec_mag, int nspec) {
     Ooc& o = c->ooc;
     const int ns = nspec_of(c->N);
+    if (o.world > 1) return c->fail(MHD_ERR_INVALID_ARG, "mhd_diagnostics is not available on a decomposed context");
     if (spec_kin) return c->fail(MHD_ERR_INVALID_ARG, "the kinetic spectrum needs an unpruned transform: not available in the chunked pipeline");
     if (spec_mag && nspec != ns) return c->fail(MHD_ERR_INVALID_ARG, "nspec must equal mhd_nspec(N)");
     int rc = stage_diag_bricks(c, spec_mag != nullptr);
@@ -610,4 +620,83 @@ int ooc_diagnostics(mhd_ctx* c, mhd_diag* d, double* spec_kin, double* spec_mag,
     d->rho_min = host[8]; d->p_min = host[9]; d->max_divb = host[16];
     if (spec_mag) std::memcpy(spec_mag, host.data() + 64 + ns, ns * sizeof(double));
     return MHD_OK;
+}
+
+// ---- slab decomposition over several GPUs (include/mhd.h mhd_dist_*) ------------------------------
+// The chunked pipeline already separates what is local to a ky range (stages A, C: z passes, assembly, update) from what
+// is local to a z range (stage B: y passes, fused x sweep).  Rank r of `world` runs A / C on its share of the compact ky
+// axis and B on its share of the z planes; between them the z-full work arrays [z][ky_c][kx_c] are transposed across
+// ranks by an all-to-all that the caller performs (torch.distributed / NCCL) on buffers packed and unpacked here.
+int ooc_dist_config(mhd_ctx* c, int rank, int world) {
+    Ooc& o = c->ooc;
+    if (!o.on || o.state_host || o.work_host) return c->fail(MHD_ERR_INVALID_ARG, "decomposition needs MHD_FLAG_OUT_OF_CORE with everything in device memory");
+    if (world < 1 || rank < 0 || rank >= world || world > o.nyc || world > c->N) return c->fail(MHD_ERR_INVALID_ARG, "rank / world");
+    o.rank = rank; o.world = world;
+    c->have_fields = false; c->have_old = false; c->step = 0;
+    return MHD_OK;
+}
+
+int ooc_dist_phase(mhd_ctx* c, int phase, int arg) {
+    switch (phase) {
+        case MHD_DIST_PHASE_A: return stage_inverse_z(c, c->ooc.Uc, true);
+        case MHD_DIST_PHASE_B: { SlabIO io; io.nin = 11; io.nout = 16; return stage_slabs(c, SLAB_FLUX, io); }
+        case MHD_DIST_PHASE_C: {
+            if (c->integrator != 0) return c->fail(MHD_ERR_INVALID_ARG, "the chunked pipeline implements Adams-Bashforth only");
+            int rc = stage_forward_z_assemble(c, c->have_old ? 2 : 1, arg != 0);
+            if (rc) return rc;
+            c->have_old = true; ++c->step;
+            return MHD_OK;
+        }
+        case MHD_DIST_PHASE_STORE: {
+            int rc = stage_forward_z_store(c);
+            if (rc) return rc;
+            c->have_fields = true; c->have_old = false; c->step = 0;
+            return MHD_OK;
+        }
+        case MHD_DIST_PHASE_STATE_Z: return stage_inverse_z(c, c->ooc.Uc, false);
+        default: return c->fail(MHD_ERR_INVALID_ARG, "unknown phase");
+    }
+}
+
+// block exchanged with peer s, in doubles.  dir 0 (bricks -> slabs): send my ky range x peer's z range, receive the peer's
+// ky range x my z range; dir 1 (slabs -> bricks) the other way round.
+int ooc_dist_counts(mhd_ctx* c, int dir, int nf, long long* send, long long* recv) {
+    const Ooc& o = c->ooc;
+    if ((dir != 0 && dir != 1) || nf < 1 || nf > 16) return c->fail(MHD_ERR_INVALID_ARG, "dir / nf");
+    const long long ny_me = o.ky_lo(o.rank + 1) - o.ky_lo(o.rank), nz_me = o.z_lo(o.rank + 1, c->N) - o.z_lo(o.rank, c->N);
+    for (int s = 0; s < o.world; ++s) {
+        const long long ny_s = o.ky_lo(s + 1) - o.ky_lo(s), nz_s = o.z_lo(s + 1, c->N) - o.z_lo(s, c->N);
+        long long a = 2LL * nf * nz_s * ny_me * o.nxp, b = 2LL * nf * nz_me * ny_s * o.nxp;
+        if (s == o.rank) a = b = 0;          // the rank's own block (my ky range x my z range) is already in place
+        if (send) send[s] = dir == 0 ? a : b;
+        if (recv) recv[s] = dir == 0 ? b : a;
+    }
+    return MHD_OK;
+}
+
+// pack (unpack = 0): work arrays -> buf = [peer 0 block | peer 1 block | ...], block = [f][z][ky][kx_c]; unpack = 1: the
+// received buffer of the same exchange -> work arrays.  One 2-D device copy per (peer, field) on the solver's stream.
+int ooc_dist_pack(mhd_ctx* c, int dir, int nf, double* buf, int unpack) {
+    const Ooc& o = c->ooc;
+    if ((dir != 0 && dir != 1) || nf < 1 || nf > 16 || !buf) return c->fail(MHD_ERR_INVALID_ARG, "dir / nf / buffer");
+    const int N = c->N, me = o.rank;
+    cd* p = reinterpret_cast<cd*>(buf);
+    const size_t pitch = (size_t)o.nyc * o.nxp;
+    for (int s = 0; s < o.world; ++s) {
+        if (s == me) continue;                                   // own block: stays where it is
+        // geometry of the block in the work arrays: which rank's z range and which rank's ky range
+        const bool mine_ky = (dir == 0) != (unpack != 0);        // pack dir 0 / unpack dir 1: my ky, peer's z
+        const int rz = mine_ky ? s : me, ry = mine_ky ? me : s;
+        const int z0 = o.z_lo(rz, N), nz = o.z_lo(rz + 1, N) - z0, y0 = o.ky_lo(ry), ny = o.ky_lo(ry + 1) - y0;
+        const size_t width = (size_t)ny * o.nxp;
+        for (int f = 0; f < nf; ++f) {
+            cd* w = o.Wz[f] + (size_t)z0 * pitch + (size_t)y0 * o.nxp;
+            if (nz > 0 && ny > 0) {
+                if (!unpack) cudaMemcpy2DAsync(p, width * sizeof(cd), w, pitch * sizeof(cd), width * sizeof(cd), nz, cudaMemcpyDeviceToDevice, c->st);
+                else cudaMemcpy2DAsync(w, pitch * sizeof(cd), p, width * sizeof(cd), width * sizeof(cd), nz, cudaMemcpyDeviceToDevice, c->st);
+            }
+            p += width * nz;
+        }
+    }
+    return check_cuda(c, unpack ? "dist unpack" : "dist pack");
 }

@@ -1,0 +1,110 @@
+"""Slab decomposition over several GPUs, tested on ONE GPU: `world` virtual ranks run the
+protocol of paper_1810_12707_b200/dist.py one after the other in one process (no kernel waits on another rank), the
+all-to-all is a set of device copies.  The result must equal the undecomposed chunked pipeline BITWISE — the same
+kernels see the same data, only who computes which brick / slab changes — and the oracle within the usual tolerance."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1810_12707_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def mods():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1810_12707_b200 import build, binding, dist
+    build.build()
+    return binding, dist
+
+
+def make_ranks(dist, cfg, world, dt=None):
+    return dist.Lockstep([dist.DistMHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, dt or cfg.dt, rank=r, world=world)
+                          for r in range(world)])
+
+
+@pytest.mark.parametrize("N,world", [(32, 2), (32, 3), (64, 4), (128, 8), (64, 7)])
+def test_decomposed_step_is_bitwise_the_single_gpu_step(mods, N, world):
+    binding, dist = mods
+    cfg = inputs.config3(N, kmax=4) if N >= 64 else inputs.config2(N)
+    ref = binding.MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, flags=binding.MHD_FLAG_OUT_OF_CORE)
+    ref.set_fields(cfg.prim, "primitive")
+    grp = make_ranks(dist, cfg, world)
+    grp.set_fields(cfg.prim, "primitive")
+    U0r, U0g = ref.get_fields(), grp.get_fields()
+    for f in range(8):
+        assert np.array_equal(U0r[f], U0g[f]), ("after set_fields", f)
+    ref.step(3); grp.step(3)            # Euler start + AB2, phase A of steps 2, 3 fused into phase C
+    ref.step(2); grp.step(2)            # a second call: phase A runs on its own again
+    Ur, Ug = ref.get_fields("primitive"), grp.get_fields("primitive")
+    for f in range(8):
+        assert np.array_equal(Ur[f], Ug[f]), ("after 5 steps", f)
+
+
+def test_decomposed_run_matches_oracle(orc, mods):
+    binding, dist = mods
+    cfg = inputs.config1(32)
+    o = orc.Oracle(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+    o.set_fields(cfg.prim, "primitive")
+    grp = make_ranks(dist, cfg, 4)
+    grp.set_fields(cfg.prim, "primitive")
+    o.step(10); grp.step(10)
+    Uo, Ug = o.get_fields(), grp.get_fields()
+    scale = max(np.linalg.norm(x) for x in Uo)
+    for f in range(8):
+        assert np.linalg.norm(Ug[f] - Uo[f]) <= 1e-12 * scale
+
+
+def test_library_partition_and_packing_match_the_host_logic(mods):
+    """mhd_dist_ranges / mhd_dist_counts / mhd_dist_pack against dist.ranges / split_counts / pack_host (the host
+    logic that the gloo test exercises with a real all_to_all_single)."""
+    import torch
+    binding, dist = mods
+    N, world = 32, 3
+    cfg = inputs.config2(N)
+    nyc, nxp = dist.compact_extents(N)
+    for rank in range(world):
+        g = dist.DistMHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, rank=rank, world=world)
+        for r in range(world):
+            assert g.ranges(r) == dist.ranges(N, world, r)
+        for d in (0, 1):
+            for nf in (8, 11, 16):
+                assert g.counts(d, nf) == dist.split_counts(N, world, rank, d, nf)
+        # fill the work arrays through the public path: slab part of set_fields writes work[0..7] on own z planes
+        binding.MHD.set_fields(g, cfg.prim, "primitive")
+        send, sc, rc = g.pack(dist.SLABS_TO_BRICKS, 8)
+        g.stream.synchronize()
+        # unpack into a second context of the same rank and pack again: the round trip is the identity on the blocks
+        (ya, yb), (za, zb) = g.ranges()
+        assert send.numel() == sum(sc) == 2 * 8 * (zb - za) * (nyc - (yb - ya)) * nxp       # all but the own block
+        h = dist.DistMHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, rank=rank, world=world)
+        # the receive side of BRICKS_TO_SLABS has the geometry of the send side of SLABS_TO_BRICKS
+        h.unpack(dist.BRICKS_TO_SLABS, 8, send)
+        again, _, _ = h.pack(dist.SLABS_TO_BRICKS, 8)
+        h.stream.synchronize()
+        assert torch.equal(send, again)
+        # layout: [peer][f][z][ky][kx]: compare with pack_host on a work array rebuilt from the blocks
+        work = np.zeros((8, N, nyc, nxp), dtype=np.complex128)
+        dist.unpack_host(work, send.cpu().numpy(), N, world, rank, dist.BRICKS_TO_SLABS)
+        assert np.array_equal(dist.pack_host(work, N, world, rank, dist.SLABS_TO_BRICKS), send.cpu().numpy())
+
+
+def test_decomposed_context_refuses_the_undecomposed_calls(mods):
+    binding, dist = mods
+    cfg = inputs.config1(32)
+    g = dist.DistMHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, rank=0, world=2)
+    with pytest.raises(RuntimeError):
+        g.phase(dist.PHASE_A)                       # no fields yet
+    binding.MHD.set_fields(g, cfg.prim, "primitive")
+    with pytest.raises(RuntimeError):
+        binding.MHD.step(g, 1)                      # must be driven through the phases
+    with pytest.raises(RuntimeError):
+        g.rhs()
+    with pytest.raises(RuntimeError):
+        g.diagnostics()
+    inc = binding.MHD(cfg.N)                        # an in-core context cannot be decomposed
+    rc = inc._L.mhd_dist_config(inc._h, 0, 2)
+    assert rc == -1
