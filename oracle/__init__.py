@@ -35,6 +35,7 @@ def lib():
         L.orc_get_threads.restype = C.c_int
         L.orc_use_direct_dft.argtypes = [C.c_void_p, C.c_int]
         L.orc_set_variant.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int]
+        L.orc_set_integrator.argtypes = [C.c_void_p, C.c_int]
         L.orc_set_fields.argtypes = [C.c_void_p, C.c_int, PP]
         L.orc_get_fields.argtypes = [C.c_void_p, C.c_int, PP]
         L.orc_rhs.argtypes = [C.c_void_p, PP]
@@ -140,6 +141,10 @@ class Oracle:
 
     def use_direct_dft(self, on=True):
         _check(lib().orc_use_direct_dft(self._h, int(on)))
+
+    def set_integrator(self, which):
+        """'ab2' (default), 'rk4' or 'pc' (predictor-corrector / Heun)."""
+        _check(lib().orc_set_integrator(self._h, {"ab2": 0, "rk4": 1, "pc": 2}[which]))
 
     def set_variant(self, cs2=0.0, f0=0.0, kf=1, evolve=3):
         """Equation-set variants: barotropic closure (cs2 > 0), ABC forcing (f0, kf), switched-off equations."""

@@ -415,7 +415,42 @@ public:
     // --------------------------------------------------------------------------------------------
     // O4. Adams-Bashforth 2, forward-Euler start (reading R6)
     // --------------------------------------------------------------------------------------------
+    // integrator: 0 = Adams-Bashforth 2 (above); 1 = classical Runge-Kutta 4; 2 = predictor-corrector (Heun):
+    // U* = U + dt R(U), U+ = U + dt/2 (R(U) + R(U*)) — the paper's other two time solvers (Table I)
+    int integrator = 0;
+
+    void axpy(rfield<T> (&y)[NF], const rfield<T> (&base)[NF], T a, const rfield<T> (&x)[NF]) const {   // y = base + a x
+        for (int c = 0; c < NF; ++c) {
+            y[c].resize(N3);
+            for (std::int64_t i = 0; i < N3; ++i) y[c][i] = base[c][i] + a * x[c][i];
+        }
+    }
+    void step_rk4() {
+        rfield<T> k1[NF], k2[NF], k3[NF], k4[NF], S[NF];
+        rhs(U, k1);
+        axpy(S, U, T(0.5) * dt, k1); rhs(S, k2);
+        axpy(S, U, T(0.5) * dt, k2); rhs(S, k3);
+        axpy(S, U, dt, k3);          rhs(S, k4);
+        for (int c = 0; c < NF; ++c)
+            for (std::int64_t i = 0; i < N3; ++i)
+                U[c][i] += dt * (k1[c][i] / T(6) + k2[c][i] / T(3) + k3[c][i] / T(3) + k4[c][i] / T(6));
+    }
+    void step_heun() {
+        rfield<T> r0[NF], r1[NF], S[NF];
+        rhs(U, r0);
+        axpy(S, U, dt, r0);          // predictor
+        rhs(S, r1);
+        for (int c = 0; c < NF; ++c)
+            for (std::int64_t i = 0; i < N3; ++i) U[c][i] += T(0.5) * dt * (r0[c][i] + r1[c][i]);
+    }
+
     void step(int nsteps) {
+        for (int s = 0; s < nsteps && integrator != 0; ++s) {
+            if (integrator == 1) step_rk4(); else step_heun();
+            ++nstep;
+            time = T(nstep) * dt;
+        }
+        if (integrator != 0) return;
         for (int s = 0; s < nsteps; ++s) {
             rfield<T> R[NF];
             rhs(U, R);

@@ -129,6 +129,12 @@ int orc_set_variant(orc_ctx* c, double cs2, double f0, int kf, int evolve) {
         DISPATCH(c, { S.cs2 = cs2; S.f0 = f0; S.kf = kf; S.evolve = evolve; S.have_old = false; });
     });
 }
+int orc_set_integrator(orc_ctx* c, int integrator) {
+    return guarded([&] {
+        if (integrator < 0 || integrator > 2) throw std::invalid_argument("integrator");
+        DISPATCH(c, { S.integrator = integrator; S.have_old = false; });
+    });
+}
 int orc_set_fields(orc_ctx* c, int kind, const double* const f[8]) {
     return guarded([&] { if (kind != 0 && kind != 1) throw std::invalid_argument("kind"); DISPATCH(c, S.set_fields(kind, f)); });
 }

@@ -263,6 +263,28 @@ def test_other_integrators_agree_with_ab2(orc, MHD, integ):
         assert rel_l2(c, a) <= 1e-7, NAMES[f]
 
 
+@pytest.mark.parametrize("integ,name", [(1, "rk4"), (2, "pc")])
+@pytest.mark.parametrize("cfgname,N,fused", [("2", 32, 1), ("3", 128, 1), ("3", 64, 0)])
+def test_other_integrators_match_oracle(orc, MHD, integ, name, cfgname, N, fused):
+    """RK4 and the predictor-corrector against the oracle's own RK4 / Heun (pins P15), state after several steps."""
+    from paper_1810_12707_b200 import binding as b
+    cfg = inputs.by_name(cfgname, N)
+    o = orc.Oracle(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+    o.set_integrator(name)
+    o.set_fields(cfg.prim, "primitive")
+    g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+    g.set_option(b.MHD_OPT_INTEGRATOR, integ)
+    g.set_option(b.MHD_OPT_FUSED, fused)
+    g.set_fields(cfg.prim, "primitive")
+    n = 3 if N >= 128 else 8
+    o.step(n); g.step(n)
+    Uo, Ug = o.get_fields(), g.get_fields()
+    scale = max(np.linalg.norm(x) for x in Uo)
+    for f in range(8):
+        assert np.linalg.norm(Ug[f] - Uo[f]) <= 1e-12 * scale, NAMES[f]
+    assert g.diagnostics()["step"] == n
+
+
 def test_rk4_alfven_wave_fourth_order(MHD):
     # exact nonlinear circularly polarised Alfven wave (pin P8): RK4 error falls 16x per halving of dt
     from paper_1810_12707_b200 import binding as b

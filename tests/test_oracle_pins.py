@@ -464,3 +464,50 @@ def test_long_double_oracle_agrees(orc):
     for f in range(8):
         beta = np.linalg.norm(R[f] - Rl[f]) / (kc * phi[f] + kc * kc * dsc[f] + 1e-300)
         assert beta <= 2e-15, (NAMES[f], beta)
+
+
+# ---------------------------------------------------------------------------------------------------
+# P15  the other two time solvers (Table I): RK4 and the predictor-corrector (Heun)
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("which,poly", [("rk4", (1, 1, 1 / 2, 1 / 6, 1 / 24)), ("pc", (1, 1, 1 / 2))])
+def test_p15_stability_polynomial(orc, which, poly):
+    """Tiny-amplitude resistive mode (linear ODE dB/dt = -eta k^2 B, the regime of P12): after n steps the amplitude
+    is b * p(z)^n with the scheme's stability polynomial p, z = -eta k^2 dt — fixes every stage weight."""
+    N, b, k, eta, dt, n = 16, 1e-8, 3, 0.5, 0.02, 6
+    X, Y, Z = grid(N)
+    o = make(orc, N, [1.0, 0, 0, 0, 1.0, 0, b * np.cos(k * X), 0], eta=eta, dt=dt)
+    o.set_integrator(which)
+    z = -eta * k * k * dt
+    p = sum(c * z ** j for j, c in enumerate(poly))
+    for j in range(1, n + 1):
+        o.step(1)
+        By = o.get_fields()[6]
+        amp = (np.fft.fftn(By)[0, 0, k] / N ** 3 * 2).real
+        assert abs(amp - b * p ** j) <= 1e-14 * b, (which, j)
+    assert o.diagnostics()["step"] == n
+
+
+@pytest.mark.parametrize("which,order", [("rk4", 4), ("pc", 2)])
+def test_p15_order_on_the_exact_alfven_wave(orc, which, order):
+    """Error against the exact nonlinear Alfven-wave solution (P8) falls by 2^order per halving of dt."""
+    N, r0, P0, B0, b, k, T = 16, 1.0, 1.0, 1.0, 0.1, 1, 0.4
+    errs = []
+    for dt in ((0.1, 0.05) if which == "rk4" else (0.02, 0.01)):
+        o = make(orc, N, alfven_state(N, r0, P0, B0, b, k), dt=dt)
+        o.set_integrator(which)
+        o.step(int(round(T / dt)))
+        got = o.get_fields("primitive")
+        ref = alfven_state(N, r0, P0, B0, b, k, t=T)
+        errs.append(max(maxabs(got[i] - full(N, ref[i])) for i in range(8)))
+    ratio = errs[0] / errs[1]
+    assert 0.8 * 2 ** order <= ratio <= 1.25 * 2 ** order, (which, errs)
+
+
+def test_p15_step_split_and_integrator_switch(orc):
+    c = inputs.config1(16)
+    o1 = make(orc, 16, c.prim, c.mu, c.eta, c.dt); o1.set_integrator("rk4")
+    o2 = make(orc, 16, c.prim, c.mu, c.eta, c.dt); o2.set_integrator("rk4")
+    o1.step(4)
+    o2.step(1); o2.step(3)
+    for a, b in zip(o1.get_fields(), o2.get_fields()):
+        assert np.array_equal(a, b)
