@@ -36,6 +36,7 @@ def lib():
         L.orc_use_direct_dft.argtypes = [C.c_void_p, C.c_int]
         L.orc_set_variant.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_int, C.c_int]
         L.orc_set_integrator.argtypes = [C.c_void_p, C.c_int]
+        L.orc_set_stress.argtypes = [C.c_void_p, C.c_int]
         L.orc_set_fields.argtypes = [C.c_void_p, C.c_int, PP]
         L.orc_get_fields.argtypes = [C.c_void_p, C.c_int, PP]
         L.orc_rhs.argtypes = [C.c_void_p, PP]
@@ -141,6 +142,10 @@ class Oracle:
 
     def use_direct_dft(self, on=True):
         _check(lib().orc_use_direct_dft(self._h, int(on)))
+
+    def set_stress(self, on=True):
+        """Viscous terms of PAPER.md Eq. 11-12 (div(2 nu rho S), energy flux -2 nu rho u.S) instead of mu lap u."""
+        _check(lib().orc_set_stress(self._h, int(bool(on))))
 
     def set_integrator(self, which):
         """'ab2' (default), 'rk4' or 'pc' (predictor-corrector / Heun)."""

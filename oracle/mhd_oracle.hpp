@@ -171,6 +171,8 @@ public:
     T cs2 = T(0);      // > 0: barotropic closure P = C_s^2 rho of Eq. 5 / Eq. 18 (L63, L192); E is then not evolved
     T f0 = T(0);       // amplitude of the ABC forcing rho f of Eq. 18 / L215, f = f0 (sin kz + cos ky, sin kx + cos kz, sin ky + cos kx)
     int kf = 1;        // its integer mode number k_f (k = k_f 2 pi/L)
+    int stress = 0;    // 1: the viscous terms of Eq. 11-12 (L92-96): + div(2 nu rho S) in the momentum equation and the energy
+                       //    flux -2 nu rho u.S, with S of Eq. 3-4 (L57-61) and nu = the `mu` parameter, instead of R3's mu lap u
     int evolve = 3;    // bit 0: Eq. 17-18 (+ energy) evolve; bit 1: Eq. 19 evolves ("turn off" of L199 / L205)
     bool use_direct_dft = false;   // P13: substitute the O(N^6) definition for the FFT
     bool have_fields = false;
@@ -327,8 +329,10 @@ public:
                 accum_phi(MX + c, flux);
                 for (std::int64_t i = 0; i < N3; ++i) out[i] -= dj[i];
             }
-            const rfield<T> lu = lap(u[c]);
-            for (std::int64_t i = 0; i < N3; ++i) out[i] += mu * lu[i];
+            if (!stress) {
+                const rfield<T> lu = lap(u[c]);
+                for (std::int64_t i = 0; i < N3; ++i) out[i] += mu * lu[i];
+            }
         }
 
         // Eq. 12:  dE/dt = - d_j ( (E+Pt) u_j - (u.B) B_j - eta (B x J)_j ) + mu lap (|u|^2/2)
@@ -347,8 +351,40 @@ public:
                 accum_phi(EN, flux);
                 for (std::int64_t i = 0; i < N3; ++i) out[i] -= dj[i];
             }
-            const rfield<T> lq = lap(q);
-            for (std::int64_t i = 0; i < N3; ++i) out[i] += mu * lq[i];
+            if (!stress) {
+                const rfield<T> lq = lap(q);
+                for (std::int64_t i = 0; i < N3; ++i) out[i] += mu * lq[i];
+            }
+        }
+
+        // Eq. 11-12 viscous terms (variant `stress`): S_ij = (d_i u_j + d_j u_i)/2 - delta_ij theta/3, theta = div u (Eq. 3-4);
+        // momentum + d_j (2 nu rho S_ij); energy - d_j ( -2 nu rho u_i S_ij ) = + d_j (2 nu rho u_i S_ij)
+        if (stress) {
+            rfield<T> du[3][3];                         // du[i][j] = d_i u_j
+            for (int i = 0; i < 3; ++i)
+                for (int j = 0; j < 3; ++j) du[i][j] = d(u[j], i);
+            rfield<T> V[3][3];                          // 2 nu rho S_ij
+            for (int i = 0; i < 3; ++i)
+                for (int j = 0; j < 3; ++j) V[i][j].resize(N3);
+            for (std::int64_t p = 0; p < N3; ++p) {
+                const T theta = du[0][0][p] + du[1][1][p] + du[2][2][p];
+                for (int i = 0; i < 3; ++i)
+                    for (int j = 0; j < 3; ++j) {
+                        const T Sij = T(0.5) * (du[i][j][p] + du[j][i][p]) - (i == j ? theta / T(3) : T(0));
+                        V[i][j][p] = T(2) * mu * rho[p] * Sij;
+                    }
+            }
+            for (int i = 0; i < 3; ++i)
+                for (int j = 0; j < 3; ++j) {
+                    const rfield<T> dj = d(V[i][j], j);
+                    for (std::int64_t p = 0; p < N3; ++p) R[MX + i][p] += dj[p];
+                }
+            for (int j = 0; j < 3; ++j) {
+                rfield<T> w(N3);
+                for (std::int64_t p = 0; p < N3; ++p) w[p] = u[0][p] * V[0][j][p] + u[1][p] * V[1][j][p] + u[2][p] * V[2][j][p];
+                const rfield<T> dj = d(w, j);
+                for (std::int64_t p = 0; p < N3; ++p) R[EN][p] += dj[p];
+            }
         }
 
         // Eq. 19 / 13:  dB/dt = curl~ (u x B) + eta lap B, component form of PAPER.md:L110

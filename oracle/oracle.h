@@ -31,6 +31,7 @@ int orc_use_direct_dft(orc_ctx *c, int on); /* substitute the O(N^6) DFT for the
  * equations): cs2 > 0 selects P = cs2*rho; f0, kf = forcing amplitude and integer mode; evolve bit 0 = Eq. 17-18 (+E),
  * bit 1 = Eq. 19 */
 int orc_set_variant(orc_ctx *c, double cs2, double f0, int kf, int evolve);
+int orc_set_stress(orc_ctx *c, int on);   /* 1: viscous terms of Eq. 11-12 (2 nu rho S, nu = mu) instead of mu lap u */
 int orc_set_integrator(orc_ctx *c, int integrator);   /* 0 AB2 (default), 1 RK4, 2 predictor-corrector (Heun); L25, L39 */
 int orc_set_fields(orc_ctx *c, int kind, const double *const f[8]);  /* 0 conservative, 1 primitive  */
 int orc_get_fields(orc_ctx *c, int kind, double *const out[8]);

@@ -129,6 +129,9 @@ int orc_set_variant(orc_ctx* c, double cs2, double f0, int kf, int evolve) {
         DISPATCH(c, { S.cs2 = cs2; S.f0 = f0; S.kf = kf; S.evolve = evolve; S.have_old = false; });
     });
 }
+int orc_set_stress(orc_ctx* c, int on) {
+    return guarded([&] { DISPATCH(c, { S.stress = on ? 1 : 0; S.have_old = false; }); });
+}
 int orc_set_integrator(orc_ctx* c, int integrator) {
     return guarded([&] {
         if (integrator < 0 || integrator > 2) throw std::invalid_argument("integrator");

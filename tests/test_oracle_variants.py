@@ -116,3 +116,62 @@ def test_v3_switched_off_equations():
     for c in range(5):
         assert np.array_equal(U0[c], U1[c])
     assert not np.array_equal(U0[5], U1[5])
+
+
+# ---- V4: the viscous terms of Eq. 11-12 (2 nu rho S with the traceless rate of strain of Eq. 3-4) -----------------------
+def _visc_part(N, prim, nu):
+    """R(stress form, nu) - R(nu = 0): the viscous terms alone."""
+    o = oracle.Oracle(N, L, G, nu, 0.0, 1e-3)
+    o.set_stress(True)
+    o.set_fields(prim)
+    R1 = o.rhs()
+    o0 = oracle.Oracle(N, L, G, 0.0, 0.0, 1e-3)
+    o0.set_fields(prim)
+    R0 = o0.rhs()
+    return [a - b for a, b in zip(R1, R0)]
+
+
+def test_v4_shear_and_compression_closed_forms():
+    N, k, a, rho0, nu = 16, 2, 0.3, 1.7, 0.05
+    X, _, _ = inputs.grid(N)
+    s, c = (np.broadcast_to(f(k * X), (N, N, N)) for f in (np.sin, np.cos))
+    s2, c2 = (np.broadcast_to(f(2 * k * X), (N, N, N)) for f in (np.sin, np.cos))
+    z = full(N, 0)
+    # shear u = (0, a sin kx, 0): S_xy = a k cos(kx)/2, theta = 0
+    D = _visc_part(N, [full(N, rho0), z, a * s, z, full(N, 2.0), z, z, z], nu)
+    assert np.max(np.abs(D[2] + nu * rho0 * a * k * k * s)) <= 1e-14
+    assert np.max(np.abs(D[4] - nu * rho0 * a * a * k * k * c2)) <= 1e-14
+    for f in (0, 1, 3, 5, 6, 7):
+        assert np.max(np.abs(D[f])) <= 1e-14
+    # compression u = (a sin kx, 0, 0): S_xx = theta - theta/3 = (2/3) a k cos kx  -> the factor 4/3 of the bulk part
+    D = _visc_part(N, [full(N, rho0), a * s, z, z, full(N, 2.0), z, z, z], nu)
+    assert np.max(np.abs(D[1] + (4.0 / 3.0) * nu * rho0 * a * k * k * s)) <= 1e-14
+    assert np.max(np.abs(D[4] - (4.0 / 3.0) * nu * rho0 * a * a * k * k * c2)) <= 1e-14
+    # S_yy = S_zz = -theta/3 do not act on a flow that depends on x only
+    for f in (0, 2, 3, 5, 6, 7):
+        assert np.max(np.abs(D[f])) <= 1e-14
+
+
+def test_v4_density_sits_inside_the_divergence():
+    """rho = rho0 + r cos kx, u = (0, a sin kx, 0): d_x(nu rho a k cos kx) = -nu a k^2 (rho0 sin kx + r sin 2kx)."""
+    N, k, a, rho0, r, nu = 16, 2, 0.3, 1.7, 0.4, 0.05
+    X, _, _ = inputs.grid(N)
+    s, c = (np.broadcast_to(f(k * X), (N, N, N)) for f in (np.sin, np.cos))
+    s2 = np.broadcast_to(np.sin(2 * k * X), (N, N, N))
+    z = full(N, 0)
+    D = _visc_part(N, [rho0 + r * c, z, a * s, z, full(N, 2.0), z, z, z], nu)
+    assert np.max(np.abs(D[2] + nu * a * k * k * (rho0 * s + r * s2))) <= 1e-14
+
+
+def test_v4_abc_flow_against_the_laplacian_form():
+    """Solenoidal Beltrami flow, rho = 1: div(2 nu S) = nu lap u = -nu u (as R3's form), while the work term is
+    d_j(2 nu u_i S_ij) = nu (lap q + div(u.grad u)) = 2 nu lap q, twice R3's mu lap q."""
+    N, U0, nu = 16, 0.5, 0.02
+    ux, uy, uz = inputs.abc_flow(N, U0, 1)
+    z = full(N, 0)
+    D = _visc_part(N, [full(N, 1.0), ux, uy, uz, full(N, 3.0), z, z, z], nu)
+    for cidx, u in enumerate((ux, uy, uz)):
+        assert np.max(np.abs(D[1 + cidx] + nu * u)) <= 1e-14
+    q = 0.5 * (ux * ux + uy * uy + uz * uz)
+    lap_q = -2.0 * (q - 1.5 * U0 * U0)                 # pin P4
+    assert np.max(np.abs(D[4] - 2 * nu * lap_q)) <= 1e-14
