@@ -83,6 +83,10 @@ extern "C" {
 /* Equation-set variants of the paper (readings V1-V3).  Changing one resets the integrator history. */
 #define MHD_OPT_EVOLVE 8  /* bit 0: Eq. 17-18 and the energy equation evolve, bit 1: Eq. 19 evolves (default 3).  2 = the
                              kinematic dynamo of PAPER.md L205 ("turn off Eq. 17 and 18"), 1 = hydrodynamic (L199)      */
+#define MHD_OPT_STRESS 12 /* 1: the viscous terms of PAPER.md Eq. 11-12 (L92-96): + div(2 nu rho S) in the momentum equation and
+                             the energy flux -2 nu rho u.S, with the traceless rate of strain S of Eq. 3-4 (L57-61) and nu = the
+                             `mu` of mhd_init, instead of mu lap(u) (R3).  An unfused add-on pass (22 more transforms
+                             per right-hand side); in-core contexts, Adams-Bashforth only                                  */
 #define MHD_OPT_FORCE_K 9 /* integer mode number k_f >= 1 of the ABC forcing (default 1)                               */
 /* parameters for mhd_set_param() */
 #define MHD_PARAM_CS2 1       /* C_s^2 > 0: barotropic closure P = C_s^2 rho (Eq. 5, Eq. 18): E is carried

@@ -195,6 +195,10 @@ class MHD:
         self.set_param(2, f0)
         self.set_option(8, evolve)
 
+    def set_stress(self, on=True):
+        """MHD_OPT_STRESS: viscous terms of Eq. 11-12 (2 nu rho S) instead of mu lap(u)."""
+        self.set_option(12, 1 if on else 0)
+
     def set_fields(self, fields, kind="primitive"):
         where, ptrs, keep = self._marshal(fields)
         self._check(self._L.mhd_set_fields(self._h, MHD_PRIMITIVE if kind == "primitive" else MHD_CONSERVATIVE, where, ptrs))

@@ -109,7 +109,14 @@ void launch_build_current(const SpecGeom& g, const cd* const B[3], cd* const J[3
 // mode 1: Euler update U += dt R, Rold = R; mode 2: AB2 update U += dt(1.5 R - 0.5 Rold), Rold = R
 // force (or null): 4 arrays F^_x, F^_y, F^_z, (m.f)^ added to R_m and R_E (launch_forcing below)
 void launch_assemble(const SpecGeom& g, const cd* const prod[16], cd* const U[8], cd* const Rold[8],
-                     cd* const rout[8], int mode, double dt, Phys ph, cudaStream_t st, const cd* const force[4] = nullptr);
+                     cd* const rout[8], int mode, double dt, Phys ph, cudaStream_t st, const cd* const force[4] = nullptr,
+                     const cd* const visc[9] = nullptr);   // visc: V^xx,xy,xz,yy,yz,zz, Wv^x,y,z: R_m += i k_j V^_ij, R_E += i k.Wv^
+// full stress tensor variant (Eq. 3-4, 11-12): u = m/rho in real space; S^ (xx,xy,xz,yy,yz,zz) from u^;
+// V_ij = 2 nu rho S_ij (in place over S) and Wv_j = u_i V_ij in real space
+void launch_velocity_real(long long n, const double* rho, const double* const m[3], double* const u[3], cudaStream_t st);
+void launch_strain_spec(const SpecGeom& g, const cd* const u[3], cd* const S[6], Phys ph, cudaStream_t st);
+void launch_viscous_flux(long long n, double nu, const double* rho, const double* const u[3], double* const SV[6],
+                         double* const Wv[3], cudaStream_t st);
 // ABC forcing in k-space (full layout only): F^ = M (rho f)^ and M (m.f)^ as +-kf shifts of rho^, m^ (exact: the
 // state is band-limited to the mask).  add = 0: out[0..3] = F ; add = 1: out[1..4] += F (out = an 8-field R^ array)
 void launch_forcing(const SpecGeom& g, const cd* const U[8], cd* const out[], int add, Phys ph, cudaStream_t st);

@@ -105,7 +105,9 @@ void launch_divergence(const SpecGeom& g, const cd* const B[3], cd* out, Phys ph
 // ---- R^ assembly (+ explicit update) -------------------------------------------------------------------
 // mode 0: rout = R ; 1: U += dt R, Rold = R ; 2: U += dt (1.5 R - 0.5 Rold), Rold = R
 struct PtrC4 { const cd* p[4]; };
-__global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 rout, int mode, double dt, Phys ph, PtrC4 force) {
+struct PtrC9 { const cd* p[9]; };
+__global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 rout, int mode, double dt, Phys ph, PtrC4 force,
+                                PtrC9 visc) {
     ModeIt m;
     if (!mode_of_thread(g, m)) return;
     const long long i = m.idx, j = m.sidx;     // products / state
@@ -129,6 +131,13 @@ __global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 r
         R[5] = imul(ky, ez) - imul(kz, ey) - (ph.eta * k2) * u[5];
         R[6] = imul(kz, ex) - imul(kx, ez) - (ph.eta * k2) * u[6];
         R[7] = imul(kx, ey) - imul(ky, ex) - (ph.eta * k2) * u[7];
+        if (visc.p[0]) {         // variant: + d_j (2 nu rho S_ij) and + d_j (2 nu rho u_i S_ij)  (Eq. 11-12)
+            const cd vxx = visc.p[0][j], vxy = visc.p[1][j], vxz = visc.p[2][j], vyy = visc.p[3][j], vyz = visc.p[4][j], vzz = visc.p[5][j];
+            R[1] = R[1] + (imul(kx, vxx) + imul(ky, vxy) + imul(kz, vxz));
+            R[2] = R[2] + (imul(kx, vxy) + imul(ky, vyy) + imul(kz, vyz));
+            R[3] = R[3] + (imul(kx, vxz) + imul(ky, vyz) + imul(kz, vzz));
+            R[4] = R[4] + (imul(kx, visc.p[6][j]) + imul(ky, visc.p[7][j]) + imul(kz, visc.p[8][j]));
+        }
         if (force.p[0]) {        // variants: rho f and its work m.f (launch_forcing), state geometry
 #pragma unroll
             for (int f = 0; f < 4; ++f) R[1 + f] = R[1 + f] + force.p[f][j];
@@ -155,12 +164,38 @@ __global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 r
     }
 }
 void launch_assemble(const SpecGeom& g, const cd* const prod[16], cd* const U[8], cd* const Rold[8],
-                     cd* const rout[8], int mode, double dt, Phys ph, cudaStream_t st, const cd* const force[4]) {
-    PtrC16 p; Ptr8 u, ro, rr; PtrC4 fc;
+                     cd* const rout[8], int mode, double dt, Phys ph, cudaStream_t st, const cd* const force[4],
+                     const cd* const visc[9]) {
+    PtrC16 p; Ptr8 u, ro, rr; PtrC4 fc; PtrC9 vc;
+    for (int f = 0; f < 9; ++f) vc.p[f] = visc ? visc[f] : nullptr;
     for (int f = 0; f < 4; ++f) fc.p[f] = force ? force[f] : nullptr;
     for (int f = 0; f < 16; ++f) p.p[f] = prod[f];
     for (int f = 0; f < 8; ++f) { u.p[f] = U[f]; ro.p[f] = Rold ? Rold[f] : nullptr; rr.p[f] = rout ? rout[f] : nullptr; }
-    assemble_kernel<<<mode_grid(g, KT), KT, 0, st>>>(g, p, u, ro, rr, mode, dt, ph, fc);
+    assemble_kernel<<<mode_grid(g, KT), KT, 0, st>>>(g, p, u, ro, rr, mode, dt, ph, fc, vc);
+}
+
+// ---- full stress tensor variant (Eq. 3-4, 11-12) -------------------------------------------------------
+struct PtrW6 { cd* p[6]; };
+// S^_ij = i (k_i u^_j + k_j u^_i)/2 - delta_ij i k.u^/3 on the masked modes; slot order xx, xy, xz, yy, yz, zz
+__global__ void strain_spec_kernel(SpecGeom g, Ptr3 u, PtrW6 S, Phys ph) {
+    ModeIt m;
+    if (!mode_of_thread(g, m) || !m.inside) return;
+    const double kx = ph.k0 * m.nx, ky = ph.k0 * m.ny, kz = ph.k0 * m.nz;
+    const cd ux = u.p[0][m.idx], uy = u.p[1][m.idx], uz = u.p[2][m.idx];
+    const cd dxx = imul(kx, ux), dyy = imul(ky, uy), dzz = imul(kz, uz);
+    const cd th3 = (1.0 / 3.0) * (dxx + dyy + dzz);
+    S.p[0][m.idx] = dxx - th3;
+    S.p[1][m.idx] = 0.5 * (imul(kx, uy) + imul(ky, ux));
+    S.p[2][m.idx] = 0.5 * (imul(kx, uz) + imul(kz, ux));
+    S.p[3][m.idx] = dyy - th3;
+    S.p[4][m.idx] = 0.5 * (imul(ky, uz) + imul(kz, uy));
+    S.p[5][m.idx] = dzz - th3;
+}
+void launch_strain_spec(const SpecGeom& g, const cd* const u[3], cd* const S[6], Phys ph, cudaStream_t st) {
+    Ptr3 uu; PtrW6 ss;
+    for (int c = 0; c < 3; ++c) uu.p[c] = u[c];
+    for (int c = 0; c < 6; ++c) ss.p[c] = S[c];
+    strain_spec_kernel<<<mode_grid(g, KT), KT, 0, st>>>(g, uu, ss, ph);
 }
 
 // ---- ABC forcing in k-space ------------------------------------------------------------------------------
@@ -275,6 +310,40 @@ void launch_flux_real(long long n, const double* const in[11], double* const out
     for (int f = 0; f < 11; ++f) a.p[f] = in[f];
     for (int f = 0; f < 16; ++f) b.p[f] = out[f];
     flux_real_kernel<<<ew_blocks(n, 256), 256, 0, st>>>(n, a, b, ph);
+}
+
+struct PtrRC3 { const double* p[3]; };
+struct PtrRW6 { double* p[6]; };
+__global__ void velocity_real_kernel(long long n, const double* rho, PtrRC3 m, PtrRW3 u) {
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const double r = rho[i];
+        u.p[0][i] = m.p[0][i] / r; u.p[1][i] = m.p[1][i] / r; u.p[2][i] = m.p[2][i] / r;
+    }
+}
+void launch_velocity_real(long long n, const double* rho, const double* const m[3], double* const u[3], cudaStream_t st) {
+    PtrRC3 mm; PtrRW3 uu;
+    for (int c = 0; c < 3; ++c) { mm.p[c] = m[c]; uu.p[c] = u[c]; }
+    velocity_real_kernel<<<ew_blocks(n, 256), 256, 0, st>>>(n, rho, mm, uu);
+}
+// V_ij = 2 nu rho S_ij in place; Wv_j = u_i V_ij
+__global__ void viscous_flux_kernel(long long n, double nu, const double* rho, PtrRC3 u, PtrRW6 SV, PtrRW3 Wv) {
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const double f = 2.0 * nu * rho[i];
+        const double vxx = f * SV.p[0][i], vxy = f * SV.p[1][i], vxz = f * SV.p[2][i];
+        const double vyy = f * SV.p[3][i], vyz = f * SV.p[4][i], vzz = f * SV.p[5][i];
+        const double ux = u.p[0][i], uy = u.p[1][i], uz = u.p[2][i];
+        SV.p[0][i] = vxx; SV.p[1][i] = vxy; SV.p[2][i] = vxz; SV.p[3][i] = vyy; SV.p[4][i] = vyz; SV.p[5][i] = vzz;
+        Wv.p[0][i] = ux * vxx + uy * vxy + uz * vxz;
+        Wv.p[1][i] = ux * vxy + uy * vyy + uz * vyz;
+        Wv.p[2][i] = ux * vxz + uy * vyz + uz * vzz;
+    }
+}
+void launch_viscous_flux(long long n, double nu, const double* rho, const double* const u[3], double* const SV[6],
+                         double* const Wv[3], cudaStream_t st) {
+    PtrRC3 uu; PtrRW6 ss; PtrRW3 ww;
+    for (int c = 0; c < 3; ++c) { uu.p[c] = u[c]; ww.p[c] = Wv[c]; }
+    for (int c = 0; c < 6; ++c) ss.p[c] = SV[c];
+    viscous_flux_kernel<<<ew_blocks(n, 256), 256, 0, st>>>(n, nu, rho, uu, ss, ww);
 }
 
 __global__ void prim_to_cons_kernel(long long n, PtrR8 f, double gamma) {

@@ -169,23 +169,61 @@ void products(mhd_ctx* c, cd* const Uin[8], double* const breal[3] = nullptr) {
     strided_pass(c, -1, 2, 16, c->W, c->W, c->hx(), c->hx(), prune);      // S5a
 }
 
+// Variant MHD_OPT_STRESS (Eq. 3-4, 11-12): V_ij = 2 nu rho S_ij and Wv_j = u_i V_ij, transformed, for the assembly.
+// An unfused add-on pass (22 extra 3-D transforms): Uin -> real rho, m -> u = m/rho -> u^ -> S^ -> real S -> V, Wv -> V^, Wv^.
+// Buffers: X[0..3] real rho, m; X[4..6] real u; u^ in Y[6], Y[7], X[7]; S / V in Y[0..5]; Wv over u^.
+void viscous_pass(mhd_ctx* c, cd* const Uin[8]) {
+    const long long n3 = c->n3();
+    SpecGeom gp = c->geom(); gp.pruned = 1;
+    const cd* spec4[4] = {Uin[0], Uin[1], Uin[2], Uin[3]};
+    cd* work4[4] = {c->X[0], c->X[1], c->X[2], c->X[3]};
+    double* real4[4];
+    for (int f = 0; f < 4; ++f) real4[f] = reinterpret_cast<double*>(c->X[f]);
+    inverse3d(c, 4, spec4, work4, real4, true);
+    double* u[3] = {reinterpret_cast<double*>(c->X[4]), reinterpret_cast<double*>(c->X[5]), reinterpret_cast<double*>(c->X[6])};
+    const double* m[3] = {real4[1], real4[2], real4[3]};
+    { mhd_ctx::Scope s(c, F_POINT); launch_velocity_real(n3, real4[0], m, u, c->st); }
+    const double* uc[3] = {u[0], u[1], u[2]};
+    cd* uhat[3] = {c->Y[6], c->Y[7], c->X[7]};
+    forward3d(c, 3, uc, uhat, nullptr, true);
+    const cd* uhc[3] = {uhat[0], uhat[1], uhat[2]};
+    cd* S[6] = {c->Y[0], c->Y[1], c->Y[2], c->Y[3], c->Y[4], c->Y[5]};
+    { mhd_ctx::Scope s(c, F_POINT); launch_strain_spec(gp, uhc, S, c->phys(), c->st); }
+    const cd* Sc[6]; double* Sr[6];
+    for (int f = 0; f < 6; ++f) { Sc[f] = S[f]; Sr[f] = reinterpret_cast<double*>(S[f]); }
+    inverse3d(c, 6, Sc, S, Sr, true);
+    double* Wv[3] = {reinterpret_cast<double*>(uhat[0]), reinterpret_cast<double*>(uhat[1]), reinterpret_cast<double*>(uhat[2])};
+    { mhd_ctx::Scope s(c, F_POINT); launch_viscous_flux(n3, c->mu, real4[0], uc, Sr, Wv, c->st); }
+    const double* r9[9]; cd* s9[9];
+    for (int f = 0; f < 6; ++f) { r9[f] = Sr[f]; s9[f] = S[f]; }
+    for (int f = 0; f < 3; ++f) { r9[6 + f] = Wv[f]; s9[6 + f] = uhat[f]; }
+    forward3d(c, 9, r9, s9, nullptr, true);
+}
+
 // R^(Uin) -> rout (mode 0) or explicit update of Uin / Rold (mode 1 Euler, 2 AB2)
 void rhs_spectral(mhd_ctx* c, cd* const Uin[8], cd* const rout[8], int mode, double* const breal[3] = nullptr) {
+    const bool stress = c->opt_stress != 0;
+    const cd* visc[9] = {c->Y[0], c->Y[1], c->Y[2], c->Y[3], c->Y[4], c->Y[5], c->Y[6], c->Y[7], c->X[7]};
+    if (stress) viscous_pass(c, Uin);                 // V^_ij, Wv^_j -> Y[0..7], X[7]   (before the products: uses X, Y)
     products(c, Uin, breal);
     const bool forced = c->f0 != 0.0;
     SpecGeom gp = c->geom(); gp.pruned = 1;
     const cd* Uc[8];
     for (int f = 0; f < 8; ++f) Uc[f] = Uin[f];
-    const cd* force[4] = {c->Y[0], c->Y[1], c->Y[2], c->Y[3]};
+    cd* fbuf[4] = {c->X[3], c->X[4], c->X[5], c->X[6]};           // X[0..2] may hold the tracers' real-space B
+    const cd* force[4] = {fbuf[0], fbuf[1], fbuf[2], fbuf[3]};
     if (forced && mode != 0) {      // the update is in place: the +-k_f neighbours of U^ must be read before it starts
         mhd_ctx::Scope s(c, F_POINT);
-        launch_forcing(gp, Uc, c->Y, 0, c->phys(), c->st);
+        launch_forcing(gp, Uc, fbuf, 0, c->phys(), c->st);
     }
     {
+        Phys ph = c->phys();
+        if (stress) ph.mu = 0.0;                      // the viscous terms come from `visc`, not from mu k^2 u^
         mhd_ctx::Scope s(c, F_ASSEMBLE);
-        launch_assemble(c->geom(), c->W, Uin, c->Rold, rout, mode, c->dt, c->phys(), c->st, (forced && mode != 0) ? force : nullptr);
+        launch_assemble(c->geom(), c->W, Uin, c->Rold, rout, mode, c->dt, ph, c->st, (forced && mode != 0) ? force : nullptr,
+                        stress ? visc : nullptr);
     }
-    if (forced && mode == 0) {      // U^ is not modified: add F^ to the assembled R^ (Y may hold integrator stages)
+    if (forced && mode == 0) {      // U^ is not modified: add F^ to the assembled R^ (X, Y may hold integrator stages)
         mhd_ctx::Scope s(c, F_POINT);
         launch_forcing(gp, Uc, rout, 1, c->phys(), c->st);
     }
@@ -347,6 +385,9 @@ int mhd_set_option(mhd_ctx* c, int option, int value) {
         case MHD_OPT_TRACER_SORT:
             if (value < 0) return c->fail(MHD_ERR_INVALID_ARG, "tracer sort interval must be >= 0");
             c->opt_tracer_sort = value; return MHD_OK;
+        case MHD_OPT_STRESS:
+            if (value != 0 && c->ooc.on) return c->fail(MHD_ERR_INVALID_ARG, "the stress-tensor variant needs an in-core context");
+            c->opt_stress = value ? 1 : 0; c->have_old = false; return MHD_OK;
         case MHD_OPT_EVOLVE:
             if (value < 0 || value > 3) return c->fail(MHD_ERR_INVALID_ARG, "evolve must be 0..3");
             c->evolve = value; c->have_old = false; return MHD_OK;
@@ -434,6 +475,7 @@ int mhd_step(mhd_ctx* c, int nsteps) {
     if (c->ooc.on) return ooc_step(c, nsteps);
     const SpecGeom g = c->geom();
     SpecGeom gp = g; gp.pruned = 1;
+    if (c->opt_stress && c->integrator != 0) return c->fail(MHD_ERR_INVALID_ARG, "the stress-tensor variant is implemented for Adams-Bashforth only");
     const bool tracers = tracers_active(c), emit = tracers && tracers_fused_emit(c);
     double* Breal[3] = {reinterpret_cast<double*>(c->X[0]), reinterpret_cast<double*>(c->X[1]), reinterpret_cast<double*>(c->X[2])};
     for (int s = 0; s < nsteps; ++s) {

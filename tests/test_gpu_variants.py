@@ -141,3 +141,63 @@ def test_variant_change_resets_the_history(orc, MHD):
     o.set_variant(f0=0.3, kf=2); g.set_variant(f0=0.3, kf=2)
     o.step(3); g.step(3)
     check_state(o, g)
+
+
+# ---- MHD_OPT_STRESS: the viscous terms of Eq. 11-12 --------------------------------------------------------------------
+def pair_stress(orc, MHD, N, mu=0.02, eta=0.01, dt=1e-3, opts=None, variant=None):
+    st = inputs.random_smooth_state(N, 9)
+    o = orc.Oracle(N, 2 * math.pi, 5.0 / 3.0, mu, eta, dt)
+    o.set_stress(True)
+    if variant:
+        o.set_variant(**variant)
+    o.set_fields(st, "primitive")
+    g = MHD(N, 2 * math.pi, 5.0 / 3.0, mu, eta, dt)
+    for k, v in (opts or {}).items():
+        g.set_option(k, v)
+    g.set_stress(True)
+    if variant:
+        g.set_variant(**variant)
+    g.set_fields(st, "primitive")
+    return o, g
+
+
+@pytest.mark.parametrize("N,opts", [(32, None), (128, None), (64, {1: 0}), (128, {1: 2})])
+def test_stress_tensor_variant(orc, MHD, N, opts):
+    """Non-uniform density, compressive + solenoidal velocity: RHS (backward error; the viscous flux 2 nu rho S has one
+    more derivative than the Laplacian form, covered by the k_c^2 d_f term) and the state after a few AB2 steps."""
+    o, g = pair_stress(orc, MHD, N, opts=opts)
+    check_rhs(o, g, N)
+    n = 3 if N >= 128 else 10
+    o.step(n); g.step(n)
+    check_state(o, g)
+    check_rhs(o, g, N)
+
+
+def test_stress_tensor_with_forcing_and_tracers(orc, MHD):
+    """The add-on pass shares the X / Y buffers with the forcing pre-pass and the tracers' real-space B: all three at once."""
+    N = 32
+    o, g = pair_stress(orc, MHD, N, variant=dict(f0=0.4, kf=2))
+    rng = np.random.default_rng(1)
+    pos = [rng.uniform(0, 2 * math.pi, 500) for _ in range(3)]
+    vel = [rng.standard_normal(500) for _ in range(3)]
+    o.tracers_set(pos, vel); g.tracers_set(pos, vel)
+    check_rhs(o, g, N, 0.4)
+    o.step(6); g.step(6)
+    check_state(o, g)
+    (po, vo), (pg, vg) = o.tracers_get(), g.tracers_get()
+    for c in range(3):
+        d = np.abs(pg[c] - po[c]); d = np.minimum(d, 2 * math.pi - d)
+        assert np.max(d) <= 1e-12 and np.max(np.abs(vg[c] - vo[c])) <= 1e-12
+
+
+def test_stress_tensor_restrictions(MHD):
+    from paper_1810_12707_b200 import binding as B
+    g = MHD(32)
+    g.set_stress(True)
+    g.set_option(3, 1)
+    g.set_fields(inputs.random_smooth_state(32, 1), "primitive")
+    with pytest.raises(RuntimeError):
+        g.step(1)                                  # Adams-Bashforth only
+    ooc = MHD(32, flags=B.MHD_FLAG_OUT_OF_CORE)
+    with pytest.raises(RuntimeError):
+        ooc.set_stress(True)
