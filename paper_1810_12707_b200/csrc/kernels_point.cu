@@ -56,7 +56,12 @@ static dim3 mode_grid(const SpecGeom& g, int threads) {
     const int nyv = g.pruned ? 2 * g.kc + 1 : g.N;
     return dim3((nxv + threads - 1) / threads, nyv, nyv);
 }
-constexpr int KT = 64;   // threads along kx for the k-space kernels
+// threads along kx for the point-wise k-space kernels: 64, or 32 when that wastes fewer lanes on the last block of a row
+// (N = 256: kc + 1 = 86 columns -> 3 x 32 instead of 2 x 64: 90 % instead of 67 % of the lanes carry a mode)
+static int kt_for(const SpecGeom& g) {
+    const int nxv = (g.compact || g.pruned) ? g.kc + 1 : g.hx;
+    return ((nxv + 31) / 32) * 32 < ((nxv + 63) / 64) * 64 ? 32 : 64;
+}
 
 struct Ptr3 { const cd* p[3]; };
 struct PtrW3 { cd* p[3]; };
@@ -82,7 +87,7 @@ __global__ void build_current_kernel(SpecGeom g, Ptr3 B, PtrW3 J, Phys ph) {
 void launch_build_current(const SpecGeom& g, const cd* const B[3], cd* const J[3], Phys ph, cudaStream_t st) {
     Ptr3 b; PtrW3 j;
     for (int c = 0; c < 3; ++c) { b.p[c] = B[c]; j.p[c] = J[c]; }
-    build_current_kernel<<<mode_grid(g, KT), KT, 0, st>>>(g, b, j, ph);
+    build_current_kernel<<<mode_grid(g, kt_for(g)), kt_for(g), 0, st>>>(g, b, j, ph);
 }
 
 // ---- div^ = M i k . B^ ---------------------------------------------------------------------------------
@@ -99,13 +104,16 @@ __global__ void divergence_kernel(SpecGeom g, Ptr3 B, cd* out, Phys ph) {
 void launch_divergence(const SpecGeom& g, const cd* const B[3], cd* out, Phys ph, cudaStream_t st) {
     Ptr3 b;
     for (int c = 0; c < 3; ++c) b.p[c] = B[c];
-    divergence_kernel<<<mode_grid(g, KT), KT, 0, st>>>(g, b, out, ph);
+    divergence_kernel<<<mode_grid(g, kt_for(g)), kt_for(g), 0, st>>>(g, b, out, ph);
 }
 
 // ---- R^ assembly (+ explicit update) -------------------------------------------------------------------
 // mode 0: rout = R ; 1: U += dt R, Rold = R ; 2: U += dt (1.5 R - 0.5 Rold), Rold = R
 struct PtrC4 { const cd* p[4]; };
 struct PtrC9 { const cd* p[9]; };
+// VAR = false: the default equation set (no forcing, no stress-tensor terms, nothing switched off) — the hot path keeps
+// its register budget; VAR = true: all variants of DESIGN.md section 13
+template <bool VAR>
 __global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 rout, int mode, double dt, Phys ph, PtrC4 force,
                                 PtrC9 visc) {
     ModeIt m;
@@ -131,6 +139,7 @@ __global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 r
         R[5] = imul(ky, ez) - imul(kz, ey) - (ph.eta * k2) * u[5];
         R[6] = imul(kz, ex) - imul(kx, ez) - (ph.eta * k2) * u[6];
         R[7] = imul(kx, ey) - imul(ky, ex) - (ph.eta * k2) * u[7];
+        if constexpr (VAR) {
         if (visc.p[0]) {         // variant: + d_j (2 nu rho S_ij) and + d_j (2 nu rho u_i S_ij)  (Eq. 11-12)
             const cd vxx = visc.p[0][j], vxy = visc.p[1][j], vxz = visc.p[2][j], vyy = visc.p[3][j], vyz = visc.p[4][j], vzz = visc.p[5][j];
             R[1] = R[1] + (imul(kx, vxx) + imul(ky, vxy) + imul(kz, vxz));
@@ -145,6 +154,7 @@ __global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 r
         if (ph.cs2 > 0.0) R[4] = mk(0, 0);                      // barotropic: no energy equation
         if (!(ph.evolve & 1)) { R[0] = R[1] = R[2] = R[3] = R[4] = mk(0, 0); }
         if (!(ph.evolve & 2)) { R[5] = R[6] = R[7] = mk(0, 0); }
+        }
         if (mode == 0) {
 #pragma unroll
             for (int f = 0; f < 8; ++f) rout.p[f][i] = R[f];     // work-array geometry (may alias the products)
@@ -171,7 +181,9 @@ void launch_assemble(const SpecGeom& g, const cd* const prod[16], cd* const U[8]
     for (int f = 0; f < 4; ++f) fc.p[f] = force ? force[f] : nullptr;
     for (int f = 0; f < 16; ++f) p.p[f] = prod[f];
     for (int f = 0; f < 8; ++f) { u.p[f] = U[f]; ro.p[f] = Rold ? Rold[f] : nullptr; rr.p[f] = rout ? rout[f] : nullptr; }
-    assemble_kernel<<<mode_grid(g, KT), KT, 0, st>>>(g, p, u, ro, rr, mode, dt, ph, fc, vc);
+    const bool var = force || visc || ph.cs2 > 0.0 || ph.evolve != 3;
+    if (var) assemble_kernel<true><<<mode_grid(g, kt_for(g)), kt_for(g), 0, st>>>(g, p, u, ro, rr, mode, dt, ph, fc, vc);
+    else assemble_kernel<false><<<mode_grid(g, kt_for(g)), kt_for(g), 0, st>>>(g, p, u, ro, rr, mode, dt, ph, fc, vc);
 }
 
 // ---- full stress tensor variant (Eq. 3-4, 11-12) -------------------------------------------------------
@@ -195,7 +207,7 @@ void launch_strain_spec(const SpecGeom& g, const cd* const u[3], cd* const S[6],
     Ptr3 uu; PtrW6 ss;
     for (int c = 0; c < 3; ++c) uu.p[c] = u[c];
     for (int c = 0; c < 6; ++c) ss.p[c] = S[c];
-    strain_spec_kernel<<<mode_grid(g, KT), KT, 0, st>>>(g, uu, ss, ph);
+    strain_spec_kernel<<<mode_grid(g, kt_for(g)), kt_for(g), 0, st>>>(g, uu, ss, ph);
 }
 
 // ---- ABC forcing in k-space ------------------------------------------------------------------------------
@@ -247,7 +259,7 @@ void launch_forcing(const SpecGeom& g, const cd* const U[8], cd* const out[], in
     Ptr8 u, o;
     for (int f = 0; f < 8; ++f) { u.p[f] = const_cast<cd*>(U[f]); o.p[f] = nullptr; }
     for (int f = 0; f < (add ? 8 : 4); ++f) o.p[f] = out[f];
-    forcing_kernel<<<mode_grid(g, KT), KT, 0, st>>>(g, u, o, add, ph);
+    forcing_kernel<<<mode_grid(g, kt_for(g)), kt_for(g), 0, st>>>(g, u, o, add, ph);
 }
 
 // ---- y = a y + b x on the masked modes (integrator stages) -----------------------------------------------
@@ -264,7 +276,7 @@ __global__ void axpby_kernel(SpecGeom g, int nf, double a, PtrN y, double b, Ptr
 void launch_axpby(const SpecGeom& g, int nf, double a, cd* const y[], double b, const cd* const x[], cudaStream_t st) {
     PtrN yy; PtrCN xx;
     for (int f = 0; f < nf; ++f) { yy.p[f] = y[f]; xx.p[f] = x[f]; }
-    axpby_kernel<<<mode_grid(g, KT), KT, 0, st>>>(g, nf, a, yy, b, xx);
+    axpby_kernel<<<mode_grid(g, kt_for(g)), kt_for(g), 0, st>>>(g, nf, a, yy, b, xx);
 }
 void launch_copy_masked(const SpecGeom& g, int nf, cd* const dst[], const cd* const src[], cudaStream_t st) {
     launch_axpby(g, nf, 0.0, dst, 1.0, src, st);
@@ -280,7 +292,7 @@ void launch_zero_outside_mask(const SpecGeom& g0, int nf, cd* const f[], cudaStr
     SpecGeom g = g0; g.pruned = 0;
     PtrN p;
     for (int c = 0; c < nf; ++c) p.p[c] = f[c];
-    zero_outside_kernel<<<mode_grid(g, KT), KT, 0, st>>>(g, nf, p);
+    zero_outside_kernel<<<mode_grid(g, kt_for(g)), kt_for(g), 0, st>>>(g, nf, p);
 }
 
 // ---- real-space point-wise kernels -----------------------------------------------------------------------
