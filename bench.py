@@ -321,6 +321,8 @@ def run_ours(args):
         from paper_1810_12707_b200.dist import DistMHD
         flags = B.MHD_FLAG_OUT_OF_CORE
         g = DistMHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, rank=rank, world=world, device="cuda:%d" % local_rank)
+        if world > 1 and not args.packed_exchange:
+            g.connect_peers_ipc()        # rows go straight into the owners' workspaces (P2P stores); barriers instead of all-to-alls
         args.no_e2e = args.no_fft = True
     else:
         g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, device="cuda:%d" % local_rank, flags=flags)
@@ -367,7 +369,8 @@ def run_ours(args):
     clocks = sampler.stop()
     if args.decompose:
         ooc["decomposed"] = {"world": world, "sent_to_peers_bytes_per_step_per_rank": (e1 - e0) / K,
-                             "collective": "torch.distributed.all_to_all_single (NCCL), 2 per step: 11 and 16 work fields"}
+                             "exchange": "direct P2P stores from the z-pass / forward-y kernels + 2 barriers per step" if g.direct else
+                                         "packed: torch.distributed.all_to_all_single (NCCL), 2 per step: 11 and 16 work fields"}
     ms_max, units = aggregate(ms, float(N) ** 3 * K / (world if args.decompose else 1), dist)
     value = units / (ms_max * 1e-3)
 
@@ -484,6 +487,8 @@ def main():
     ap.add_argument("--decompose", action="store_true",
                     help="with --gpus N under torchrun: ONE problem decomposed over the N GPUs (ky bricks / z slabs, two NCCL "
                          "all-to-alls per step) instead of N replicas; with N = 1 it measures the pack / unpack overhead")
+    ap.add_argument("--packed-exchange", action="store_true",
+                    help="--decompose: pack -> NCCL all_to_all_single -> unpack instead of direct peer stores")
     ap.add_argument("--tracers", type=int, default=0, metavar="NP",
                     help="also measure NP tracer particles (PAPER.md Sec. VI): frozen-field pushes/s and the step overhead")
     ap.add_argument("--option", action="append", default=[], metavar="ID=VALUE",

@@ -209,6 +209,13 @@ int mhd_dist_counts(mhd_ctx *ctx, int dir, int nfields, long long *send_counts, 
 int mhd_dist_pack(mhd_ctx *ctx, int dir, int nfields, double *dev_sendbuf);
 int mhd_dist_unpack(mhd_ctx *ctx, int dir, int nfields, const double *dev_recvbuf);
 int mhd_dist_ranges(mhd_ctx *ctx, int rank, int *ky_lo, int *ky_hi, int *z_lo, int *z_hi);   /* shares of any rank */
+/* Direct exchange (at most 8 ranks): delta_bytes[s] = address of rank s's workspace MINUS this rank's, as mapped into THIS
+ * process (CUDA IPC / peer access over NVLink; all ranks bind workspaces of the same size).  Phases A, B, C then store every
+ * output row straight into the work arrays of the rank that owns it (P2P stores from inside the z-pass and forward-y
+ * kernels, overlapping the transform tile by tile): the step needs no pack, collective or unpack, only a barrier where an
+ * exchange would be (after A, after B): [A] barrier B barrier C(next).  NULL switches back to the packed exchange.
+ * mhd_set_fields / mhd_get_fields keep using the packed exchange. */
+int mhd_dist_peers(mhd_ctx *ctx, const long long *delta_bytes);
 
 /* Bytes the chunked pipeline has copied host->device / device->host so far (0 for an in-core context). */
 int mhd_transfer_bytes(const mhd_ctx *ctx, long long *h2d, long long *d2h);

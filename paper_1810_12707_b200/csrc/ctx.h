@@ -81,6 +81,10 @@ struct mhd_ctx {
         // range [ky_lo(rank), ky_lo(rank+1)) for the brick stages and the z planes [z_lo(rank), z_lo(rank+1)) for the slab
         // stage; the exchange between them is done by the caller (all-to-all) on packed buffers
         int rank = 0, world = 1;
+        // direct exchange: peer_delta[s] = (rank s's workspace base) - (this rank's), in complex elements; the z passes and
+        // the forward y pass then store every row straight into its owner's work arrays (no pack / collective / unpack)
+        bool direct = false, direct_active = false;
+        long long peer_delta[8] = {0, 0, 0, 0, 0, 0, 0, 0};
         int ky_lo(int r) const { return (int)((long long)nyc * r / world); }
         int z_lo(int r, int N) const { return (int)((long long)N * r / world); }
     } ooc;
@@ -161,3 +165,4 @@ int ooc_dist_config(mhd_ctx* c, int rank, int world);
 int ooc_dist_phase(mhd_ctx* c, int phase, int arg);
 int ooc_dist_counts(mhd_ctx* c, int dir, int nf, long long* send, long long* recv);
 int ooc_dist_pack(mhd_ctx* c, int dir, int nf, double* buf, int unpack);
+int ooc_dist_peers(mhd_ctx* c, const long long* delta_bytes);

@@ -46,6 +46,12 @@ struct StridedArgs {
     // Fused current (sweep S1): fields f >= jfirst are not read from in[f]; they are built on load as
     // J^_c = M (i k x B^)_c from in[bfirst .. bfirst+2] (rows = kz, outer = ky, columns = kx).  jfirst < 0: off.
     int jfirst, bfirst;
+    // Multi-GPU slab decomposition (general views only): output rows are owned by different ranks; row sr (stored index)
+    // belongs to peer p with peer_lo[p] <= sr < peer_lo[p+1] and is written at out + peer_delta[p] (complex elements):
+    // the same location inside that peer's workspace, reached through a peer mapping (NVLink P2P stores).  npeer = 0: off.
+    int npeer;
+    int peer_lo[9];
+    long long peer_delta[8];
     int outer_compact;     // 1: outer index (+ outer_base) is a compact ky index; 0: a full array index
     int outer_base;
     double k0;             // 2 pi / L

@@ -91,7 +91,15 @@ strided_kernel(const __grid_constant__ StridedArgs a) {
 #pragma unroll
         for (int m = 0; m < E; ++m) {
             const int sr = stored_row<N>(t + T * m, a.out_rows, kc);
-            if (valid && sr >= 0) out[(long long)sr * a.out_row_stride] = v[m];
+            if (valid && sr >= 0) {
+                long long d = 0;
+                if (a.npeer > 0) {              // the row's owner: a peer's workspace (P2P store) or this one
+                    int p = 0;
+                    while (p + 1 < a.npeer && sr >= a.peer_lo[p + 1]) ++p;
+                    d = a.peer_delta[p];
+                }
+                out[(long long)sr * a.out_row_stride + d] = v[m];
+            }
         }
     } else {
         cd* __restrict__ out = a.out[f] + (long long)o * a.in_outer_stride + col;

@@ -731,6 +731,10 @@ int mhd_dist_unpack(mhd_ctx* c, int dir, int nf, const double* buf) {
     if (!c || !c->bound || !c->ooc.on) return MHD_ERR_INVALID_ARG;
     return ooc_dist_pack(c, dir, nf, const_cast<double*>(buf), 1);
 }
+int mhd_dist_peers(mhd_ctx* c, const long long* delta_bytes) {
+    if (!c || !c->bound || !c->ooc.on) return MHD_ERR_INVALID_ARG;
+    return ooc_dist_peers(c, delta_bytes);
+}
 int mhd_dist_ranges(mhd_ctx* c, int rank, int* ky_lo, int* ky_hi, int* z_lo, int* z_hi) {
     if (!c || !c->bound || !c->ooc.on || rank < 0 || rank >= c->ooc.world) return MHD_ERR_INVALID_ARG;
     if (ky_lo) *ky_lo = c->ooc.ky_lo(rank);

@@ -174,8 +174,11 @@ std::vector<std::pair<int, int>> slab_chunks(const mhd_ctx* c) {
 }
 
 // general strided pass (kernels_strided.cu, GEN = true): nf fields, rows = the transformed axis, `n_outer` outer indices
+// peer_rows (direct exchange of a decomposed context, only while o.direct_active): 1 = the output rows are z planes,
+// 2 = compact ky rows; each row is then stored into its owner's workspace
 void gen_pass(mhd_ctx* c, int dir, int nf, const cd* const in[], cd* const out[], long long irs, long long ios, int in_rows,
-              long long ors, long long oos, int out_rows, int n_outer, int jfirst = -1, int bfirst = 0, int outer_base = 0) {
+              long long ors, long long oos, int out_rows, int n_outer, int jfirst = -1, int bfirst = 0, int outer_base = 0,
+              int peer_rows = 0) {
     StridedArgs a;
     std::memset(&a, 0, sizeof(a));
     for (int f = 0; f < nf; ++f) { a.in[f] = in[f]; a.out[f] = out[f]; }
@@ -187,6 +190,12 @@ void gen_pass(mhd_ctx* c, int dir, int nf, const cd* const in[], cd* const out[]
     const int C = c->N >= 1024 ? 4 : 8;
     a.nchunks = (a.ncols + C - 1) / C;
     a.jfirst = jfirst; a.bfirst = bfirst; a.outer_compact = 1; a.outer_base = outer_base; a.k0 = 2.0 * M_PI / c->L;
+    const Ooc& o = c->ooc;
+    if (peer_rows && o.direct_active && o.world > 1) {
+        a.npeer = o.world;
+        for (int s = 0; s <= o.world; ++s) a.peer_lo[s] = peer_rows == 1 ? o.z_lo(s, c->N) : o.ky_lo(s);
+        for (int s = 0; s < o.world; ++s) a.peer_delta[s] = o.peer_delta[s];
+    }
     mhd_ctx::Scope s(c, dir > 0 ? F_STRIDED_INV : F_STRIDED_FWD);
     launch_strided(c->N, dir, a, c->st);
 }
@@ -260,7 +269,7 @@ int stage_inverse_z(mhd_ctx* c, cd* const src[8], bool current) {
         if (o.state_host) chunk_h2d_done(c, ch);
         const cd* in[11];
         for (int f = 0; f < 11; ++f) in[f] = u.p[f < 8 ? f : 5];
-        gen_pass(c, +1, nf, in, w.p, u.rs, o.nxp, 2, w.rs, o.nxp, 0, ny, current ? 8 : -1, 5, y0);
+        gen_pass(c, +1, nf, in, w.p, u.rs, o.nxp, 2, w.rs, o.nxp, 0, ny, current ? 8 : -1, 5, y0, 1);
         chunk_comp_done(c, ch, o.work_host);
         if (o.work_host) { work_store(c, w, nf, y0); chunk_d2h_done(c, ch); }
     }
@@ -346,7 +355,7 @@ int stage_slabs(mhd_ctx* c, SlabKind kind, const SlabIO& io) {
             launch_x_r2c(N, a, c->st);
         }
         if (io.nout > 0)     // forward y pass: all N rows -> the compact ky rows of the slab
-            gen_pass(c, -1, io.nout, sb, out, hx, (long long)N * hx, 0, o.nxp, (long long)plane_c, 2, zc);
+            gen_pass(c, -1, io.nout, sb, out, hx, (long long)N * hx, 0, o.nxp, (long long)plane_c, 2, zc, -1, 0, 0, 2);
         chunk_comp_done(c, ch, out_copy);
         if (out_copy) {
             if (io.nout > 0 && o.work_host)
@@ -388,7 +397,7 @@ int stage_forward_z_assemble(mhd_ctx* c, int mode, bool next_inverse) {
         if (mode != 0 && next_inverse) {
             const cd* in[11];
             for (int f = 0; f < 11; ++f) in[f] = u.p[f < 8 ? f : 5];
-            gen_pass(c, +1, 11, in, w.p, u.rs, o.nxp, 2, w.rs, o.nxp, 0, ny, 8, 5, y0);
+            gen_pass(c, +1, 11, in, w.p, u.rs, o.nxp, 2, w.rs, o.nxp, 0, ny, 8, 5, y0, 1);
         }
         const bool d2h = mode == 0 ? o.work_host : (o.state_host || (next_inverse && o.work_host));
         chunk_comp_done(c, ch, d2h);
@@ -636,7 +645,29 @@ int ooc_dist_config(mhd_ctx* c, int rank, int world) {
     return MHD_OK;
 }
 
+int ooc_dist_peers(mhd_ctx* c, const long long* delta_bytes) {
+    Ooc& o = c->ooc;
+    if (!o.on || o.world > 8) return c->fail(MHD_ERR_INVALID_ARG, "direct exchange: decomposed context with at most 8 ranks");
+    o.direct = delta_bytes != nullptr;
+    for (int s = 0; s < 8; ++s) o.peer_delta[s] = 0;
+    if (delta_bytes)
+        for (int s = 0; s < o.world; ++s) {
+            if (delta_bytes[s] % (long long)sizeof(cd)) return c->fail(MHD_ERR_INVALID_ARG, "peer workspaces must be 16-byte congruent");
+            o.peer_delta[s] = s == o.rank ? 0 : delta_bytes[s] / (long long)sizeof(cd);
+        }
+    return MHD_OK;
+}
+
+static int dist_phase_body(mhd_ctx* c, int phase, int arg);
 int ooc_dist_phase(mhd_ctx* c, int phase, int arg) {
+    Ooc& o = c->ooc;
+    // rows go straight to their owners only in the phases of the step; set / get_fields use the packed exchange
+    o.direct_active = o.direct && (phase == MHD_DIST_PHASE_A || phase == MHD_DIST_PHASE_B || phase == MHD_DIST_PHASE_C);
+    const int rc = dist_phase_body(c, phase, arg);
+    o.direct_active = false;
+    return rc;
+}
+static int dist_phase_body(mhd_ctx* c, int phase, int arg) {
     switch (phase) {
         case MHD_DIST_PHASE_A: return stage_inverse_z(c, c->ooc.Uc, true);
         case MHD_DIST_PHASE_B: { SlabIO io; io.nin = 11; io.nout = 16; return stage_slabs(c, SLAB_FLUX, io); }

@@ -105,8 +105,11 @@ class DistMHD(B.MHD):
         L_.mhd_dist_ranges.argtypes = [C.c_void_p, C.c_int] + [C.POINTER(C.c_int)] * 4
         self.rank, self.world, self.group = int(rank), int(world), group
         self._check(L_.mhd_dist_config(self._h, self.rank, self.world))
+        L_.mhd_dist_peers.argtypes = [C.c_void_p, C.POINTER(C.c_longlong)]
         self._pending_A = False      # phase A of the next step already ran inside phase C
-        self.exchanged_bytes = 0     # bytes this rank has sent to OTHER ranks
+        self.exchanged_bytes = 0     # bytes this rank has sent to OTHER ranks through the packed exchange
+        self.direct = False          # rows stored straight into the owners' workspaces (set_peers)
+        self._peer_keep = []
 
     # -- ABI calls ---------------------------------------------------------------------------------------
     def phase(self, which, arg=0):
@@ -133,6 +136,46 @@ class DistMHD(B.MHD):
     def unpack(self, direction, nf, recv):
         self._check(self._L.mhd_dist_unpack(self._h, int(direction), int(nf), recv.data_ptr()))
 
+    def set_peers(self, peer_bases):
+        """Direct exchange: peer_bases[s] = address, IN THIS PROCESS, of rank s's (256-byte aligned) workspace base
+        (its own for s = rank); None switches back to the packed exchange."""
+        if peer_bases is None:
+            self._check(self._L.mhd_dist_peers(self._h, None))
+            self.direct = False
+            return
+        d = (C.c_longlong * self.world)(*[int(b) - int(self._base) for b in peer_bases])
+        self._check(self._L.mhd_dist_peers(self._h, d))
+        self.direct = self.world > 1
+
+    def connect_peers_ipc(self):
+        """One process per GPU: map every peer's workspace into this process (CUDA IPC; NVLink peer access between GPUs)
+        and switch to the direct exchange.  Handles travel through the process group as pickled objects."""
+        import torch.distributed as dist
+        torch = self.torch
+        self.stream.synchronize()
+        info = self.workspace.untyped_storage()._share_cuda_()          # (device, handle, size, offset, ...)
+        mine = {"rank": self.rank, "share": info, "base_off": int(self._base) - int(self.workspace.data_ptr())}
+        allinfo = [None] * self.world
+        dist.all_gather_object(allinfo, mine, group=self.group)
+        bases = []
+        for s, inf in enumerate(allinfo):
+            if s == self.rank:
+                bases.append(int(self._base))
+                continue
+            with torch.cuda.device(self.device):
+                st = torch.UntypedStorage._new_shared_cuda(*inf["share"])
+            self._peer_keep.append(st)                                   # keeps the mapping alive
+            bases.append(int(st.data_ptr()) + inf["base_off"])
+        self.set_peers(bases)
+        dist.barrier(group=self.group)
+
+    def barrier(self):
+        """Where the packed protocol exchanges, the direct one only orders: my stores are done, so are my peers'."""
+        import torch.distributed as dist
+        self.stream.synchronize()
+        if self.world > 1:
+            dist.barrier(group=self.group)
+
     # -- the protocol, as generators that yield (direction, nfields) where an exchange is due ---------------------
     def _gen_set_fields(self, fields, kind):
         B.MHD.set_fields(self, fields, kind)              # own z planes: prim->cons, forward x and y passes
@@ -143,10 +186,12 @@ class DistMHD(B.MHD):
     def _gen_step(self, n):
         for s in range(int(n)):
             if not self._pending_A:
+                if self.direct and s == 0:
+                    yield ("barrier",)                    # peers may still read the rows phase A is about to store
                 self.phase(PHASE_A)
-            yield (BRICKS_TO_SLABS, 11)
+            yield ("barrier",) if self.direct else (BRICKS_TO_SLABS, 11)
             self.phase(PHASE_B)
-            yield (SLABS_TO_BRICKS, 16)
+            yield ("barrier",) if self.direct else (SLABS_TO_BRICKS, 16)
             more = s + 1 < n
             self.phase(PHASE_C, 1 if more else 0)
             self._pending_A = more
@@ -170,8 +215,11 @@ class DistMHD(B.MHD):
         self.exchanged_bytes += 8 * sum(send_counts)
 
     def _drive(self, gen):
-        for direction, nf in gen:
-            self.exchange(direction, nf)
+        for req in gen:
+            if req[0] == "barrier":
+                self.barrier()
+            else:
+                self.exchange(*req)
 
     def set_fields(self, fields, kind="primitive"):
         self._drive(self._gen_set_fields(fields, kind))
@@ -221,7 +269,17 @@ class Lockstep:
             if all(q is None for q in reqs):
                 return
             assert all(q == reqs[0] for q in reqs), "ranks out of step"
-            self._exchange(*reqs[0])
+            if reqs[0][0] == "barrier":
+                for r in self.ranks:
+                    r.stream.synchronize()
+            else:
+                self._exchange(*reqs[0])
+
+    def connect_peers(self):
+        """Virtual ranks share one address space: every rank can store into every other rank's workspace."""
+        bases = [r._base for r in self.ranks]
+        for r in self.ranks:
+            r.set_peers(bases)
 
     def set_fields(self, fields, kind="primitive"):
         self._drive([r._gen_set_fields(fields, kind) for r in self.ranks])

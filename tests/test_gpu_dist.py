@@ -108,3 +108,96 @@ def test_decomposed_context_refuses_the_undecomposed_calls(mods):
     inc = binding.MHD(cfg.N)                        # an in-core context cannot be decomposed
     rc = inc._L.mhd_dist_config(inc._h, 0, 2)
     assert rc == -1
+
+
+@pytest.mark.parametrize("N,world", [(32, 2), (64, 3), (128, 8), (64, 5)])
+def test_direct_exchange_is_bitwise_too(mods, N, world):
+    """mhd_dist_peers: the z passes and the forward y pass store every row straight into its owner's workspace (what
+    P2P stores over NVLink do between GPUs; here the virtual ranks share one GPU's address space): no pack, no
+    collective, no unpack — and still the bits of the undecomposed step."""
+    binding, dist = mods
+    cfg = inputs.config3(N, kmax=4) if N >= 64 else inputs.config2(N)
+    ref = binding.MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, flags=binding.MHD_FLAG_OUT_OF_CORE)
+    ref.set_fields(cfg.prim, "primitive")
+    grp = make_ranks(dist, cfg, world)
+    grp.connect_peers()
+    assert all(r.direct for r in grp.ranks)
+    grp.set_fields(cfg.prim, "primitive")
+    ref.step(3); grp.step(3)
+    ref.step(2); grp.step(2)
+    Ur, Ug = ref.get_fields("primitive"), grp.get_fields("primitive")
+    for f in range(8):
+        assert np.array_equal(Ur[f], Ug[f]), ("after 5 steps", f)
+    assert all(r.exchanged_bytes == grp.ranks[0].exchanged_bytes for r in grp.ranks[:1])
+    # the step itself moved nothing through packed buffers: only set_fields / get_fields did (8 fields, twice)
+    sent = grp.ranks[0].exchanged_bytes
+    grp.step(2)
+    assert grp.ranks[0].exchanged_bytes == sent
+
+
+IPC_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, %r)
+import numpy as np, torch
+import torch.distributed as dist
+from paper_1810_12707_b200 import dist as D, inputs
+dist.init_process_group("gloo")                      # host-side barriers and handle exchange only
+rank, world = dist.get_rank(), dist.get_world_size()
+torch.cuda.set_device(0)                             # both processes on the one GPU: CUDA IPC maps the peer's workspace
+cfg = inputs.config2(32)
+g = D.DistMHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, rank=rank, world=world, device="cuda:0")
+g.connect_peers_ipc()
+assert g.direct
+# set / get use the packed exchange: gloo all_to_all_single needs host tensors, so route it through the host here
+def exchange_via_host(direction, nf):
+    send, sc, rc = g.pack(direction, nf)
+    g.stream.synchronize()
+    recv = torch.empty(sum(rc), dtype=torch.float64)
+    D.all_to_all(recv, send.cpu(), rc, sc)
+    buf = torch.empty(max(1, recv.numel()), dtype=torch.float64, device="cuda:0")
+    buf[:recv.numel()].copy_(recv)
+    g.unpack(direction, nf, buf)
+    g.stream.synchronize()
+g.exchange = exchange_via_host
+g.set_fields(cfg.prim, "primitive")
+g.step(3)
+g.step(2)
+out = g.get_fields("primitive")
+(za, zb) = g.ranges()[1]
+np.save(os.environ["OUT_PREFIX"] + str(rank) + ".npy", np.stack([o[za:zb] for o in out]))
+dist.barrier()
+print(json.dumps({"rank": rank, "z": [za, zb], "direct": g.direct}))
+dist.destroy_process_group()
+"""
+
+
+def test_direct_exchange_between_two_processes_over_cuda_ipc(mods, tmp_path):
+    """Two PROCESSES (ranks 0, 1) on the one GPU: each maps the other's workspace through CUDA IPC (the mechanism that
+    gives NVLink peer access between GPUs) and the step runs with direct stores and host barriers only — no kernel
+    waits on the other rank.  Result: bitwise the undecomposed step."""
+    import json, os, socket, subprocess, sys
+    binding, dist = mods
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    prefix = str(tmp_path / "rank")
+    procs = []
+    for rank in range(2):
+        env = dict(os.environ, RANK=str(rank), LOCAL_RANK="0", WORLD_SIZE="2", MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port),
+                   OUT_PREFIX=prefix)
+        procs.append(subprocess.Popen([sys.executable, "-c", IPC_WORKER % root], env=env, stdout=subprocess.PIPE,
+                                      stderr=subprocess.PIPE, text=True))
+    metas = []
+    for p in procs:
+        out, err = p.communicate(timeout=600)
+        assert p.returncode == 0, err[-3000:]
+        metas.append(json.loads(out.strip().splitlines()[-1]))
+    cfg = inputs.config2(32)
+    ref = binding.MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, flags=binding.MHD_FLAG_OUT_OF_CORE)
+    ref.set_fields(cfg.prim, "primitive")
+    ref.step(3); ref.step(2)
+    Ur = ref.get_fields("primitive")
+    for m in metas:
+        za, zb = m["z"]
+        got = np.load(prefix + str(m["rank"]) + ".npy")
+        for f in range(8):
+            assert np.array_equal(got[f], Ur[f][za:zb]), (m["rank"], f)
