@@ -120,16 +120,22 @@ unsigned blocks_for(long long np) { return (unsigned)((np + 127) / 128); }
 // ---- spatial sort (counting sort by grid row) ------------------------------------------------------------------
 // Random particle order makes the gather DRAM-bound at sector granularity (ncu: ~670 B of DRAM reads per push at 256^3,
 // against 48 B of particle state).  Sorted by the (z, y) row of their cell, consecutive threads read the same few grid
-// rows, which then come from L1 / L2.  key = iz * N + iy (N^2 <= 2^20 bins); three kernels: histogram (the atomic's
+// rows, which then come from L1 / L2.  key = (iz * N + iy) * xb + coarse x (<= 2^20 bins); three kernels: histogram (the atomic's
 // return value is the particle's rank inside its bin), exclusive scan of the bins, scatter.  The order inside a bin
 // depends on the atomics, but every particle's own trajectory does not depend on where it is stored, and
 // mhd_tracers_get un-permutes by id: results are bitwise independent of the sort.
+__host__ __device__ inline unsigned sort_xbins(int N) {
+    const unsigned cap = (1u << 20) / ((unsigned)N * (unsigned)N);
+    return cap >= 16 ? 16u : (cap >= 4 ? 4u : 1u);
+}
 __global__ void sort_hist_kernel(const __grid_constant__ TracerArgs a, unsigned* __restrict__ hist, unsigned* __restrict__ key,
                                  unsigned* __restrict__ rank) {
     const long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (m >= a.np) return;
     const CellIdx c = locate(a.N, (double)a.N / a.L, a.pos[0][m], a.pos[1][m], a.pos[2][m]);
-    const unsigned k = (unsigned)c.i0[2] * (unsigned)a.N + (unsigned)c.i0[1];
+    // (z, y) row of the cell, refined by a coarse x index while the bins fit (xb = 1, 4, 16 sub-bins per row at 1024, 512, <= 256)
+    const unsigned xb = sort_xbins(a.N);
+    const unsigned k = ((unsigned)c.i0[2] * (unsigned)a.N + (unsigned)c.i0[1]) * xb + (unsigned)c.i0[0] * xb / (unsigned)a.N;
     key[m] = k;
     rank[m] = atomicAdd(&hist[k], 1u);
 }
@@ -182,7 +188,7 @@ void launch_tracer_unpermute(long long np, const long long* id, const double* in
 void launch_tracer_sort(const TracerArgs& a, const long long* id, double* const alt[6], long long* alt_id, unsigned* hist,
                         unsigned* key, unsigned* rank, cudaStream_t st) {
     if (a.np <= 0) return;
-    const int nbins = a.N * a.N;
+    const int nbins = a.N * a.N * (int)sort_xbins(a.N);
     cudaMemsetAsync(hist, 0, (size_t)nbins * sizeof(unsigned), st);
     sort_hist_kernel<<<blocks_for(a.np), 128, 0, st>>>(a, hist, key, rank);
     sort_scan_kernel<<<1, 1024, 0, st>>>(hist, nbins);
