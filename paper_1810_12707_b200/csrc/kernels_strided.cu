@@ -40,10 +40,13 @@ strided_kernel(const __grid_constant__ StridedArgs a) {
 
     const int tid = threadIdx.x;
     const int c = tid % C, t = tid / C;
-    const int col = blockIdx.x * C + c;
+    // FJ: the field is the fastest block index, so that the CTAs which read the same B^ tile (B itself and the two J
+    // components built from it) run back to back and share it through L2 instead of fetching it from DRAM three times
+    const int bx = FJ ? blockIdx.x / a.nfields : blockIdx.x;
+    const int col = bx * C + c;
     int o = blockIdx.y;
     if (!GEN && o >= a.outer_split) o += a.outer_skip;
-    const int f = blockIdx.z;
+    const int f = FJ ? blockIdx.x % a.nfields : blockIdx.z;
     const bool valid = col < a.ncols;
     const int kc = a.kc;
 
@@ -121,6 +124,7 @@ template <int N, int DIR, int C, bool GEN, bool FJ> static void launch_one(const
         configured = true;
     }
     dim3 grid((a.ncols + C - 1) / C, a.n_outer, a.nfields);
+    if (FJ) grid = dim3(grid.x * a.nfields, a.n_outer, 1);
     strided_kernel<N, DIR, C, GEN, FJ><<<grid, threads, smem, st>>>(a);
 }
 

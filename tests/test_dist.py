@@ -153,3 +153,24 @@ def test_partition_is_balanced_and_counts_match():
             own = sum(2 * 11 * (D.ranges(N, world, r)[1][1] - D.ranges(N, world, r)[1][0])
                       * (D.ranges(N, world, r)[0][1] - D.ranges(N, world, r)[0][0]) * nxp for r in range(world))
             assert tot_s == tot_r == 2 * 11 * N * nyc * nxp - own      # everything but the ranks' own blocks travels
+
+
+def test_algorithmic_bytes_match_the_measured_dram_traffic():
+    """bench.sweep_bytes (the algorithmic bytes behind every roofline fraction) against the DRAM bytes per launch that
+    ncu measured (profiles/traffic_r01.json, from the committed captures): equal to within 4 %, i.e. no
+    kernel re-reads what it should stream once, and the accounting does not flatter the fractions."""
+    import json
+    sys.path.insert(0, ROOT)
+    import bench
+    traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic_r01.json")))
+    for N in (256, 512):
+        sb = bench.sweep_bytes(N, prune=True)
+        launches = {"strided_inverse": 2, "strided_forward": 2, "x_fused": 1, "assemble": 1}
+        for fam, n in launches.items():
+            alg = sb[fam] / n
+            meas = traffic[str(N)][fam]
+            assert abs(meas / alg - 1.0) <= 0.04, (N, fam, meas / alg)
+    # unpruned accounting: SURVEY.md's 148 field sweeps + the 32 of the separate forward z pass
+    f = 8.0 * 512 ** 3
+    assert abs(sum(bench.sweep_bytes(512, prune=False).values()) / f - 180.0) < 1e-9
+    assert bench.unpruned_reference_bytes(512) == 1184.0 * 512 ** 3
