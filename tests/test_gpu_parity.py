@@ -218,6 +218,24 @@ def test_100_steps(orc, MHD, cfgname, N):
         assert rel_l2(b[f], a[f]) <= 1e-9, NAMES[f]
 
 
+@pytest.mark.parametrize("cfgname,N,nsteps", [("2", 64, 200), ("3", 128, 40)])
+def test_config_runs_at_full_size(orc, MHD, cfgname, N, nsteps):
+    """BASELINE.json config 2 in full (64^3, 200 steps) and config 3 at its full 128^3 (the second-generation fused x
+    sweep; 40 of its 500 steps: the oracle needs ~1 s per step there): state <= 1e-9 (north_star), diagnostics too."""
+    cfg = inputs.by_name(cfgname, N)
+    o, g = both(orc, MHD, cfg)
+    o.step(nsteps)
+    g.step(nsteps)
+    a, b = o.get_fields(), g.get_fields()
+    scale = max(np.linalg.norm(x) for x in a)
+    for f in range(8):
+        assert np.linalg.norm(b[f] - a[f]) <= 1e-9 * max(np.linalg.norm(a[f]), 1e-6 * scale), NAMES[f]
+    do, dg = o.diagnostics(), g.diagnostics()
+    for k in ("ke", "me", "ie", "mass", "etot"):
+        assert abs(dg[k] - do[k]) <= 1e-11 * abs(do[k]), k
+    assert dg["step"] == nsteps and dg["max_divb"] <= 1e-11
+
+
 def test_step_split_is_bitwise_and_step0_is_noop(orc, MHD):
     cfg = inputs.config1(32)
     _, g1 = both(orc, MHD, cfg)
