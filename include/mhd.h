@@ -216,6 +216,9 @@ int mhd_dist_ranges(mhd_ctx *ctx, int rank, int *ky_lo, int *ky_hi, int *z_lo, i
  * exchange would be (after A, after B): [A] barrier B barrier C(next).  NULL switches back to the packed exchange.
  * mhd_set_fields / mhd_get_fields keep using the packed exchange. */
 int mhd_dist_peers(mhd_ctx *ctx, const long long *delta_bytes);
+/* Lets kernels of the current device dereference memory of `peer_device` (cudaDeviceEnablePeerAccess; "already enabled"
+ * is not an error).  Needed once per peer GPU before the direct exchange; a no-op for the current device itself. */
+int mhd_dist_enable_peer_access(mhd_ctx *ctx, int peer_device);
 
 /* Bytes the chunked pipeline has copied host->device / device->host so far (0 for an in-core context). */
 int mhd_transfer_bytes(const mhd_ctx *ctx, long long *h2d, long long *d2h);

@@ -36,7 +36,8 @@ SYMBOLS = ["mhd_init", "mhd_workspace_bytes", "mhd_pinned_bytes", "mhd_bind", "m
            "mhd_fft3d_c2r", "mhd_launch_count", "mhd_transfer_bytes", "mhd_profile_enable", "mhd_profile_get", "mhd_last_error",
            "mhd_destroy", "mhd_tracers_bytes", "mhd_tracers_bind", "mhd_tracers_set", "mhd_tracers_get",
            "mhd_tracers_push", "mhd_set_param", "mhd_probe_fp64", "mhd_dist_config", "mhd_dist_phase",
-           "mhd_dist_counts", "mhd_dist_pack", "mhd_dist_unpack", "mhd_dist_ranges", "mhd_dist_peers"]
+           "mhd_dist_counts", "mhd_dist_pack", "mhd_dist_unpack", "mhd_dist_ranges", "mhd_dist_peers",
+           "mhd_dist_enable_peer_access"]
 
 
 class MhdDiag(C.Structure):

@@ -735,6 +735,21 @@ int mhd_dist_peers(mhd_ctx* c, const long long* delta_bytes) {
     if (!c || !c->bound || !c->ooc.on) return MHD_ERR_INVALID_ARG;
     return ooc_dist_peers(c, delta_bytes);
 }
+int mhd_dist_enable_peer_access(mhd_ctx* c, int peer_device) {
+    if (!c) return MHD_ERR_INVALID_ARG;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return c->fail(MHD_ERR_CUDA, "no current CUDA device"); }
+    if (peer_device == dev) return MHD_OK;
+    int can = 0;
+    if (cudaDeviceCanAccessPeer(&can, dev, peer_device) != cudaSuccess || !can) {
+        cudaGetLastError();
+        return c->fail(MHD_ERR_CUDA, "no peer access between the two devices");
+    }
+    const cudaError_t e = cudaDeviceEnablePeerAccess(peer_device, 0);
+    if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) return c->fail(MHD_ERR_CUDA, cudaGetErrorString(e));
+    cudaGetLastError();
+    return MHD_OK;
+}
 int mhd_dist_ranges(mhd_ctx* c, int rank, int* ky_lo, int* ky_hi, int* z_lo, int* z_hi) {
     if (!c || !c->bound || !c->ooc.on || rank < 0 || rank >= c->ooc.world) return MHD_ERR_INVALID_ARG;
     if (ky_lo) *ky_lo = c->ooc.ky_lo(rank);

@@ -162,6 +162,11 @@ class DistMHD(B.MHD):
             if s == self.rank:
                 bases.append(int(self._base))
                 continue
+            peer_dev = int(inf["share"][0])
+            if peer_dev != self.device.index:             # another GPU: kernels here must be allowed to store into it
+                with torch.cuda.device(self.device):
+                    self._L.mhd_dist_enable_peer_access.argtypes = [C.c_void_p, C.c_int]
+                    self._check(self._L.mhd_dist_enable_peer_access(self._h, peer_dev))
             with torch.cuda.device(self.device):
                 st = torch.UntypedStorage._new_shared_cuda(*inf["share"])
             self._peer_keep.append(st)                                   # keeps the mapping alive
