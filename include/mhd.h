@@ -80,7 +80,7 @@ extern "C" {
 #define MHD_OPT_TRACER_SORT 11 /* re-sort the tracer storage by grid row every this many pushes (default 32; 0 = never):
                                   gather locality only, results do not depend on it (mhd_tracers_get returns id order) */
 
-/* Equation-set variants of the paper (readings V1-V3).  Changing one resets the integrator history. */
+/* Equation-set variants of the paper (readings V1-V4).  Changing one resets the integrator history. */
 #define MHD_OPT_EVOLVE 8  /* bit 0: Eq. 17-18 and the energy equation evolve, bit 1: Eq. 19 evolves (default 3).  2 = the
                              kinematic dynamo of PAPER.md L205 ("turn off Eq. 17 and 18"), 1 = hydrodynamic (L199)      */
 #define MHD_OPT_STRESS 12 /* 1: the viscous terms of PAPER.md Eq. 11-12 (L92-96): + div(2 nu rho S) in the momentum equation and

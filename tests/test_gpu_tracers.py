@@ -191,3 +191,38 @@ def test_spatial_sort_does_not_change_results(MHD, every):
         out.append((ph, vh))
     for c in range(3):
         assert np.array_equal(out[0][0][c], out[1][0][c]) and np.array_equal(out[0][1][c], out[1][1][c])
+
+
+def test_bench_scale_256_both_B_sources_agree(MHD):
+    """At the bench's 256^3 with 2 M tracers (the configuration `bench.py --tracers` times): B taken from the fused x
+    sweep's by-product and B from the separate inverse transform move the particles identically to round-off, and the
+    oracle's push on sampled particles reproduces one step."""
+    import oracle
+    cfg = inputs.config45(256)
+    res = []
+    for fused in (1, 2):
+        g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+        g.set_option(1, fused)
+        g.set_fields(cfg.prim, "primitive")
+        pos, _ = particles(2_000_003, 77)
+        g.tracers_set(pos)                       # v0 = CIC of u
+        p0, v0 = g.tracers_get()
+        if fused == 1:
+            B = g.get_fields("conservative")[5:8]
+            idx = np.arange(0, 2_000_003, 4001)
+            ps, vs = oracle.tracers_push(B, [p[idx] for p in p0], [v[idx] for v in v0], cfg.dt, 1, L=cfg.L)
+        g.step(4)
+        res.append(g.tracers_get())
+        if fused == 1:
+            g2 = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+            g2.set_fields(cfg.prim, "primitive")
+            g2.tracers_set(p0, v0)
+            g2.step(1)
+            p1, v1 = g2.tracers_get()
+            for c in range(3):
+                assert np.max(wrapped_diff(p1[c][idx], ps[c])) <= 1e-13 * L and np.max(np.abs(v1[c][idx] - vs[c])) <= 1e-13 * 10
+            del g2
+        del g
+    for c in range(3):
+        assert np.max(wrapped_diff(res[0][0][c], res[1][0][c])) <= 1e-12 * L
+        assert np.max(np.abs(res[0][1][c] - res[1][1][c])) <= 1e-12 * 10
