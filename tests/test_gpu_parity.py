@@ -236,6 +236,36 @@ def test_config_runs_at_full_size(orc, MHD, cfgname, N, nsteps):
     assert dg["step"] == nsteps and dg["max_divb"] <= 1e-11
 
 
+def test_config4_as_specified_100_steps_diagnostics_every_10(orc, MHD):
+    """BASELINE.json config 4 as written: 256^3 ABC dynamo, 100 steps, energy and div B diagnostics every 10 steps (the
+    driver of paper_1810_12707_b200/run.py).  Checked: conservation of <rho>, <m>, <E> (pin P11) and div B (P10) along
+    the series, closed-form values at t = 0 (P14), the same series from a 128^3 run of the same band-limited initial
+    condition (resolution independence), and the oracle's series at 64^3 over the first 20 steps."""
+    import io
+    from paper_1810_12707_b200 import run as runner
+    s256 = runner.run("4", 256, 100, 10, out=io.StringIO())
+    s128 = runner.run("4", 128, 100, 10, out=io.StringIO())
+    assert [d["step"] for d in s256] == list(range(0, 101, 10))
+    d0 = s256[0]
+    assert abs(d0["ke"] - 1.5) <= 1e-12 and abs(d0["me"] - 5e-9) <= 1e-18 and abs(d0["ie"] - 90.0) <= 1e-10
+    for d in s256:
+        assert abs(d["mass"] - 1.0) <= 1e-13 and abs(d["etot"] - d0["etot"]) <= 1e-12 * d0["etot"]
+        assert max(abs(m - m0) for m, m0 in zip(d["mom"], d0["mom"])) <= 1e-13
+        assert d["max_divb"] <= 1e-13 * 85 * 1e-4 * 10
+    for a, b in zip(s256, s128):
+        for k in ("ke", "me", "ie"):
+            assert abs(a[k] - b[k]) <= 1e-11 * abs(b[k]), (a["step"], k)
+    assert s256[-1]["ke"] < d0["ke"] and s256[-1]["me"] != d0["me"]          # viscous decay; B is being stretched
+    cfg = inputs.config45(64)
+    o = orc.Oracle(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+    o.set_fields(cfg.prim, "primitive")
+    for i in (1, 2):
+        o.step(10)
+        do = o.diagnostics()
+        for k in ("ke", "me", "ie"):
+            assert abs(s256[i][k] - do[k]) <= 1e-11 * abs(do[k]), (i, k)
+
+
 def test_step_split_is_bitwise_and_step0_is_noop(orc, MHD):
     cfg = inputs.config1(32)
     _, g1 = both(orc, MHD, cfg)
