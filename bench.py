@@ -326,7 +326,8 @@ def run_ours(args):
         # slab decomposition: ONE problem over all ranks, two all-to-alls per step (strong scaling)
         from paper_1810_12707_b200.dist import DistMHD
         flags = B.MHD_FLAG_OUT_OF_CORE
-        g = DistMHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, rank=rank, world=world, device="cuda:%d" % local_rank)
+        g = DistMHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, rank=rank, world=world, device="cuda:%d" % local_rank,
+                    per_rank_storage=True)
         if world > 1 and not args.packed_exchange:
             g.connect_peers_ipc()        # rows go straight into the owners' workspaces (P2P stores); barriers instead of all-to-alls
         args.no_e2e = args.no_fft = True

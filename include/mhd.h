@@ -57,6 +57,10 @@ extern "C" {
 #define MHD_FLAG_OUT_OF_CORE 1u   /* chunked pipeline on compact storage; with no placement flag everything stays in HBM */
 #define MHD_FLAG_STATE_ON_HOST 2u /* U^ and the Adams-Bashforth history live in pinned host memory                      */
 #define MHD_FLAG_WORK_ON_HOST 4u  /* the 16 work fields between the z and y passes live in pinned host memory           */
+#define MHD_FLAG_RANKS(g) ((unsigned)((g) - 1) << 4) /* slab decomposition over g = 1..8 GPUs with PER-RANK storage: the context
+                                     allocates only one rank's share (1/g of the state, 2/g of the work arrays: a brick-shaped
+                                     and a slab-shaped set); needs MHD_FLAG_OUT_OF_CORE without host placement, and
+                                     mhd_dist_config(rank, g) before any field call                                      */
 #define MHD_FLAG_BUDGET_MIB(m) ((unsigned)(m) << 8) /* cap on the device workspace in MiB (0 = none): bounds the staging
                                      buffers; mhd_workspace_bytes() returns 0 if the placement cannot fit the budget     */
 

@@ -68,7 +68,16 @@ struct mhd_ctx {
         static constexpr int NBUF = 3;
         bool on = false, state_host = false, work_host = false;
         int nzc = 0, nyc = 0, nxp = 0;           // compact extents: 2kc+1, 2kc+1, kc+1 rounded up to 8
-        cd *Uc[8], *Rc[8], *Wz[16];              // compact state / history [nzc][nyc][nxp]; z-full work [N][nyc][nxp]
+        cd *Uc[8], *Rc[8];                       // compact state / history [nzc][nyc][nxp]
+        // work arrays between the z and y passes.  Unified layout (one context holds everything): WzB = WzS = [N][nyc][nxp].
+        // Per-rank layout (MHD_FLAG_RANKS, `split`): WzB = [N][ny_max][nxp] holds all z of the rank's ky share (stages A, C),
+        // WzS = [nz_max][nyc][nxp] all ky of its z share (stage B); the state arrays are [nzc][ny_max][nxp]
+        cd *WzB[16], *WzS[16];
+        bool split = false;
+        int ny_max = 0, nz_max = 0;
+        int yoff() const { return split ? ky_lo(rank) : 0; }                       // first ky / z index that is stored
+        int zoff(int N) const { return split ? z_lo(rank, N) : 0; }
+        long long bstride() const { return (long long)(split ? ny_max : nyc) * nxp; }   // z stride of brick-shaped arrays
         char* stage = nullptr;                   // NBUF staging sets (one big set when nothing lives on the host)
         size_t stage_bytes = 0;                  // bytes of one set
         int nbuf = 1;

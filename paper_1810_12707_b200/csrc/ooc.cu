@@ -27,8 +27,10 @@ constexpr int NBUF = Ooc::NBUF;
 
 struct OocSizes {
     int kc, nzc, nyc, nxp, hx;
-    size_t celems, welems;        // elements of one compact / one z-full array
-    size_t cbytes, wbytes;
+    size_t celems, welems, selems;   // elements of one compact state / one brick-shaped work / one slab-shaped work array
+    size_t cbytes, wbytes, sbytes;
+    int ranks, ny_max, nz_max;       // per-rank storage (MHD_FLAG_RANKS): shares of the ky and z axes
+    size_t slab_off;
     size_t tw_off, ftw_off, state_off, work_off, stage_off, stage_total, part_off, part_bytes, res_off, total;
     size_t per_ky, per_z;         // staging bytes per ky column of a brick / per z plane of a slab
     bool state_host, work_host;
@@ -46,14 +48,19 @@ bool ooc_sizes(int N, unsigned flags, OocSizes& s) {
     s.kc = N / 3; s.nzc = 2 * s.kc + 1; s.nyc = s.nzc; s.nxp = (s.kc + 1 + 7) / 8 * 8; s.hx = N / 2;
     s.state_host = (flags & MHD_FLAG_STATE_ON_HOST) != 0;
     s.work_host = (flags & MHD_FLAG_WORK_ON_HOST) != 0;
-    s.celems = (size_t)s.nzc * s.nyc * s.nxp; s.welems = (size_t)N * s.nyc * s.nxp;
-    s.cbytes = align_up(s.celems * sizeof(cd)); s.wbytes = align_up(s.welems * sizeof(cd));
+    s.ranks = (int)((flags >> 4) & 7u) + 1;
+    if (s.ranks > 1 && (s.state_host || s.work_host || s.ranks > s.nyc || s.ranks > N)) return false;
+    s.ny_max = (s.nyc + s.ranks - 1) / s.ranks; s.nz_max = (N + s.ranks - 1) / s.ranks;
+    s.celems = (size_t)s.nzc * s.ny_max * s.nxp; s.welems = (size_t)N * s.ny_max * s.nxp;
+    s.selems = s.ranks > 1 ? (size_t)s.nz_max * s.nyc * s.nxp : 0;
+    s.cbytes = align_up(s.celems * sizeof(cd)); s.wbytes = align_up(s.welems * sizeof(cd)); s.sbytes = align_up(s.selems * sizeof(cd));
     const int ns = nspec_of(N);
     size_t off = 0;
     s.tw_off = off; off += align_up((size_t)N * sizeof(cd));
     s.ftw_off = off; off += align_up((size_t)(4 * N + 64) * sizeof(cd));
     s.state_off = off; if (!s.state_host) off += 16 * s.cbytes;
     s.work_off = off; if (!s.work_host) off += 16 * s.wbytes;
+    s.slab_off = off; off += 16 * s.sbytes;
     s.part_bytes = align_up((size_t)(diag_partial_doubles() + absmax_partial_doubles() + spectrum_partial_doubles(ns)) * sizeof(double));
     s.part_off = off; off += s.part_bytes;
     s.res_off = off; off += align_up((size_t)(64 + 2 * ns) * sizeof(double));
@@ -194,7 +201,10 @@ void gen_pass(mhd_ctx* c, int dir, int nf, const cd* const in[], cd* const out[]
     if (peer_rows && o.direct_active && o.world > 1) {
         a.npeer = o.world;
         for (int s = 0; s <= o.world; ++s) a.peer_lo[s] = peer_rows == 1 ? o.z_lo(s, c->N) : o.ky_lo(s);
-        for (int s = 0; s < o.world; ++s) a.peer_delta[s] = o.peer_delta[s];
+        // per-rank storage: the owner's array starts at its own first z plane / ky row
+        const long long plane = (long long)o.nyc * o.nxp;
+        for (int s = 0; s < o.world; ++s)
+            a.peer_delta[s] = o.peer_delta[s] - (o.split ? (peer_rows == 1 ? o.z_lo(s, c->N) * plane : (long long)o.ky_lo(s) * o.nxp) : 0);
     }
     mhd_ctx::Scope s(c, dir > 0 ? F_STRIDED_INV : F_STRIDED_FWD);
     launch_strided(c->N, dir, a, c->st);
@@ -213,8 +223,8 @@ View state_view(mhd_ctx* c, Chunk& ch, cd* const arr[], int nf, int y0, int ny, 
             if (load && !ch.overflow) h2d_2d(c, v.p[f], (size_t)v.rs, arr[f] + (size_t)y0 * o.nxp, (size_t)o.nyc * o.nxp, (size_t)v.rs, o.nzc);
         }
     } else {
-        v.rs = (long long)o.nyc * o.nxp;
-        for (int f = 0; f < nf; ++f) v.p[f] = arr[f] + (size_t)y0 * o.nxp;
+        v.rs = o.bstride();
+        for (int f = 0; f < nf; ++f) v.p[f] = arr[f] + (size_t)(y0 - o.yoff()) * o.nxp;
     }
     return v;
 }
@@ -231,11 +241,11 @@ View work_view(mhd_ctx* c, Chunk& ch, int nf, int y0, int ny, bool load) {
         v.rs = (long long)ny * o.nxp;
         for (int f = 0; f < nf; ++f) {
             v.p[f] = ch.alloc((size_t)c->N * ny * o.nxp);
-            if (load && !ch.overflow) h2d_2d(c, v.p[f], (size_t)v.rs, o.Wz[f] + (size_t)y0 * o.nxp, (size_t)o.nyc * o.nxp, (size_t)v.rs, c->N);
+            if (load && !ch.overflow) h2d_2d(c, v.p[f], (size_t)v.rs, o.WzB[f] + (size_t)y0 * o.nxp, (size_t)o.nyc * o.nxp, (size_t)v.rs, c->N);
         }
     } else {
-        v.rs = (long long)o.nyc * o.nxp;
-        for (int f = 0; f < nf; ++f) v.p[f] = o.Wz[f] + (size_t)y0 * o.nxp;
+        v.rs = o.bstride();
+        for (int f = 0; f < nf; ++f) v.p[f] = o.WzB[f] + (size_t)(y0 - o.yoff()) * o.nxp;
     }
     return v;
 }
@@ -243,13 +253,24 @@ void work_store(mhd_ctx* c, const View& v, int nf, int y0) {
     const Ooc& o = c->ooc;
     if (!o.work_host) return;
     for (int f = 0; f < nf; ++f)
-        d2h_2d(c, o.Wz[f] + (size_t)y0 * o.nxp, (size_t)o.nyc * o.nxp, v.p[f], (size_t)v.rs, (size_t)v.rs, c->N);
+        d2h_2d(c, o.WzB[f] + (size_t)y0 * o.nxp, (size_t)o.nyc * o.nxp, v.p[f], (size_t)v.rs, (size_t)v.rs, c->N);
 }
 SpecGeom brick_geom(const mhd_ctx* c, int y0, int ny, long long wrs, long long srs) {
     SpecGeom g = c->geom();
     g.pruned = 1; g.compact = 1; g.y0 = y0; g.ny = ny;
     g.wsy = c->ooc.nxp; g.wsz = wrs; g.ssy = c->ooc.nxp; g.ssz = srs;
     return g;
+}
+
+// where the inverse z pass of a brick writes: its own brick view — or, in the direct exchange with per-rank storage, the
+// SLAB-shaped arrays of the z planes' owners (addressed from this rank's slab array; gen_pass adds the owner's offset)
+View inverse_z_target(const mhd_ctx* c, const View& w, int y0) {
+    const Ooc& o = c->ooc;
+    if (!(o.direct_active && o.split)) return w;
+    View v;
+    v.rs = (long long)o.nyc * o.nxp;
+    for (int f = 0; f < 16; ++f) v.p[f] = o.WzS[f] + (size_t)y0 * o.nxp;
+    return v;
 }
 
 int overflow(mhd_ctx* c) { return c->fail(MHD_ERR_NOMEM, "chunked pipeline: staging set too small for one chunk"); }
@@ -269,7 +290,8 @@ int stage_inverse_z(mhd_ctx* c, cd* const src[8], bool current) {
         if (o.state_host) chunk_h2d_done(c, ch);
         const cd* in[11];
         for (int f = 0; f < 11; ++f) in[f] = u.p[f < 8 ? f : 5];
-        gen_pass(c, +1, nf, in, w.p, u.rs, o.nxp, 2, w.rs, o.nxp, 0, ny, current ? 8 : -1, 5, y0, 1);
+        const View wo = inverse_z_target(c, w, y0);
+        gen_pass(c, +1, nf, in, wo.p, u.rs, o.nxp, 2, wo.rs, o.nxp, 0, ny, current ? 8 : -1, 5, y0, 1);
         chunk_comp_done(c, ch, o.work_host);
         if (o.work_host) { work_store(c, w, nf, y0); chunk_d2h_done(c, ch); }
     }
@@ -308,11 +330,16 @@ int stage_slabs(mhd_ctx* c, SlabKind kind, const SlabIO& io) {
         for (int f = 0; f < io.nin; ++f) {
             if (o.work_host) {
                 cd* p = ch.alloc((size_t)zc * plane_c);
-                if (!ch.overflow) h2d_1d(c, p, o.Wz[f] + (size_t)z0 * plane_c, (size_t)zc * plane_c * sizeof(cd));
+                if (!ch.overflow) h2d_1d(c, p, o.WzS[f] + (size_t)z0 * plane_c, (size_t)zc * plane_c * sizeof(cd));
                 in[f] = p;
-            } else in[f] = o.Wz[f] + (size_t)z0 * plane_c;
+            } else in[f] = o.WzS[f] + (size_t)(z0 - o.zoff(N)) * plane_c;
         }
-        for (int f = 0; f < io.nout; ++f) out[f] = o.work_host ? ch.alloc((size_t)zc * plane_c) : o.Wz[f] + (size_t)z0 * plane_c;
+        // direct exchange with per-rank storage: the forward y pass stores each ky row into its owner's BRICK-shaped array
+        const bool to_bricks = io.nout > 0 && kind == SLAB_FLUX && o.direct_active && o.split;
+        for (int f = 0; f < io.nout; ++f)
+            out[f] = o.work_host ? ch.alloc((size_t)zc * plane_c)
+                   : to_bricks ? o.WzB[f] + (size_t)z0 * o.bstride()
+                               : o.WzS[f] + (size_t)(z0 - o.zoff(N)) * plane_c;
         if (ch.overflow) return overflow(c);
         if (kind == SLAB_FROM_REAL) {
             for (int f = 0; f < 8; ++f) {
@@ -355,11 +382,12 @@ int stage_slabs(mhd_ctx* c, SlabKind kind, const SlabIO& io) {
             launch_x_r2c(N, a, c->st);
         }
         if (io.nout > 0)     // forward y pass: all N rows -> the compact ky rows of the slab
-            gen_pass(c, -1, io.nout, sb, out, hx, (long long)N * hx, 0, o.nxp, (long long)plane_c, 2, zc, -1, 0, 0, 2);
+            gen_pass(c, -1, io.nout, sb, out, hx, (long long)N * hx, 0, o.nxp, to_bricks ? o.bstride() : (long long)plane_c, 2, zc,
+                     -1, 0, 0, 2);
         chunk_comp_done(c, ch, out_copy);
         if (out_copy) {
             if (io.nout > 0 && o.work_host)
-                for (int f = 0; f < io.nout; ++f) d2h_1d(c, o.Wz[f] + (size_t)z0 * plane_c, out[f], (size_t)zc * plane_c * sizeof(cd));
+                for (int f = 0; f < io.nout; ++f) d2h_1d(c, o.WzS[f] + (size_t)z0 * plane_c, out[f], (size_t)zc * plane_c * sizeof(cd));
             if (user_d2h)
                 for (int f = 0; f < 8; ++f) d2h_1d(c, io.user_out[f] + (size_t)z0 * plane_r, real[f], (size_t)zc * plane_r * sizeof(double));
             chunk_d2h_done(c, ch);
@@ -397,7 +425,8 @@ int stage_forward_z_assemble(mhd_ctx* c, int mode, bool next_inverse) {
         if (mode != 0 && next_inverse) {
             const cd* in[11];
             for (int f = 0; f < 11; ++f) in[f] = u.p[f < 8 ? f : 5];
-            gen_pass(c, +1, 11, in, w.p, u.rs, o.nxp, 2, w.rs, o.nxp, 0, ny, 8, 5, y0, 1);
+            const View wo = inverse_z_target(c, w, y0);
+            gen_pass(c, +1, 11, in, wo.p, u.rs, o.nxp, 2, wo.rs, o.nxp, 0, ny, 8, 5, y0, 1);
         }
         const bool d2h = mode == 0 ? o.work_host : (o.state_host || (next_inverse && o.work_host));
         chunk_comp_done(c, ch, d2h);
@@ -502,9 +531,13 @@ int ooc_bind(mhd_ctx* c, char* base, size_t bytes, char* pinned, size_t pinned_b
         else dst = reinterpret_cast<cd*>(base + s.state_off + (size_t)f * s.cbytes);
     }
     for (int f = 0; f < 16; ++f) {
-        if (s.work_host) { o.Wz[f] = reinterpret_cast<cd*>(hp); hp += s.wbytes; }
-        else o.Wz[f] = reinterpret_cast<cd*>(base + s.work_off + (size_t)f * s.wbytes);
+        if (s.work_host) { o.WzB[f] = reinterpret_cast<cd*>(hp); hp += s.wbytes; }
+        else o.WzB[f] = reinterpret_cast<cd*>(base + s.work_off + (size_t)f * s.wbytes);
+        o.WzS[f] = s.ranks > 1 ? reinterpret_cast<cd*>(base + s.slab_off + (size_t)f * s.sbytes) : o.WzB[f];
     }
+    o.split = s.ranks > 1; o.ny_max = s.ny_max; o.nz_max = s.nz_max;
+    o.rank = 0; o.world = s.ranks;            // per-rank storage: mhd_dist_config(rank, ranks) must follow
+    o.direct = false;
     const bool any_host = s.state_host || s.work_host;
     o.nbuf = any_host ? NBUF : 1;
     o.stage = base + s.stage_off;
@@ -640,6 +673,7 @@ int ooc_dist_config(mhd_ctx* c, int rank, int world) {
     Ooc& o = c->ooc;
     if (!o.on || o.state_host || o.work_host) return c->fail(MHD_ERR_INVALID_ARG, "decomposition needs MHD_FLAG_OUT_OF_CORE with everything in device memory");
     if (world < 1 || rank < 0 || rank >= world || world > o.nyc || world > c->N) return c->fail(MHD_ERR_INVALID_ARG, "rank / world");
+    if (o.split && world != o.world) return c->fail(MHD_ERR_INVALID_ARG, "world must equal the MHD_FLAG_RANKS the context was bound with");
     o.rank = rank; o.world = world;
     c->have_fields = false; c->have_old = false; c->step = 0;
     return MHD_OK;
@@ -712,7 +746,7 @@ int ooc_dist_pack(mhd_ctx* c, int dir, int nf, double* buf, int unpack) {
     if ((dir != 0 && dir != 1) || nf < 1 || nf > 16 || !buf) return c->fail(MHD_ERR_INVALID_ARG, "dir / nf / buffer");
     const int N = c->N, me = o.rank;
     cd* p = reinterpret_cast<cd*>(buf);
-    const size_t pitch = (size_t)o.nyc * o.nxp;
+    const size_t plane = (size_t)o.nyc * o.nxp;
     for (int s = 0; s < o.world; ++s) {
         if (s == me) continue;                                   // own block: stays where it is
         // geometry of the block in the work arrays: which rank's z range and which rank's ky range
@@ -720,13 +754,28 @@ int ooc_dist_pack(mhd_ctx* c, int dir, int nf, double* buf, int unpack) {
         const int rz = mine_ky ? s : me, ry = mine_ky ? me : s;
         const int z0 = o.z_lo(rz, N), nz = o.z_lo(rz + 1, N) - z0, y0 = o.ky_lo(ry), ny = o.ky_lo(ry + 1) - y0;
         const size_t width = (size_t)ny * o.nxp;
+        // "my ky, all z" lives in the brick-shaped arrays, "my z, all ky" in the slab-shaped ones (the same array when unified)
+        const size_t pitch = mine_ky ? (size_t)o.bstride() : plane;
         for (int f = 0; f < nf; ++f) {
-            cd* w = o.Wz[f] + (size_t)z0 * pitch + (size_t)y0 * o.nxp;
+            cd* w = mine_ky ? o.WzB[f] + (size_t)z0 * pitch + (size_t)(y0 - o.yoff()) * o.nxp
+                            : o.WzS[f] + (size_t)(z0 - o.zoff(N)) * pitch + (size_t)y0 * o.nxp;
             if (nz > 0 && ny > 0) {
                 if (!unpack) cudaMemcpy2DAsync(p, width * sizeof(cd), w, pitch * sizeof(cd), width * sizeof(cd), nz, cudaMemcpyDeviceToDevice, c->st);
                 else cudaMemcpy2DAsync(w, pitch * sizeof(cd), p, width * sizeof(cd), width * sizeof(cd), nz, cudaMemcpyDeviceToDevice, c->st);
             }
             p += width * nz;
+        }
+    }
+    if (unpack && o.split) {
+        // per-rank storage: the rank's own block (its ky share x its z share) changes arrays too — brick-shaped -> slab-shaped
+        // for dir 0, the other way for dir 1 (with the unified layout both are the same memory and nothing moves)
+        const int z0 = o.z_lo(me, N), nz = o.z_lo(me + 1, N) - z0, y0 = o.ky_lo(me), ny = o.ky_lo(me + 1) - y0;
+        const size_t width = (size_t)ny * o.nxp, bp = (size_t)o.bstride();
+        for (int f = 0; f < nf && nz > 0 && ny > 0; ++f) {
+            cd* b = o.WzB[f] + (size_t)z0 * bp;                   // [z][ky - y0]
+            cd* sl = o.WzS[f] + (size_t)y0 * o.nxp;               // [z - z0][ky]
+            if (dir == 0) cudaMemcpy2DAsync(sl, plane * sizeof(cd), b, bp * sizeof(cd), width * sizeof(cd), nz, cudaMemcpyDeviceToDevice, c->st);
+            else cudaMemcpy2DAsync(b, bp * sizeof(cd), sl, plane * sizeof(cd), width * sizeof(cd), nz, cudaMemcpyDeviceToDevice, c->st);
         }
     }
     return check_cuda(c, unpack ? "dist unpack" : "dist pack");

@@ -94,8 +94,11 @@ class DistMHD(B.MHD):
     """Rank `rank` of `world`: a chunked-pipeline context (everything in device memory) restricted to its shares."""
 
     def __init__(self, N, L=2 * np.pi, gamma=5.0 / 3.0, mu=0.0, eta=0.0, dt=1e-3, rank=0, world=1, device="cuda:0",
-                 stream=None, group=None):
-        super().__init__(N, L, gamma, mu, eta, dt, device=device, stream=stream, flags=B.MHD_FLAG_OUT_OF_CORE)
+                 stream=None, group=None, per_rank_storage=False):
+        """per_rank_storage: allocate only this rank's share (MHD_FLAG_RANKS: 1/world of the state, 2/world of the work
+        arrays) instead of full-size arrays of which the rank uses its share."""
+        flags = B.MHD_FLAG_OUT_OF_CORE | (((int(world) - 1) << 4) if per_rank_storage and world > 1 else 0)
+        super().__init__(N, L, gamma, mu, eta, dt, device=device, stream=stream, flags=flags)
         L_ = self._L
         L_.mhd_dist_config.argtypes = [C.c_void_p, C.c_int, C.c_int]
         L_.mhd_dist_phase.argtypes = [C.c_void_p, C.c_int, C.c_int]

@@ -78,6 +78,11 @@ def test_chunked_pipeline_sizes(lib):
     # the paper's scenario (512^3 on a 16 GB P100): fits a 16 GiB budget with everything on the host
     assert 0 < lib.mhd_workspace_bytes(512, OOC | STATE | WORK | (16384 << 8)) <= 16384 << 20
     assert lib.mhd_workspace_bytes(512, OOC | 0x80) == 0      # unknown flag bit
+    # per-rank storage of the slab decomposition (MHD_FLAG_RANKS(g) = (g - 1) << 4): 1/g of the state, 2/g of the work arrays
+    r8 = lib.mhd_workspace_bytes(1024, OOC | (7 << 4))
+    assert (16 * compact + 2 * 16 * zfull) / 8 < r8 < (16 * compact + 2 * 16 * zfull) / 8 * 1.1 + 12e9 and r8 < all_dev / 3
+    assert lib.mhd_workspace_bytes(1024, OOC | STATE | (7 << 4)) == 0     # per-rank storage lives in HBM
+    assert lib.mhd_workspace_bytes(1024, (7 << 4)) == 0                   # needs the chunked pipeline
     assert lib.mhd_workspace_bytes(512, STATE) == 0           # placement without the chunked pipeline
 
 

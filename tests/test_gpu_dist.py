@@ -21,18 +21,23 @@ def mods():
     return binding, dist
 
 
-def make_ranks(dist, cfg, world, dt=None):
-    return dist.Lockstep([dist.DistMHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, dt or cfg.dt, rank=r, world=world)
-                          for r in range(world)])
+def make_ranks(dist, cfg, world, dt=None, per_rank=False):
+    return dist.Lockstep([dist.DistMHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, dt or cfg.dt, rank=r, world=world,
+                                       per_rank_storage=per_rank) for r in range(world)])
 
 
+@pytest.mark.parametrize("per_rank", [False, True])
 @pytest.mark.parametrize("N,world", [(32, 2), (32, 3), (64, 4), (128, 8), (64, 7)])
-def test_decomposed_step_is_bitwise_the_single_gpu_step(mods, N, world):
+def test_decomposed_step_is_bitwise_the_single_gpu_step(mods, N, world, per_rank):
+    """per_rank: MHD_FLAG_RANKS — every rank allocates only its share (brick- and slab-shaped work arrays)."""
     binding, dist = mods
     cfg = inputs.config3(N, kmax=4) if N >= 64 else inputs.config2(N)
     ref = binding.MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, flags=binding.MHD_FLAG_OUT_OF_CORE)
     ref.set_fields(cfg.prim, "primitive")
-    grp = make_ranks(dist, cfg, world)
+    grp = make_ranks(dist, cfg, world, per_rank=per_rank)
+    if per_rank:
+        full = binding.MHD(cfg.N, flags=binding.MHD_FLAG_OUT_OF_CORE).workspace_bytes
+        assert grp.ranks[0].workspace_bytes < full * (3.0 / world + 0.35)      # 1/G state + 2/G work + staging
     grp.set_fields(cfg.prim, "primitive")
     U0r, U0g = ref.get_fields(), grp.get_fields()
     for f in range(8):
@@ -110,8 +115,9 @@ def test_decomposed_context_refuses_the_undecomposed_calls(mods):
     assert rc == -1
 
 
+@pytest.mark.parametrize("per_rank", [False, True])
 @pytest.mark.parametrize("N,world", [(32, 2), (64, 3), (128, 8), (64, 5)])
-def test_direct_exchange_is_bitwise_too(mods, N, world):
+def test_direct_exchange_is_bitwise_too(mods, N, world, per_rank):
     """mhd_dist_peers: the z passes and the forward y pass store every row straight into its owner's workspace (what
     P2P stores over NVLink do between GPUs; here the virtual ranks share one GPU's address space): no pack, no
     collective, no unpack — and still the bits of the undecomposed step."""
@@ -119,7 +125,7 @@ def test_direct_exchange_is_bitwise_too(mods, N, world):
     cfg = inputs.config3(N, kmax=4) if N >= 64 else inputs.config2(N)
     ref = binding.MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, flags=binding.MHD_FLAG_OUT_OF_CORE)
     ref.set_fields(cfg.prim, "primitive")
-    grp = make_ranks(dist, cfg, world)
+    grp = make_ranks(dist, cfg, world, per_rank=per_rank)
     grp.connect_peers()
     assert all(r.direct for r in grp.ranks)
     grp.set_fields(cfg.prim, "primitive")
@@ -145,7 +151,8 @@ dist.init_process_group("gloo")                      # host-side barriers and ha
 rank, world = dist.get_rank(), dist.get_world_size()
 torch.cuda.set_device(0)                             # both processes on the one GPU: CUDA IPC maps the peer's workspace
 cfg = inputs.config2(32)
-g = D.DistMHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, rank=rank, world=world, device="cuda:0")
+g = D.DistMHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, rank=rank, world=world, device="cuda:0",
+              per_rank_storage=True)
 g.connect_peers_ipc()
 assert g.direct
 # set / get use the packed exchange: gloo all_to_all_single needs host tensors, so route it through the host here
