@@ -266,6 +266,39 @@ def test_config4_as_specified_100_steps_diagnostics_every_10(orc, MHD):
             assert abs(s256[i][k] - do[k]) <= 1e-11 * abs(do[k]), (i, k)
 
 
+def _golden_runs():
+    import json, os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "long_runs.txt")
+    return [json.loads(line) for line in open(path) if line.startswith("{")]
+
+
+@pytest.mark.parametrize("name", ["config3", "config4"])
+def test_full_length_runs_against_stored_oracle_states(MHD, name):
+    """BASELINE.json config 3 (128^3, all 500 steps) and config 4 (256^3, all 100 steps) against the oracle's end state
+    stored by tests/golden/make_golden.py (oracle/ only; ~1 h of CPU): field norms, 48 sampled points per field and the
+    diagnostics, to north_star's 1e-9 (relative to the field's own scale)."""
+    recs = [r for r in _golden_runs() if r["name"] == name]
+    if not recs:
+        pytest.skip("no stored oracle state for " + name)
+    r = recs[0]
+    cfg = inputs.by_name(r["config"], r["N"])
+    assert cfg.dt == r["dt"]
+    g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+    g.set_fields(cfg.prim, "primitive")
+    g.step(r["steps"])
+    U = g.get_fields("conservative")
+    N = r["N"]
+    scale_all = max(r["norms"])
+    for f in range(8):
+        rms = r["norms"][f] / N ** 1.5
+        assert abs(np.linalg.norm(U[f]) - r["norms"][f]) <= 1e-9 * max(r["norms"][f], 1e-6 * scale_all), NAMES[f]
+        got = np.array([U[f][z, y, x] for (z, y, x) in r["points"]])
+        assert np.max(np.abs(got - np.array(r["samples"][f]))) <= 1e-9 * max(rms, 1e-6 * scale_all / N ** 1.5), NAMES[f]
+    d = g.diagnostics()
+    for k, v in r["diag"].items():
+        assert abs(d[k] - v) <= 1e-10 * abs(v), k
+
+
 def test_step_split_is_bitwise_and_step0_is_noop(orc, MHD):
     cfg = inputs.config1(32)
     _, g1 = both(orc, MHD, cfg)

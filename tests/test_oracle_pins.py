@@ -511,3 +511,24 @@ def test_p15_step_split_and_integrator_switch(orc):
     o2.step(1); o2.step(3)
     for a, b in zip(o1.get_fields(), o2.get_fields()):
         assert np.array_equal(a, b)
+
+
+def test_golden_file_is_the_oracles(orc):
+    """tests/golden/long_runs.txt (written by tests/golden/make_golden.py from oracle/ alone) cannot drift from the oracle:
+    the stored diagnostics after the first 10 steps of config 3 (128^3) are re-derived here."""
+    import json, os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "long_runs.txt")
+    if not os.path.exists(path):
+        pytest.skip("golden file not generated")
+    recs = [json.loads(line) for line in open(path) if line.startswith("{")]
+    r = [x for x in recs if x["name"] == "config3"]
+    if not r:
+        pytest.skip("config3 not stored")
+    r = r[0]
+    cfg = inputs.by_name(r["config"], r["N"])
+    o = orc.Oracle(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+    o.set_fields(cfg.prim, "primitive")
+    o.step(10)
+    d = o.diagnostics()
+    for k, v in r["diag_after_10"].items():
+        assert abs(d[k] - v) <= 1e-13 * abs(v), k   # same code, same inputs (bitwise on the same libm)
