@@ -194,8 +194,7 @@ void gen_pass(mhd_ctx* c, int dir, int nf, const cd* const in[], cd* const out[]
     a.out_row_stride = ors; a.out_outer_stride = oos; a.out_rows = out_rows;
     a.n_outer = n_outer; a.outer_split = n_outer; a.outer_skip = 0;
     a.ncols = c->kc() + 1;
-    const int C = c->N >= 1024 ? 4 : 8;
-    a.nchunks = (a.ncols + C - 1) / C;
+    a.cols = c->opt_strided_cols;
     a.jfirst = jfirst; a.bfirst = bfirst; a.outer_compact = 1; a.outer_base = outer_base; a.k0 = 2.0 * M_PI / c->L;
     const Ooc& o = c->ooc;
     if (peer_rows && o.direct_active && o.world > 1) {
