@@ -416,7 +416,11 @@ def run_ours(args):
         tpath = os.path.join(ROOT, "profiles", "traffic_r01.json")
         if os.path.exists(tpath):   # DRAM bytes per launch from the committed ncu --set full capture
             try:
-                roofline["traffic"] = json.load(open(tpath)).get(str(N), {}).get(dom)
+                tr = json.load(open(tpath)).get(str(N), {})
+                roofline["traffic"] = tr.get(dom)
+                if not flags and all(k in tr for k in fam):
+                    # measured DRAM bytes of one whole step (ncu) beside the algorithmic bytes
+                    roofline["whole_step"]["dram_bytes_measured_ncu"] = sum(tr[k] * fam[k]["launches_per_step"] for k in fam)
             except Exception:
                 pass
         if dom == "x_fused" and N in X_FUSED_FP64_INSTR_PER_LINE and not flags:
