@@ -303,7 +303,11 @@ def run_ours(args):
     dist = None
     if world > 1:
         import torch.distributed as dist_mod
-        dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        backend = os.environ.get("MHD_BENCH_BACKEND", "nccl")      # "gloo": several ranks on ONE GPU in the tests
+        if backend == "nccl":
+            dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        else:
+            dist_mod.init_process_group(backend)
         dist = dist_mod
     from paper_1810_12707_b200 import build as mhd_build
     if rank == 0:

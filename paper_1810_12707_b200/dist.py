@@ -217,8 +217,15 @@ class DistMHD(B.MHD):
         send, send_counts, recv_counts = self.pack(direction, nf)
         n = sum(recv_counts)
         recv = self.torch.empty(max(n, 1), dtype=self.torch.float64, device=self.device)[:n]
-        with self.torch.cuda.stream(self.stream):
-            all_to_all(recv, send, recv_counts, send_counts, self.group)
+        import torch.distributed as dist
+        if dist.get_backend(self.group) == "gloo":        # gloo moves host tensors (tests; NCCL is the production backend)
+            self.stream.synchronize()
+            host = self.torch.empty(n, dtype=self.torch.float64)
+            all_to_all(host, send.cpu(), recv_counts, send_counts, self.group)
+            recv.copy_(host)
+        else:
+            with self.torch.cuda.stream(self.stream):
+                all_to_all(recv, send, recv_counts, send_counts, self.group)
         self.unpack(direction, nf, recv)
         self.exchanged_bytes += 8 * sum(send_counts)
 

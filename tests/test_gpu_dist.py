@@ -208,3 +208,41 @@ def test_direct_exchange_between_two_processes_over_cuda_ipc(mods, tmp_path):
         got = np.load(prefix + str(m["rank"]) + ".npy")
         for f in range(8):
             assert np.array_equal(got[f], Ur[f][za:zb]), (m["rank"], f)
+
+
+@pytest.mark.parametrize("mode", ["decompose", "decompose_packed", "replicas"])
+def test_bench_with_two_ranks_on_one_gpu(mods, mode):
+    """bench.py as the driver launches it for N = 2 (one process per rank, env RANK / WORLD_SIZE / MASTER_*), with both ranks
+    on the one GPU and gloo instead of NCCL (NCCL refuses two ranks on a device): the whole multi-rank flow — build on rank 0,
+    barriers, IPC peer mapping or packed exchange, max-over-ranks timing, one JSON line from rank 0."""
+    import json, os, socket, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
+    extra = {"decompose": ["--decompose"], "decompose_packed": ["--decompose", "--packed-exchange"], "replicas": []}[mode]
+    cmd = [sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--size", "128", "--steps", "4", "--warmup", "3",
+           "--no-cpu", "--no-fft", "--no-e2e"] + extra
+    procs = []
+    for rank in range(2):
+        env = dict(os.environ, RANK=str(rank), LOCAL_RANK="0", WORLD_SIZE="2", MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port),
+                   MHD_BENCH_BACKEND="gloo")
+        procs.append(subprocess.Popen(cmd, env=env, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True, cwd=root))
+    outs = []
+    for p in procs:
+        out, err = p.communicate(timeout=900)
+        assert p.returncode == 0, err[-3000:]
+        outs.append(out.strip())
+    assert outs[1] == ""                                   # only rank 0 prints
+    line = json.loads(outs[0].splitlines()[-1])
+    assert line["n_gpus"] == 2 and line["steps"] == 4 and line["value"] > 0
+    if mode == "replicas":
+        assert line["scaling"] == "weak" and line["config"]["parallelism"] == "replicas x2"
+        assert abs(line["value"] * line["ms_per_step"] * 1e-3 / (2 * 128 ** 3) - 1.0) < 1e-9       # whole-job work / max time
+    else:
+        assert line["scaling"] == "strong" and line["config"]["parallelism"] == "slab decomposition x2"
+        dec = line["out_of_core"]["decomposed"]
+        assert dec["world"] == 2 and ("direct" in dec["exchange"]) == (mode == "decompose")
+        assert abs(line["value"] * line["ms_per_step"] * 1e-3 / (128 ** 3) - 1.0) < 1e-9           # ONE problem over both ranks
+        if mode == "decompose_packed":
+            assert dec["sent_to_peers_bytes_per_step_per_rank"] > 0
+        else:
+            assert dec["sent_to_peers_bytes_per_step_per_rank"] == 0                                  # rows went by P2P stores
