@@ -56,7 +56,28 @@ def record(name):
             "samples": [[float(u[z, y, x]) for (z, y, x) in pts] for u in U]}
 
 
+def augment(rec):
+    """Adds the diagnostics after the first 2 steps (a cheap prefix for the CPU drift test) to an existing record."""
+    cfg = inputs.by_name(rec["config"], rec["N"])
+    o = oracle.Oracle(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+    o.set_fields(cfg.prim, "primitive")
+    o.step(2)
+    d = o.diagnostics()
+    rec["diag_after_2"] = {k: d[k] for k in ("ke", "me", "ie")}
+    return rec
+
+
 def main():
+    if sys.argv[1:2] == ["--augment"]:          # python tests/golden/make_golden.py --augment config3
+        recs = {}
+        for line in open(OUT):
+            if line.startswith("{"):
+                r = json.loads(line)
+                recs[r["name"]] = r
+        for n in sys.argv[2:]:
+            recs[n] = augment(recs[n])
+        write(recs)
+        return
     names = sys.argv[1:] or list(RUNS)
     have = {}
     if os.path.exists(OUT):
@@ -66,11 +87,15 @@ def main():
                 have[r["name"]] = r
     for n in names:
         have[n] = record(n)
-        with open(OUT, "w") as f:
-            f.write("# Oracle end states of full-length runs (tests/golden/make_golden.py; oracle/ only). Cite: BASELINE.json configs 3, 4;\n")
-            f.write("# SURVEY.md 8(d). One JSON record per line; floats are repr-exact.\n")
-            for k in sorted(have):
-                f.write(json.dumps(have[k]) + "\n")
+        write(have)
+
+
+def write(have):
+    with open(OUT, "w") as f:
+        f.write("# Oracle end states of full-length runs (tests/golden/make_golden.py; oracle/ only). Cite: BASELINE.json configs 3, 4;\n")
+        f.write("# SURVEY.md 8(d). One JSON record per line; floats are repr-exact.\n")
+        for k in sorted(have):
+            f.write(json.dumps(have[k]) + "\n")
 
 
 if __name__ == "__main__":
