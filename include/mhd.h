@@ -77,10 +77,6 @@ extern "C" {
 #define MHD_OPT_OOC_BRICK 5 /* chunked pipeline: largest number of ky columns per brick (0 = what the staging allows) */
 #define MHD_OPT_OOC_SLAB 6  /* chunked pipeline: largest number of z planes per slab  (0 = what the staging allows) */
 
-#define MHD_OPT_STRIDED_COLS 7 /* tuning: kx columns per CTA of the strided (y, z) passes, 0 = default, 4 / 8 / 16 */
-
-#define MHD_OPT_L2_SLAB 10 /* z planes per slab of the in-core L2 slab loop over sweeps S2-S4 (0 = whole volume per launch) */
-
 #define MHD_OPT_TRACER_SORT 11 /* re-sort the tracer storage by grid row every this many pushes (default 32; 0 = never):
                                   gather locality only, results do not depend on it (mhd_tracers_get returns id order) */
 
@@ -116,7 +112,8 @@ typedef struct {
     double p_min;      /* min P                                                                */
 } mhd_diag;
 
-/* Create a context.  N: power of two, 16 <= N <= 1024; L > 0; gamma > 1; mu, eta >= 0; dt > 0.
+/* Create a context.  N: power of two, 16 <= N <= 1024 (N = 8 is rejected: k_c = floor(8/3) = 2 leaves no usable band,
+ * DESIGN.md section 1); L > 0; gamma > 1; mu, eta >= 0; dt > 0.
  * (mu, eta are the normalised 1/Re, 1/Rm of PAPER.md L140-152.)  Does not touch the GPU. */
 int mhd_init(mhd_ctx **out, int N, double L, double gamma, double mu, double eta, double dt);
 
@@ -227,18 +224,8 @@ int mhd_dist_enable_peer_access(mhd_ctx *ctx, int peer_device);
 /* Bytes the chunked pipeline has copied host->device / device->host so far (0 for an in-core context). */
 int mhd_transfer_bytes(const mhd_ctx *ctx, long long *h2d, long long *d2h);
 
-/* Measurement helper for the bench (not part of the method): fp64 instructions per second of a register-only DFMA
- * kernel on the current device = the issue ceiling of the fp64 pipe ("measure it with an FMA
- * micro-benchmark"); flop/s of pure-FMA code is twice that. */
-int mhd_probe_fp64(mhd_ctx *ctx, double *instr_per_s);
-
 /* Number of kernels this context has launched so far (for the bench's gpu_launches claim). */
 long long mhd_launch_count(const mhd_ctx *ctx);
-/* Milliseconds and launches accumulated per kernel family since the last reset; names[i] are static strings.
- * Timing uses CUDA events on the bound stream and is only collected while enabled (adds synchronisation). */
-int mhd_profile_enable(mhd_ctx *ctx, int on);
-int mhd_profile_get(mhd_ctx *ctx, int max_entries, const char **names, double *ms, long long *launches);
-
 const char *mhd_last_error(const mhd_ctx *ctx);
 int mhd_destroy(mhd_ctx *ctx);
 

@@ -15,69 +15,71 @@
 // a uniform field to be reproduced); T2 Eq. 21 is followed as printed (pure magnetic rotation, no electric field:
 // "the time evolution of the tracers are fully governed by the magnetic fields", L241); T3 the initial velocity is
 // the CIC interpolation of u = m/rho (L241 "evaluated from the velocity at the grid"); T4 positions are stored in
-// [0, L), the cell index is floor(x N/L) evaluated in fp64.
+// [0, L), the cell index is floor(x / dx) evaluated in fp64.
+// Written from the definitions (weights as cloud overlap with minimum-image distances, wrap by fmod) and kept
+// deliberately unlike csrc/tracers.cu, so that GPU-vs-oracle parity can catch a misreading on either side.
 // Everything is fp64 (the particle arithmetic is the paper's, Table I "double").
 #pragma once
+#include <algorithm>
 #include <cmath>
 #include <cstdint>
 
 namespace orc {
 
-struct Cell {           // step 1: corner indices (periodic) and the fractional position inside the cell
-    int i0[3], i1[3];
-    double f[3];
-};
-
-inline Cell locate(int N, double L, const double x[3]) {
-    Cell c;
-    const double inv_dx = double(N) / L;
-    for (int a = 0; a < 3; ++a) {
-        const double s = x[a] * inv_dx;
-        const double fl = std::floor(s);
-        c.f[a] = s - fl;
-        long long i = (long long)fl % N;
-        if (i < 0) i += N;
-        c.i0[a] = int(i);
-        c.i1[a] = int((i + 1) % N);
-    }
-    return c;
+// minimum-image separation of two points on the periodic axis of length L: the representative of a - b in [-L/2, L/2]
+inline double min_image(double a, double b, double L) {
+    double d = std::fmod(a - b, L);
+    if (d > 0.5 * L) d -= L;
+    if (d < -0.5 * L) d += L;
+    return d;
 }
 
-// step 2, Eq. 20 for one scalar grid field g[z][y][x]
-inline double cic(int N, const double* g, const Cell& c) {
-    const double fx = c.f[0], fy = c.f[1], fz = c.f[2];
-    auto at = [&](int ix, int iy, int iz) { return g[(std::int64_t(iz) * N + iy) * N + ix]; };
+// steps 1-2, Eq. 20 for one scalar grid field g[z][y][x], written from the definition of cloud-in-cell weighting: the
+// particle is a uniform cloud of the size of one cell, and a grid point receives the fraction of the cloud that
+// overlaps its own cell, i.e. prod_axis max(0, 1 - |x_p - x_grid| / dx) with the periodic (minimum-image) distance.
+// Only the grid points of the unit cell that holds the particle can have non-zero weight (step 1: its
+// bottom-left-front corner is floor(x_p / dx), L249); they are visited corner by corner.
+inline double cic(int N, double L, const double* g, const double x[3]) {
+    const double dx = L / double(N);
+    long long corner[3];
+    for (int a = 0; a < 3; ++a) corner[a] = (long long)std::floor(x[a] / dx);
     double b = 0.0;
-    b += at(c.i0[0], c.i0[1], c.i0[2]) * ((1.0 - fx) * (1.0 - fy) * (1.0 - fz));
-    b += at(c.i1[0], c.i0[1], c.i0[2]) * (fx * (1.0 - fy) * (1.0 - fz));
-    b += at(c.i0[0], c.i1[1], c.i0[2]) * ((1.0 - fx) * fy * (1.0 - fz));
-    b += at(c.i1[0], c.i1[1], c.i0[2]) * (fx * fy * (1.0 - fz));
-    b += at(c.i0[0], c.i0[1], c.i1[2]) * ((1.0 - fx) * (1.0 - fy) * fz);
-    b += at(c.i1[0], c.i0[1], c.i1[2]) * (fx * (1.0 - fy) * fz);
-    b += at(c.i0[0], c.i1[1], c.i1[2]) * ((1.0 - fx) * fy * fz);
-    b += at(c.i1[0], c.i1[1], c.i1[2]) * (fx * fy * fz);
+    for (int oz = 0; oz <= 1; ++oz)
+        for (int oy = 0; oy <= 1; ++oy)
+            for (int ox = 0; ox <= 1; ++ox) {
+                const int off[3] = {ox, oy, oz};
+                long long idx[3];
+                double w = 1.0;
+                for (int a = 0; a < 3; ++a) {
+                    idx[a] = ((corner[a] + off[a]) % N + N) % N;                 // periodic wrap of the grid index (L255)
+                    const double sep = std::fabs(min_image(x[a], double(idx[a]) * dx, L)) / dx;
+                    w *= std::max(0.0, 1.0 - sep);
+                }
+                b += w * g[(std::int64_t(idx[2]) * N + idx[1]) * N + idx[0]];
+            }
     return b;
 }
 
-// step 3, Eq. 21 (q = M = 1)
+// step 3, Eq. 21 (q = M = 1), with the vector algebra spelled out through a cross-product helper
+inline void cross(const double a[3], const double b[3], double out[3]) {
+    for (int c = 0; c < 3; ++c) out[c] = a[(c + 1) % 3] * b[(c + 2) % 3] - a[(c + 2) % 3] * b[(c + 1) % 3];
+}
 inline void boris(const double Bp[3], double dt, double v[3]) {
-    const double t[3] = {Bp[0] * (dt / 2.0), Bp[1] * (dt / 2.0), Bp[2] * (dt / 2.0)};
-    const double t2 = t[0] * t[0] + t[1] * t[1] + t[2] * t[2];
-    const double s[3] = {2.0 * t[0] / (1.0 + t2), 2.0 * t[1] / (1.0 + t2), 2.0 * t[2] / (1.0 + t2)};
-    const double vd[3] = {v[0] + (v[1] * t[2] - v[2] * t[1]),
-                          v[1] + (v[2] * t[0] - v[0] * t[2]),
-                          v[2] + (v[0] * t[1] - v[1] * t[0])};
-    const double vn[3] = {v[0] + (vd[1] * s[2] - vd[2] * s[1]),
-                          v[1] + (vd[2] * s[0] - vd[0] * s[2]),
-                          v[2] + (vd[0] * s[1] - vd[1] * s[0])};
-    v[0] = vn[0]; v[1] = vn[1]; v[2] = vn[2];
+    double t[3], s[3], vxt[3], vd[3], vdxs[3];
+    double t2 = 0.0;
+    for (int c = 0; c < 3; ++c) { t[c] = 0.5 * dt * Bp[c]; t2 += t[c] * t[c]; }      // t = q B dt / 2M
+    for (int c = 0; c < 3; ++c) s[c] = 2.0 * t[c] / (1.0 + t2);                       // s = 2 t / (1 + t^2)
+    cross(v, t, vxt);
+    for (int c = 0; c < 3; ++c) vd[c] = v[c] + vxt[c];                                // v_d = v_t + v_t x t
+    cross(vd, s, vdxs);
+    for (int c = 0; c < 3; ++c) v[c] += vdxs[c];                                      // v_{t+dt} = v_t + v_d x s
 }
 
+// Eq. 22 periodic wrap: the representative of x in [0, L)
 inline double wrap(double x, double L) {
-    x -= L * std::floor(x / L);
-    if (x >= L) x -= L;      // x = -tiny gives L after rounding
-    if (x < 0.0) x = 0.0;
-    return x;
+    double r = std::fmod(x, L);          // exact; sign of x
+    if (r < 0.0) r += L;                 // may round to L when r = -tiny
+    return r < L ? r : 0.0;              // L is the same point as 0
 }
 
 // steps 1-4 for np particles; B[c] are the three grid components; pos[c], vel[c] are updated in place
@@ -85,8 +87,7 @@ inline void tracers_push(int N, double L, double dt, const double* const B[3], l
                          double* const vel[3]) {
     for (long long m = 0; m < np; ++m) {
         const double x[3] = {pos[0][m], pos[1][m], pos[2][m]};
-        const Cell c = locate(N, L, x);
-        const double Bp[3] = {cic(N, B[0], c), cic(N, B[1], c), cic(N, B[2], c)};
+        const double Bp[3] = {cic(N, L, B[0], x), cic(N, L, B[1], x), cic(N, L, B[2], x)};
         double v[3] = {vel[0][m], vel[1][m], vel[2][m]};
         boris(Bp, dt, v);
         for (int a = 0; a < 3; ++a) {
@@ -101,8 +102,7 @@ inline void tracers_interp(int N, double L, int nf, const double* const g[], lon
                            double* const out[]) {
     for (long long m = 0; m < np; ++m) {
         const double x[3] = {pos[0][m], pos[1][m], pos[2][m]};
-        const Cell c = locate(N, L, x);
-        for (int f = 0; f < nf; ++f) out[f][m] = cic(N, g[f], c);
+        for (int f = 0; f < nf; ++f) out[f][m] = cic(N, L, g[f], x);
     }
 }
 

@@ -175,7 +175,20 @@ class MHD:
         torch = self.torch
         shape = (self.N,) * 3
         if out is not None:
-            return self._marshal(out)[1], out
+            # the library writes through these pointers: a silently made contiguous / float64 copy would receive the
+            # result instead of the caller's arrays, so outputs must already be C-contiguous float64 in the right place
+            for f in out:
+                if isinstance(f, np.ndarray):
+                    ok = f.dtype == np.float64 and f.flags["C_CONTIGUOUS"] and f.flags["WRITEABLE"]
+                else:
+                    ok = f.dtype == torch.float64 and f.is_contiguous()
+                if not ok:
+                    raise ValueError("output fields must be C-contiguous float64 arrays")
+            w, ptrs, _ = self._marshal(out)
+            if w != where:
+                raise ValueError("output arrays live on the %s but where=%s was requested"
+                                 % ("host" if w == MHD_HOST else "device", "host" if where == MHD_HOST else "device"))
+            return ptrs, out
         if where == MHD_HOST:
             arrs = [np.empty(shape, dtype=np.float64) for _ in range(8)]
             return _ptr_array([a.ctypes.data for a in arrs]), arrs

@@ -25,7 +25,8 @@ def sources():
 
 def deps():
     d = [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
-    d.append(os.path.join(os.path.dirname(HERE), "include", "mhd.h"))
+    inc = os.path.join(os.path.dirname(HERE), "include")
+    d += [os.path.join(inc, f) for f in os.listdir(inc) if f.endswith(".h")]
     return d
 
 

@@ -1,6 +1,7 @@
 // ctx.h — the solver context behind the opaque mhd_ctx of include/mhd.h (internal to libmhd).
 #pragma once
 #include "../../include/mhd.h"
+#include "../../include/mhd_bench.h"
 #include "kernels.h"
 
 #include <algorithm>
@@ -54,7 +55,7 @@ struct mhd_ctx {
     bool bound = false, have_fields = false, have_old = false;
     cudaStream_t st = nullptr;
     unsigned flags = 0;
-    int opt_fused = 1, opt_prune = 1, opt_fuse_current = 1, integrator = 0, opt_strided_cols = 0, opt_slab = 0, opt_stress = 0;
+    int opt_fused = 1, opt_prune = 1, opt_fuse_current = 1, integrator = 0, opt_stress = 0;
     long long step = 0;
     long long launches = 0;
     std::string err;

@@ -8,6 +8,18 @@ namespace mhd {
 typedef double2 cd;
 constexpr int MAXF = 16;   // largest batch of fields one launch handles
 
+// Opt-in to more than 48 KB of dynamic shared memory, once per kernel instantiation AND per device (the attribute is a
+// per-device property of the function: a process that drives several GPUs must set it on each of them).
+template <class K> inline void ensure_dynamic_smem(K kern, size_t smem) {
+    constexpr int MAX_DEV = 64;
+    static bool done[MAX_DEV] = {};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev >= 0 && dev < MAX_DEV && done[dev]) return;
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (dev >= 0 && dev < MAX_DEV) done[dev] = true;
+}
+
 // Physical constants of one context, passed by value to the point-wise kernels.
 struct Phys {
     double k0;       // 2*pi/L : wavenumber of integer mode 1
@@ -33,7 +45,6 @@ struct StridedArgs {
     long long in_row_stride, out_row_stride;      // complex elements between consecutive stored rows
     long long in_outer_stride, out_outer_stride;  // complex elements between consecutive outer indices
     int nchunks;           // (computed by the launcher from ncols and the columns per CTA)
-    int cols;              // columns per CTA: 0 = default for N (8; 4 at N = 1024); 4 / 16 = tuning variants (in-core path)
     int ncols;             // valid columns (guards the last chunk)
     int n_outer;           // number of outer indices processed
     int outer_split;       // in-core: outer index o maps to o (o < split) or o + outer_skip

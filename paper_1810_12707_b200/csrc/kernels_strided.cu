@@ -118,11 +118,7 @@ strided_kernel(const __grid_constant__ StridedArgs a) {
 template <int N, int DIR, int C, bool GEN, bool FJ> static void launch_one(const StridedArgs& a, cudaStream_t st) {
     constexpr int threads = C * PlanInfo<N>::T;
     constexpr size_t smem = size_t(N) * C * sizeof(cd);
-    static bool configured = false;
-    if (!configured) {
-        cudaFuncSetAttribute(strided_kernel<N, DIR, C, GEN, FJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        configured = true;
-    }
+    ensure_dynamic_smem(strided_kernel<N, DIR, C, GEN, FJ>, smem);
     dim3 grid((a.ncols + C - 1) / C, a.n_outer, a.nfields);
     if (FJ) grid = dim3(grid.x * a.nfields, a.n_outer, 1);
     strided_kernel<N, DIR, C, GEN, FJ><<<grid, threads, smem, st>>>(a);
@@ -143,19 +139,12 @@ void launch_strided(int N, int dir, const StridedArgs& a, cudaStream_t st) {
         case 32: launch_dir<32, 8>(dir, a, st); break;
         case 64: launch_dir<64, 8>(dir, a, st); break;
         case 128: launch_dir<128, 8>(dir, a, st); break;
-        case 256:
-            if (a.cols == 4 && !a.general) launch_dir<256, 4>(dir, a, st);
-            else if (a.cols == 16 && !a.general) launch_dir<256, 16>(dir, a, st);
-            else launch_dir<256, 8>(dir, a, st);
-            break;
-        case 512:
-            if (a.cols == 4 && !a.general) launch_dir<512, 4>(dir, a, st);
-            else launch_dir<512, 8>(dir, a, st);
-            break;
+        case 256: launch_dir<256, 8>(dir, a, st); break;
+        case 512: launch_dir<512, 8>(dir, a, st); break;
         case 1024:
             // measured at 1024^3 (chunked pipeline in HBM): the write-heavy inverse passes gain 13 % from 128-byte segments
             // (8 columns, one 128 KB tile per SM), the forward passes lose 2 %: 8 columns for the inverse, 4 for the forward
-            if (a.cols == 8 || (a.cols == 0 && dir > 0)) launch_dir<1024, 8>(dir, a, st);
+            if (dir > 0) launch_dir<1024, 8>(dir, a, st);
             else launch_dir<1024, 4>(dir, a, st);
             break;
         default: break;

@@ -196,27 +196,21 @@ __global__ void __launch_bounds__(XCfg<N, 16>::THREADS) x_fused_kernel(const __g
 // ---------------------------------------------------------------------------------------------------------
 // launchers
 // ---------------------------------------------------------------------------------------------------------
-template <class K> static void set_smem(K kern, size_t smem) {
-    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-}
 
 template <int N> static void r2c_one(const XArgs& a, cudaStream_t st) {
     constexpr int SL = 8;
-    static bool cfg = false;
-    if (!cfg) { set_smem(x_r2c_kernel<N, SL>, XCfg<N, SL>::SMEM); cfg = true; }
+    ensure_dynamic_smem(x_r2c_kernel<N, SL>, XCfg<N, SL>::SMEM);
     dim3 grid((unsigned)(a.nlines / SL), a.nfields);
     x_r2c_kernel<N, SL><<<grid, XCfg<N, SL>::THREADS, XCfg<N, SL>::SMEM, st>>>(a);
 }
 template <int N> static void c2r_one(const XArgs& a, cudaStream_t st) {
     constexpr int SL = 8;
-    static bool cfg = false;
-    if (!cfg) { set_smem(x_c2r_kernel<N, SL>, XCfg<N, SL>::SMEM); cfg = true; }
+    ensure_dynamic_smem(x_c2r_kernel<N, SL>, XCfg<N, SL>::SMEM);
     dim3 grid((unsigned)(a.nlines / SL), a.nfields);
     x_c2r_kernel<N, SL><<<grid, XCfg<N, SL>::THREADS, XCfg<N, SL>::SMEM, st>>>(a);
 }
 template <int N> static void fused_one(const FusedXArgs& a, cudaStream_t st) {
-    static bool cfg = false;
-    if (!cfg) { set_smem(x_fused_kernel<N>, XCfg<N, 16>::SMEM); cfg = true; }
+    ensure_dynamic_smem(x_fused_kernel<N>, XCfg<N, 16>::SMEM);
     x_fused_kernel<N><<<(unsigned)a.nlines, XCfg<N, 16>::THREADS, XCfg<N, 16>::SMEM, st>>>(a);
 }
 

@@ -267,11 +267,7 @@ x_fused2_kernel(const __grid_constant__ FusedXArgs a) {
 
 template <int N> static void fused2_one(const FusedXArgs& a, cudaStream_t st) {
     typedef F2<N / 2> P;
-    static bool cfg = false;
-    if (!cfg) {
-        cudaFuncSetAttribute(x_fused2_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::SMEM);
-        cfg = true;
-    }
+    ensure_dynamic_smem(x_fused2_kernel<N>, P::SMEM);
     x_fused2_kernel<N><<<(unsigned)a.nlines, P::THREADS, P::SMEM, st>>>(a);
 }
 

@@ -32,7 +32,6 @@ void strided_pass(mhd_ctx* c, int dir, int axis, int nf, const cd* const in[], c
         a.nfields = nb;
         a.jfirst = jfirst; a.bfirst = bfirst; a.k0 = 2.0 * M_PI / c->L;   // fused current: only with nf <= MAXF
         a.ncols = prune ? std::min(kc + 1, ncols_full) : ncols_full;
-        a.cols = c->opt_strided_cols;
         if (axis == 1) {            // y pass: rows along y, outer = z (all planes)
             a.in_row_stride = a.out_row_stride = hx; a.in_outer_stride = a.out_outer_stride = (long long)N * hx;
             a.n_outer = nz > 0 ? nz : N; a.outer_split = N; a.outer_skip = 0;
@@ -134,12 +133,11 @@ void products(mhd_ctx* c, cd* const Uin[8], double* const breal[3] = nullptr) {
         }
         strided_pass(c, +1, 2, 11, in, c->W, c->hx(), c->hx(), prune);    // S1b
     }
-    // S2-S4 work inside z planes.  They run slab after slab (a few planes at a time) so that what the inverse y pass
-    // writes is still in the 126 MB L2 when the fused x sweep reads it, and what that writes when the forward y pass reads
-    // it: the 27 intermediate field sweeps between S1 and S5 then never reach HBM.
+    // S2-S4 work inside z planes; one launch per sweep over the whole volume (a slab-after-slab loop that keeps the
+    // intermediates in L2 measured slower at every slab size: DESIGN.md "L2 slab loop")
     const int kmax = prune ? c->kc() : c->hx() - 1;
     const double scale = 1.0 / ((double)N * N * N);
-    const int slab = (c->opt_fused && c->opt_slab > 0) ? std::min(c->opt_slab, N) : N;
+    const int slab = N;
     for (int z0 = 0; z0 < N; z0 += slab) {
         const int nz = std::min(slab, N - z0);
         strided_pass(c, +1, 1, 11, c->W, c->W, c->hx(), c->hx(), prune, -1, 0, z0, nz);      // S2
@@ -326,6 +324,8 @@ int mhd_bind(mhd_ctx* c, void* dev_workspace, size_t bytes, void* cuda_stream, u
              size_t pinned_bytes) {
     if (!c) return MHD_ERR_INVALID_ARG;
     if (!flags_valid(flags)) return c->fail(MHD_ERR_INVALID_ARG, "invalid flags");
+    if ((flags & MHD_FLAG_OUT_OF_CORE) && (c->f0 != 0.0 || c->opt_stress))     // set before binding: refuse here, not silently later
+        return c->fail(MHD_ERR_INVALID_ARG, "forcing / the stress-tensor variant were set: they need an in-core context");
     if (!dev_workspace || ((uintptr_t)dev_workspace & 255) != 0) return c->fail(MHD_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
     const Layout l = make_layout(c->N);
     if (!(flags & MHD_FLAG_OUT_OF_CORE) && bytes < l.total) return c->fail(MHD_ERR_NOMEM, "workspace too small");
@@ -377,12 +377,6 @@ int mhd_set_option(mhd_ctx* c, int option, int value) {
         case MHD_OPT_INTEGRATOR:
             if (value < 0 || value > 2) return c->fail(MHD_ERR_INVALID_ARG, "integrator must be 0, 1 or 2");
             c->integrator = value; c->have_old = false; return MHD_OK;
-        case MHD_OPT_STRIDED_COLS:
-            if (value != 0 && value != 4 && value != 8 && value != 16) return c->fail(MHD_ERR_INVALID_ARG, "strided columns must be 0, 4, 8 or 16");
-            c->opt_strided_cols = value; return MHD_OK;
-        case MHD_OPT_L2_SLAB:
-            if (value < 0) return c->fail(MHD_ERR_INVALID_ARG, "slab planes must be >= 0");
-            c->opt_slab = value; return MHD_OK;
         case MHD_OPT_TRACER_SORT:
             if (value < 0) return c->fail(MHD_ERR_INVALID_ARG, "tracer sort interval must be >= 0");
             c->opt_tracer_sort = value; return MHD_OK;

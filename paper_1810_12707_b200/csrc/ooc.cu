@@ -194,7 +194,6 @@ void gen_pass(mhd_ctx* c, int dir, int nf, const cd* const in[], cd* const out[]
     a.out_row_stride = ors; a.out_outer_stride = oos; a.out_rows = out_rows;
     a.n_outer = n_outer; a.outer_split = n_outer; a.outer_skip = 0;
     a.ncols = c->kc() + 1;
-    a.cols = c->opt_strided_cols;
     a.jfirst = jfirst; a.bfirst = bfirst; a.outer_compact = 1; a.outer_base = outer_base; a.k0 = 2.0 * M_PI / c->L;
     const Ooc& o = c->ooc;
     if (peer_rows && o.direct_active && o.world > 1) {
@@ -578,7 +577,10 @@ int ooc_set_fields(mhd_ctx* c, int kind, int where, const double* const f[8]) {
     SlabIO io; io.nin = 0; io.nout = 8; io.kind = kind; io.where = where; io.user_in = f;
     int rc = stage_slabs(c, SLAB_FROM_REAL, io);
     if (rc) return rc;
-    if (c->ooc.world > 1) return check_cuda(c, "set_fields (decomposed, slab part)");   // exchange, then MHD_DIST_PHASE_STORE
+    if (c->ooc.world > 1) {            // exchange, then MHD_DIST_PHASE_STORE
+        if (where == MHD_HOST) cudaStreamSynchronize(c->st);     // the caller's host buffers are free again on return
+        return check_cuda(c, "set_fields (decomposed, slab part)");
+    }
     rc = stage_forward_z_store(c);
     if (rc) return rc;
     if (where == MHD_HOST) cudaStreamSynchronize(c->st);
@@ -605,7 +607,16 @@ static int ooc_products(mhd_ctx* c, bool have_inverse_z = false) {
     return stage_slabs(c, SLAB_FLUX, io);
 }
 
+// the chunked pipeline implements the base equation set only: re-checked where the work is done, because the options can
+// be set before mhd_bind makes the context a chunked one
+static int ooc_variant_check(mhd_ctx* c) {
+    if (c->f0 != 0.0) return c->fail(MHD_ERR_INVALID_ARG, "forcing (MHD_PARAM_FORCE_AMP) needs an in-core context");
+    if (c->opt_stress) return c->fail(MHD_ERR_INVALID_ARG, "the stress-tensor variant (MHD_OPT_STRESS) needs an in-core context");
+    return MHD_OK;
+}
+
 int ooc_rhs(mhd_ctx* c, int where, double* const out[8]) {
+    if (int vrc = ooc_variant_check(c)) return vrc;
     if (c->ooc.world > 1) return c->fail(MHD_ERR_INVALID_ARG, "mhd_rhs is not available on a decomposed context");
     for (int i = 0; i < 8; ++i) if (!out[i]) return c->fail(MHD_ERR_INVALID_ARG, "null field pointer");
     int rc = ooc_products(c);
@@ -622,6 +633,7 @@ int ooc_rhs(mhd_ctx* c, int where, double* const out[8]) {
 int ooc_step(mhd_ctx* c, int nsteps) {
     if (c->ooc.world > 1) return c->fail(MHD_ERR_INVALID_ARG, "decomposed context: drive the step with mhd_dist_phase and the exchanges");
     if (c->integrator != 0) return c->fail(MHD_ERR_INVALID_ARG, "the chunked pipeline implements Adams-Bashforth only");
+    if (int vrc = ooc_variant_check(c)) return vrc;
     for (int s = 0; s < nsteps; ++s) {
         int rc = ooc_products(c, s > 0);
         if (rc) return rc;
@@ -706,6 +718,7 @@ static int dist_phase_body(mhd_ctx* c, int phase, int arg) {
         case MHD_DIST_PHASE_B: { SlabIO io; io.nin = 11; io.nout = 16; return stage_slabs(c, SLAB_FLUX, io); }
         case MHD_DIST_PHASE_C: {
             if (c->integrator != 0) return c->fail(MHD_ERR_INVALID_ARG, "the chunked pipeline implements Adams-Bashforth only");
+            if (int vrc = ooc_variant_check(c)) return vrc;
             int rc = stage_forward_z_assemble(c, c->have_old ? 2 : 1, arg != 0);
             if (rc) return rc;
             c->have_old = true; ++c->step;

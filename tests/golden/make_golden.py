@@ -57,13 +57,26 @@ def record(name):
 
 
 def augment(rec):
-    """Adds the diagnostics after the first 2 steps (a cheap prefix for the CPU drift test) to an existing record."""
+    """Adds a cheap prefix to an existing record, for the CPU drift test (tests/test_oracle_pins.py):
+    config3 (128^3): diagnostics and the first 8 sample points of every field after the first 2 steps;
+    config4 (256^3): the same after the first step, at 8 seeded points whose indices are multiples of 4 — the drift test
+    re-derives them on a 64^3 grid (after one Euler step every mode of config 4 is <= 12 <= k_c(64), so the two
+    resolutions agree at the shared grid points to roundoff)."""
     cfg = inputs.by_name(rec["config"], rec["N"])
     o = oracle.Oracle(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
     o.set_fields(cfg.prim, "primitive")
-    o.step(2)
+    if rec["name"] == "config4":
+        nst, key = 1, "after_1"
+        pts = (np.random.default_rng(4).integers(0, rec["N"] // 4, size=(8, 3)) * 4).tolist()
+    else:
+        nst, key = 2, "after_2"
+        pts = rec["points"][:8]
+    o.step(nst)
     d = o.diagnostics()
-    rec["diag_after_2"] = {k: d[k] for k in ("ke", "me", "ie")}
+    U = o.get_fields("conservative")
+    rec["diag_" + key] = {k: d[k] for k in ("ke", "me", "ie", "max_divb")}
+    rec["points_" + key] = pts
+    rec["samples_" + key] = [[float(u[z, y, x]) for (z, y, x) in pts] for u in U]
     return rec
 
 

@@ -1,5 +1,5 @@
-"""Host-side checks of the C ABI (no GPU needed): libmhd.so loads, exports every symbol include/mhd.h
-declares, validates its arguments and fails loudly without a device."""
+"""Host-side checks of the C ABI (no GPU needed): libmhd.so loads, exports every symbol include/*.h
+declare, validates its arguments and fails loudly without a device."""
 import ctypes as C
 import os
 import re
@@ -17,7 +17,8 @@ def lib():
 
 
 def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "mhd.h")).read()
+    inc = os.path.join(ROOT, "include")
+    text = "".join(open(os.path.join(inc, f)).read() for f in sorted(os.listdir(inc)) if f.endswith(".h"))
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(mhd_[a-z0-9_]+)\s*\(", text)))
 
@@ -84,6 +85,24 @@ def test_chunked_pipeline_sizes(lib):
     assert lib.mhd_workspace_bytes(1024, OOC | STATE | (7 << 4)) == 0     # per-rank storage lives in HBM
     assert lib.mhd_workspace_bytes(1024, (7 << 4)) == 0                   # needs the chunked pipeline
     assert lib.mhd_workspace_bytes(512, STATE) == 0           # placement without the chunked pipeline
+
+
+def test_variants_set_before_binding_are_refused_out_of_core(lib):
+    """The ABI allows mhd_init -> mhd_set_param / mhd_set_option -> mhd_bind(MHD_FLAG_OUT_OF_CORE): forcing and the
+    stress-tensor variant are in-core only and must be refused at bind time, not silently dropped."""
+    two_pi = 6.283185307179586
+    lib.mhd_set_param.argtypes = [C.c_void_p, C.c_int, C.c_double]
+    for setup in ("force", "stress"):
+        h = C.c_void_p()
+        assert lib.mhd_init(C.byref(h), 32, two_pi, 5 / 3, 0.01, 0.01, 1e-3) == 0
+        if setup == "force":
+            assert lib.mhd_set_param(h, 2, 0.25) == 0            # MHD_PARAM_FORCE_AMP
+        else:
+            assert lib.mhd_set_option(h, 12, 1) == 0             # MHD_OPT_STRESS
+        n = lib.mhd_workspace_bytes(32, 1)
+        assert lib.mhd_bind(h, C.c_void_p(256), n, None, 1, None, 0) == -1
+        assert b"in-core" in lib.mhd_last_error(h)
+        lib.mhd_destroy(h)
 
 
 def test_bind_without_device_fails_loudly(lib):

@@ -23,12 +23,13 @@ def rand_pos(n, rng, lo=0.0, hi=L):
 
 
 def test_tp1_weights_sum_to_one():
-    """Reading T1: a uniform field is reproduced exactly (to 1 ulp), wherever the particle sits."""
+    """Reading T1: a uniform field is reproduced wherever the particle sits.  The weights are formed from coordinate
+    differences |x_p - x_grid| / dx, each good to |x| eps / dx <= N eps, so their sum is 1 to a few N eps."""
     N = 16
     rng = np.random.default_rng(1)
     pos = rand_pos(1000, rng)
     out = oracle.cic([np.full((N, N, N), 3.25)], pos)[0]
-    assert np.max(np.abs(out - 3.25)) <= 4 * np.finfo(float).eps * 3.25
+    assert np.max(np.abs(out - 3.25)) <= 4 * N * np.finfo(float).eps * 3.25
 
 
 @pytest.mark.parametrize("axis", [0, 1, 2])
@@ -218,3 +219,49 @@ def test_tp10_time_varying_field_uses_start_of_step_B():
         assert np.array_equal(p1[c], p[c]) and np.array_equal(v1[c], v[c])
     # and the field did change (so that the order matters)
     assert abs(o.get_fields()[6].max() / b - 1.0) > 0.05
+
+
+def test_tp11_particle_on_a_cell_face_and_at_the_box_edge():
+    """Edge cases of Eq. 20 that a wrong cell index or weight-to-corner assignment gets wrong: a particle exactly on a grid
+    plane takes the value of that plane (weight 1, whichever of the two adjacent cells floor() picks); at x = L - 1 ulp it
+    feels plane 0 through the periodic wrap (L255) with weight 1 - O(ulp); at x = 0 it feels plane 0 only."""
+    N = 8
+    dx = L / N
+    ix, iy, iz = idx_grid(N)
+    g = 100.0 * iz + 10.0 * iy + ix                     # every grid point has its own value
+    # on the faces x = 3 dx, y = 5 dx, z = 2 dx simultaneously: exactly g[2, 5, 3]
+    out = oracle.cic([g], [np.array([3 * dx]), np.array([5 * dx]), np.array([2 * dx])])[0]
+    assert abs(out[0] - 253.0) <= 1e-12
+    # on one face only, half-way inside the cell on the other two axes: mean of the 4 corners of that face
+    out = oracle.cic([g], [np.array([3 * dx]), np.array([5.5 * dx]), np.array([2.5 * dx])])[0]
+    assert abs(out[0] - (3 + 10 * 5.5 + 100 * 2.5)) <= 1e-12
+    # x = L - 1 ulp: in the last cell, next to plane 0 of the opposite boundary
+    edge = np.nextafter(L, 0.0)
+    for axis in range(3):
+        pos = [np.array([0.0]) for _ in range(3)]
+        pos[axis] = np.array([edge])
+        out = oracle.cic([g], pos)[0]
+        assert abs(out[0] - 0.0) <= 1e-12 * 1000, axis          # g[0,0,0] = 0; plane N-1 (value 7, 70 or 700) has weight ~1e-16
+    out = oracle.cic([g], [np.array([0.0])] * 3)[0]
+    assert out[0] == 0.0
+
+
+def test_tp12_crossing_zero_with_negative_velocity():
+    """Eq. 22 + periodic wrap: a particle that leaves through x = 0 re-enters at x = L - |overshoot|; one that lands on
+    x = -tiny (which rounds to L after the shift) is stored as 0, never as L."""
+    N = 8
+    Z = [np.zeros((N, N, N)) for _ in range(3)]          # B = 0: straight-line motion
+    dt = 0.1
+    p, v = oracle.tracers_push(Z, [np.array([0.02]), np.array([1.0]), np.array([L - 0.01])],
+                               [np.array([-0.5]), np.array([0.0]), np.array([0.3])], dt, 1)
+    assert abs(p[0][0] - (L - 0.03)) <= 2e-15 * L and p[1][0] == 1.0 and abs(p[2][0] - 0.02) <= 2e-15 * L
+    tiny = 1e-20
+    p, v = oracle.tracers_push(Z, [np.array([0.0]), np.array([0.0]), np.array([0.0])],
+                               [np.array([-tiny / dt]), np.array([0.0]), np.array([0.0])], dt, 1)
+    assert p[0][0] == 0.0
+    # many box lengths in one push, both directions
+    p, v = oracle.tracers_push(Z, [np.array([1.0]), np.array([1.0]), np.array([1.0])],
+                               [np.array([-(5 * L + 0.25) / dt]), np.array([(7 * L + 0.5) / dt]), np.array([0.0])], dt, 1)
+    assert abs(p[0][0] - 0.75) <= 1e-13 and abs(p[1][0] - 1.5) <= 1e-13
+    for c in range(3):
+        assert 0.0 <= p[c][0] < L
