@@ -62,7 +62,7 @@ def check_rhs(o, g, N, literal=1e-12, beta_tol=2e-15):
 # ---------------------------------------------------------------------------------------------------------
 # 3-D FFT alone: in-house R2C / C2R against the oracle's own FFT
 # ---------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("N", [16, 32, 64, 128])
+@pytest.mark.parametrize("N", [16, 32, 64, 128, 256])
 def test_fft3d_matches_oracle(orc, MHD, N):
     import torch
     rng = np.random.default_rng(100 + N)
@@ -417,6 +417,30 @@ def test_diagnostics_match_oracle(orc, MHD, cfgname, N):
     assert abs(dg["spec_mag"].sum() - dg["me"]) <= 1e-12 * dg["me"]
 
 
+@pytest.mark.parametrize("N", [32, 64])
+def test_diagnostics_divb_and_momentum_values(orc, MHD, N):
+    """max|div B| and <m> as VALUES (oracle pins P16): a non-solenoidal B whose divergence has its extremum at a negative
+    value on the grid, non-uniform density and three distinct momenta — equal to the oracle's to 1e-12, and to the closed form."""
+    c = np.arange(N) * (2 * math.pi / N)
+    X, Y, Z = c[None, None, :], c[None, :, None], c[:, None, None]
+    shape = (N, N, N)
+    full = lambda a: np.ascontiguousarray(np.broadcast_to(np.asarray(a, dtype=np.float64), shape))
+    b0, k = 0.37, 2
+    rho = 1.5 + 0.5 * np.cos(X) + 0.25 * np.sin(2 * Y)
+    prim = [full(rho), full(0.2), full(-0.7), full(1.1), full(2.0),
+            full(-b0 * (np.sin(k * X) + 0.25 * np.sin(2 * k * X))), full(0.3 * np.sin(Y)), full(0.1 * np.sin(3 * Z))]
+    cfg = inputs.Config("divb", N, 2 * math.pi, 5 / 3, 0.0, 0.0, 1e-3, 1, prim)
+    o, g = both(orc, MHD, cfg)
+    do, dg = o.diagnostics(), g.diagnostics()
+    # div B = -b0 k (cos kx + cos 2kx / 2) + 0.3 cos y + 0.3 cos 3z: extremum at the origin's x with y = pi, z = pi/3-type points;
+    # the oracle value (pinned by P16 on the single-axis case) is the reference, the closed-form bound is a sanity check
+    assert abs(dg["max_divb"] - do["max_divb"]) <= 1e-12 * do["max_divb"]
+    assert 1.5 * b0 * k < dg["max_divb"] <= 1.5 * b0 * k + 0.6 + 1e-12
+    for a, b_, u in zip(do["mom"], dg["mom"], (0.2, -0.7, 1.1)):
+        assert abs(a - b_) <= 1e-13 and abs(b_ - 1.5 * u) <= 1e-13
+    assert abs(dg["mass"] - 1.5) <= 1e-13
+
+
 # ---------------------------------------------------------------------------------------------------------
 # error behaviour at the boundary
 # ---------------------------------------------------------------------------------------------------------
@@ -467,7 +491,7 @@ def test_full_size_rhs_against_oracle_subsampled(orc, MHD, N):
     assert abs(d0["ke"] - 1.5) <= 1e-12 and abs(d0["ie"] - 90.0) <= 1e-10 and abs(d0["me"] - 5e-9) <= 1e-20
 
 
-@pytest.mark.parametrize("N", [256])
+@pytest.mark.parametrize("N", [256, 512])
 def test_full_size_abc_closed_form(MHD, N):
     U0, P0, mu = 0.7, 2.0, 0.013
     c = np.arange(N) * (2 * math.pi / N)
@@ -491,6 +515,131 @@ def test_full_size_abc_closed_form(MHD, N):
     assert np.max(np.abs(R[4] - RE)) <= tol
     for i in range(3):
         assert np.max(np.abs(R[5 + i])) == 0.0
+
+
+# ---------------------------------------------------------------------------------------------------------
+# full-size 3-D transforms at EVERY mode / point (the oracle's FFT at 512^3 is not affordable): a sum of seeded plane
+# waves has the closed-form spectrum F(+-n_j) = N^3 a_j/2 exp(+-i phi_j) and zero elsewhere (the definition of the DFT,
+# PAPER.md L25 / DESIGN.md R7).  The input is synthesised on the device with torch (separable phases, integer phase
+# reduction); torch is not on the transform path.  These are the transforms bench.py times for the FFT metric.
+# ---------------------------------------------------------------------------------------------------------
+def _plane_waves(N, nwaves, seed, kmax):
+    rng = np.random.default_rng(seed)
+    waves = set()
+    while len(waves) < nwaves:
+        nx = int(rng.integers(0, kmax + 1))
+        ny, nz = (int(v) for v in rng.integers(-kmax, kmax + 1, size=2))
+        if nx == 0 and (ny < 0 or (ny == 0 and nz <= 0)):
+            continue                                   # one representative of each +-n pair; no mean mode
+        waves.add((nx, ny, nz))
+    waves = sorted(waves)
+    amp = rng.uniform(0.5, 1.5, len(waves))
+    phase = rng.uniform(0, 2 * math.pi, len(waves))
+    return waves, amp, phase
+
+
+def _synthesise(torch, N, waves, amp, phase):
+    i = torch.arange(N, device="cuda", dtype=torch.int64)
+    f = torch.zeros((N, N, N), dtype=torch.float64, device="cuda")
+    for (nx, ny, nz), a, ph in zip(waves, amp, phase):
+        ex = torch.polar(torch.ones(N, dtype=torch.float64, device="cuda"), ((nx * i) % N).double() * (2 * math.pi / N))
+        ey = torch.polar(torch.ones(N, dtype=torch.float64, device="cuda"), ((ny * i) % N).double() * (2 * math.pi / N))
+        ez = torch.polar(torch.full((N,), float(a), dtype=torch.float64, device="cuda"),
+                         ((nz * i) % N).double() * (2 * math.pi / N) + float(ph))
+        f += (ez[:, None, None] * ey[None, :, None] * ex[None, None, :]).real
+    return f
+
+
+def _expected_half_spectrum(torch, N, waves, amp, phase):
+    H = N // 2
+    E = torch.zeros((N, N, H), dtype=torch.complex128, device="cuda")
+    for (nx, ny, nz), a, ph in zip(waves, amp, phase):
+        v = 0.5 * N ** 3 * a * complex(math.cos(ph), math.sin(ph))
+        E[nz % N, ny % N, nx] += v
+        if nx == 0:
+            E[(-nz) % N, (-ny) % N, 0] += v.conjugate()
+    return E
+
+
+@pytest.mark.parametrize("N", [256, 512])
+def test_full_size_fft3d_plane_waves_every_mode(MHD, N):
+    import torch
+    H, kc = N // 2, N // 3
+    waves, amp, phase = _plane_waves(N, 50, 900 + N, H - 1)         # spread over the whole stored half spectrum
+    inside = [w for w in waves if max(abs(w[0]), abs(w[1]), abs(w[2])) <= kc]
+    assert 5 <= len(inside) <= 45                                    # both sides of the 2/3 mask are populated
+    f = _synthesise(torch, N, waves, amp, phase)
+    E = _expected_half_spectrum(torch, N, waves, amp, phase)
+    fnorm = float(torch.linalg.vector_norm(f))
+    eps = np.finfo(float).eps
+    g = MHD(N)
+    spec = torch.zeros((N, N, H, 2), dtype=torch.float64, device="cuda")
+    g.fft3d_r2c([f], [spec], None, prune=False)
+    got = torch.view_as_complex(spec)
+    err = got - E
+    assert float(torch.linalg.vector_norm(err)) <= 1e-14 * float(torch.linalg.vector_norm(E))
+    assert float(err.abs().max()) <= 100 * eps * fnorm               # every single mode, incl. the 99.99 % that are zero
+    # pruned forward transform: the modes inside the mask, everything else untouched
+    spec_p = torch.full((N, N, H, 2), 7.0, dtype=torch.float64, device="cuda")
+    g.fft3d_r2c([f], [spec_p], None, prune=True)
+    n = torch.fft.fftfreq(N, 1.0 / N, device="cuda").round().long().abs()
+    m3 = (n[:, None, None] <= kc) & (n[None, :, None] <= kc) & (torch.arange(H, device="cuda")[None, None, :] <= kc)
+    gp = torch.view_as_complex(spec_p)
+    assert float((gp[m3] - E[m3]).abs().max()) <= 100 * eps * fnorm
+    assert bool(torch.all(spec_p[~m3] == 7.0))
+    # inverse: exact spectrum in, every grid point compared with the synthesised field
+    out = torch.empty((N, N, N), dtype=torch.float64, device="cuda")
+    work = torch.view_as_real(E.clone()).contiguous()
+    g.fft3d_c2r([work], [out], prune=False)
+    assert float(torch.linalg.vector_norm(out - f)) <= 1e-14 * fnorm
+    assert float((out - f).abs().max()) <= 100 * eps * float(np.sum(amp))
+    # pruned inverse = the band-limited part of the field
+    f_in = _synthesise(torch, N, inside, *zip(*[(a, p) for w, a, p in zip(waves, amp, phase) if w in set(inside)]))
+    work = torch.view_as_real(E.clone()).contiguous()
+    g.fft3d_c2r([work], [out], prune=True)
+    assert float((out - f_in).abs().max()) <= 100 * eps * float(np.sum(amp))
+
+
+# ---------------------------------------------------------------------------------------------------------
+# full-size closed form with B != 0 at EVERY grid point: the 2-D Orszag-Tang state of pin P5 (exact for any N >= 16),
+# with its plane rotated onto each pair of axes (cyclic permutations are proper rotations), so that the Lorentz force,
+# the induction term and the full energy flux of the fused x sweep are checked along x, y and z lanes.
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N,perm", [(256, (0, 1, 2)), (256, (1, 2, 0)), (256, (2, 0, 1)), (512, (0, 1, 2)), (512, (2, 0, 1))])
+def test_full_size_orszag_tang_closed_form(MHD, N, perm):
+    r0, P0, mu, eta = 25.0 / 9.0, 5.0 / 3.0, 5e-3, 7e-3
+    c = np.arange(N) * (2 * math.pi / N)
+    C3 = [c[None, None, :], c[None, :, None], c[:, None, None]]       # x, y, z as broadcastable arrays
+    A, B = C3[perm[0]], C3[perm[1]]                                    # canonical (xi, eta) = (x_p0, x_p1)
+    sx, cx, sy, cy = np.sin(A), np.cos(A), np.sin(B), np.cos(B)
+    s2x, c2x, s2y, c2y = np.sin(2 * A), np.cos(2 * A), np.sin(2 * B), np.cos(2 * B)
+    shape = (N, N, N)
+    full = lambda a: np.ascontiguousarray(np.broadcast_to(np.asarray(a, dtype=np.float64), shape))
+    zero = np.zeros(shape)
+    vec = lambda a, b: [x for _, x in sorted(zip(perm, (a, b, None)), key=lambda t: t[0])]
+    u = vec(-sy, sx)
+    Bf = vec(-sy, s2x)
+    prim = [full(r0)] + [zero if x is None else full(x) for x in u] + [full(P0)] + [zero if x is None else full(x) for x in Bf]
+    g = MHD(N, mu=mu, eta=eta)
+    g.set_fields(prim, "primitive")
+    del prim
+    R = g.rhs()
+    Jz = 2 * c2x + cy
+    Hx = r0 * sx * cx + 4 * s2x * c2x
+    Hy = (r0 + 2) * sy * cy
+    Rm = vec(-np.sin(4 * A) + cy * (r0 * sx - s2x) + mu * sy, sy * (r0 * cx - 2 * c2x) - 0.5 * s2y - mu * sx)
+    RB = vec(cy * (sx - s2x) + eta * sy, sy * (2 * c2x - cx) - 4 * eta * s2x)
+    RE = (sy * Hx - sx * Hy - sy * (cx * s2x + 2 * sx * c2x) + 2 * s2x * sy * cy
+          + eta * (Jz * Jz - 4 * s2x ** 2 - sy ** 2) + mu * (c2x + c2y))
+    kc = N // 3
+    tol = 2e-15 * kc * 10.0 * 10       # absolute: kc * |flux| * eps with |flux| <= (E + Pt)|u| ~ 10, one decade of margin
+    assert np.max(np.abs(R[0])) <= tol
+    for i in range(3):
+        exp_m = 0.0 if Rm[i] is None else Rm[i]
+        exp_b = 0.0 if RB[i] is None else RB[i]
+        assert np.max(np.abs(R[1 + i] - exp_m)) <= tol, ("m", i)
+        assert np.max(np.abs(R[5 + i] - exp_b)) <= tol, ("B", i)
+    assert np.max(np.abs(R[4] - RE)) <= tol
 
 
 # ---------------------------------------------------------------------------------------------------------
@@ -587,14 +736,18 @@ def test_chunked_pipeline_budget(MHD):
         assert rel_l2(a, r) <= 1e-13
 
 
-def test_config6_1024_maximum_size(MHD):
-    """Config 6 (BASELINE.json: 1024^3, the largest grid the ABI accepts) through the chunked pipeline.  The oracle
-    cannot hold 1024^3, so the check uses properties that hold at any size: exact conservation of <rho>, <m>, <E>
+@pytest.mark.parametrize("placement", ["host", "device"])
+def test_config6_1024_maximum_size(MHD, placement):
+    """Config 6 as BASELINE.json writes it: 1024^3, 10 steps, "field storage exceeding HBM and slabs streamed to and from
+    pinned host memory" (placement "host": MHD_FLAG_STATE_ON_HOST | MHD_FLAG_WORK_ON_HOST, 8.8 GB of device staging and
+    103 GB of pinned host memory), and the same run with the compact storage resident in HBM (placement "device").  The
+    oracle cannot hold 1024^3, so the check uses properties that hold at any size: exact conservation of <rho>, <m>, <E>
     (pin P11), solenoidal B (P10), and resolution independence — the band-limited initial condition (|n| <= 16) evolves
     identically on a 512^3 grid (in-core path, itself checked against the oracle), compared on the coinciding points."""
     import gc
+    import torch
     from paper_1810_12707_b200 import binding as b
-    nsteps = 2
+    nsteps = 10
     c5 = inputs.config6(512)
     ref = MHD(c5.N, c5.L, c5.gamma, c5.mu, c5.eta, c5.dt)
     ref.set_fields(c5.prim, "primitive")
@@ -603,15 +756,28 @@ def test_config6_1024_maximum_size(MHD):
     sref = ref.get_fields()
     del ref, c5
     gc.collect()
+    torch.cuda.empty_cache()
 
     cfg = inputs.config6(1024)
-    g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, flags=b.MHD_FLAG_OUT_OF_CORE)
-    assert g.workspace_bytes < 120e9           # compact storage: 1024^3 sits in one B200 (48 full fields would be 412 GB)
+    flags = b.MHD_FLAG_OUT_OF_CORE
+    if placement == "host":
+        flags |= b.MHD_FLAG_STATE_ON_HOST | b.MHD_FLAG_WORK_ON_HOST
+    g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, flags=flags)
+    if placement == "host":
+        assert g.workspace_bytes < 16e9 and g.pinned_bytes > 100e9      # field storage is on the host, not in HBM
+    else:
+        assert g.workspace_bytes < 120e9       # compact storage: 1024^3 sits in one B200 (48 full fields would be 412 GB)
     g.set_fields(cfg.prim, "primitive")
     cfg.prim = None
     gc.collect()
     d0 = g.diagnostics()
+    t0 = g.transfer_bytes()
     g.step(nsteps)
+    t1 = g.transfer_bytes()
+    if placement == "host":       # every step streams the state and the work fields both ways
+        assert t1[0] - t0[0] > nsteps * 100e9 and t1[1] - t0[1] > nsteps * 100e9
+    else:
+        assert t1 == t0
     d1 = g.diagnostics()
     assert d1["step"] == nsteps
     assert abs(d1["mass"] - d0["mass"]) <= 1e-13 and abs(d1["etot"] - d0["etot"]) <= 1e-13 * d0["etot"]
@@ -619,8 +785,11 @@ def test_config6_1024_maximum_size(MHD):
     assert d1["max_divb"] <= 1e-13 * (1024 // 3) * 0.5 * 10
     for k in ("ke", "me", "ie"):         # (the minima run over different point sets and are not comparable)
         assert abs(d1[k] - dref[k]) <= 1e-11 * abs(dref[k]), (k, d1[k], dref[k])
-    out = g.get_fields()
+    # the state, on the coinciding points; with the fields on the host it is taken on the device (69 GB) so that the
+    # host keeps room for the 103 GB pinned block, with the fields in HBM on the host
+    out = g.get_fields(where="device" if placement == "host" else "host")
     for f in range(8):
         sub = out[f][::2, ::2, ::2]
+        sub = sub.contiguous().cpu().numpy() if placement == "host" else sub
         assert rel_l2(sub, sref[f]) <= 1e-10, NAMES[f]
         out[f] = None
