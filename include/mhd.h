@@ -74,6 +74,13 @@ extern "C" {
 #define MHD_OPT_FUSE_CURRENT 4 /* 1 (default): J^ = M i k x B^ is built on load inside the inverse z pass (sweep S1);
                                 0: separate kernel                                                            */
 
+#define MHD_OPT_FUSE_ASSEMBLE 7 /* sweep S5 (in-core contexts, default equation set, N = 64..512) as ONE launch: the forward z
+                                pass runs in thread-block clusters — 1: 16 CTAs, one per product field; 2: 8 CTAs, two
+                                fields each — that keep the transformed rows in shared memory and assemble R^ and the
+                                explicit update from each other's tiles (distributed shared memory).  Bitwise the
+                                two-launch result; measured slower on B200, so the default is
+                                0: forward z pass and assembly as two launches                                 */
+
 #define MHD_OPT_OOC_BRICK 5 /* chunked pipeline: largest number of ky columns per brick (0 = what the staging allows) */
 #define MHD_OPT_OOC_SLAB 6  /* chunked pipeline: largest number of z planes per slab  (0 = what the staging allows) */
 

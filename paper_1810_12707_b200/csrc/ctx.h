@@ -15,10 +15,11 @@
 using namespace mhd;
 
 enum Family { F_STRIDED_INV = 0, F_STRIDED_FWD, F_X_FUSED, F_X_C2R, F_X_R2C, F_FLUX, F_CURRENT, F_ASSEMBLE, F_AXPBY,
-              F_POINT, F_DIAG, F_TRACERS, F_COUNT };
+              F_POINT, F_DIAG, F_TRACERS, F_S5, F_COUNT };
 inline const char* family_name(int f) {
     static const char* names[F_COUNT] = {"strided_inverse", "strided_forward", "x_fused", "x_c2r", "x_r2c", "flux_real",
-                                         "build_current", "assemble", "axpby", "pointwise_misc", "diagnostics", "tracers"};
+                                         "build_current", "assemble", "axpby", "pointwise_misc", "diagnostics", "tracers",
+                                         "forward_z_assemble"};
     return names[f];
 }
 
@@ -55,7 +56,7 @@ struct mhd_ctx {
     bool bound = false, have_fields = false, have_old = false;
     cudaStream_t st = nullptr;
     unsigned flags = 0;
-    int opt_fused = 1, opt_prune = 1, opt_fuse_current = 1, integrator = 0, opt_stress = 0;
+    int opt_fused = 1, opt_prune = 1, opt_fuse_current = 1, integrator = 0, opt_stress = 0, opt_fuse_assemble = 0;
     long long step = 0;
     long long launches = 0;
     std::string err;

@@ -36,24 +36,6 @@ template <int DIR> __device__ __forceinline__ cd mul_mi(cd a) {
     return mk(-a.y, a.x);
 }
 
-// a * exp(DIR * 2*pi*i * K/R), 0 <= K < R/2, R in {2,4,8,16}: constants of the in-register butterflies
-template <int R, int K, int DIR> __device__ __forceinline__ cd mul_root(cd a) {
-    constexpr int K16 = K * (16 / R);
-    constexpr double SQH = 0.70710678118654752440;   // sqrt(1/2)
-    constexpr double C8 = 0.92387953251128675613;    // cos(pi/8)
-    constexpr double S8 = 0.38268343236508977173;    // sin(pi/8)
-    constexpr double sg = (DIR < 0) ? -1.0 : 1.0;    // sign of the imaginary part of the root
-    if constexpr (K16 == 0) return a;
-    else if constexpr (K16 == 4) return mul_mi<DIR>(a);
-    else if constexpr (K16 == 2) return mk(SQH * (a.x - sg * a.y), SQH * (a.y + sg * a.x));
-    else if constexpr (K16 == 6) return mk(-SQH * (a.x + sg * a.y), SQH * (sg * a.x - a.y));
-    else {
-        constexpr double wr = (K16 == 1) ? C8 : (K16 == 3) ? S8 : (K16 == 5) ? -S8 : -C8;
-        constexpr double wi = sg * ((K16 == 1 || K16 == 7) ? S8 : C8);
-        return mk(fma(a.x, wr, -(a.y * wi)), fma(a.x, wi, a.y * wr));
-    }
-}
-
 // a * exp(DIR * 2*pi*i * K32/32) for any compile-time K32 in [0, 32): constant 32nd roots of unity
 template <int K32, int DIR> __device__ __forceinline__ cd mul_root32(cd a) {
     constexpr double C[16] = {1.0, 0.98078528040323044913, 0.92387953251128675613, 0.83146961230254523708,
@@ -87,6 +69,47 @@ template <int R, int K, int DIR> __device__ __forceinline__ cd mul_rootN(cd a) {
     return mul_root32<(K % R) * (32 / R), DIR>(a);
 }
 
+// ---------------------------------------------------------------------------------------------------
+// FMA-form radix-2 butterflies.  v = e + W o, vm = e - W o.  The product W o is never formed on its own: its two
+// multiply-adds are chained onto e (2 FMA per component), and the mirrored output is vm = 2 e - v (1 FMA per
+// component), so a butterfly with a general root costs 6 FMA instead of 4 (product) + 4 (add / subtract).  The
+// absolute error of vm is bounded by eps (|e| + |W o|) exactly as for the plain form (it inherits the rounding of
+// v), so the backward-error bound of the transform is unchanged.
+// ---------------------------------------------------------------------------------------------------
+__device__ __forceinline__ cd mirror2(cd e, cd v) { return mk(fma(2.0, e.x, -v.x), fma(2.0, e.y, -v.y)); }
+
+// constant root W = exp(DIR * 2*pi*i * K/R), 0 <= K < R/2, R in {2,4,8,16}
+template <int R, int K, int DIR> __device__ __forceinline__ void bfly_root(cd e, cd o, cd& v, cd& vm) {
+    constexpr int K16 = K * (16 / R);
+    constexpr double SQH = 0.70710678118654752440;   // sqrt(1/2)
+    constexpr double C8 = 0.92387953251128675613;    // cos(pi/8)
+    constexpr double S8 = 0.38268343236508977173;    // sin(pi/8)
+    if constexpr (K16 == 0) { v = e + o; vm = e - o; }
+    else if constexpr (K16 == 4) { const cd t = mul_mi<DIR>(o); v = e + t; vm = e - t; }
+    else if constexpr (K16 == 2) {          // W = SQH (1 + sg i):  W o = SQH (o.x - sg o.y, o.y + sg o.x)
+        const double dx = (DIR < 0) ? o.x + o.y : o.x - o.y, dy = (DIR < 0) ? o.y - o.x : o.y + o.x;
+        v = mk(fma(SQH, dx, e.x), fma(SQH, dy, e.y)); vm = mk(fma(-SQH, dx, e.x), fma(-SQH, dy, e.y));
+    } else if constexpr (K16 == 6) {        // W = SQH (-1 + sg i): W o = SQH (-(o.x + sg o.y), sg o.x - o.y)
+        const double dx = (DIR < 0) ? o.x - o.y : o.x + o.y, dy = (DIR < 0) ? -o.x - o.y : o.x - o.y;
+        v = mk(fma(-SQH, dx, e.x), fma(SQH, dy, e.y)); vm = mk(fma(SQH, dx, e.x), fma(-SQH, dy, e.y));
+    } else {
+        constexpr double wr = (K16 == 1) ? C8 : (K16 == 3) ? S8 : (K16 == 5) ? -S8 : -C8;
+        constexpr double wi = ((DIR < 0) ? -1.0 : 1.0) * ((K16 == 1 || K16 == 7) ? S8 : C8);
+        v = mk(fma(-o.y, wi, fma(o.x, wr, e.x)), fma(o.y, wr, fma(o.x, wi, e.y)));
+        vm = mirror2(e, v);
+    }
+}
+
+// run-time root: forward (DIR < 0) W = w, inverse W = conj(w), w = forward table entry; ROT: W is additionally
+// multiplied by -i (forward) / +i (inverse), i.e. the root a quarter turn further — the same table entry serves both
+template <int DIR, bool ROT> __device__ __forceinline__ void bfly_tw(cd e, cd o, cd w, cd& v, cd& vm) {
+    if constexpr (DIR < 0 && !ROT) v = mk(fma(-o.y, w.y, fma(o.x, w.x, e.x)), fma(o.y, w.x, fma(o.x, w.y, e.y)));
+    else if constexpr (DIR > 0 && !ROT) v = mk(fma(o.y, w.y, fma(o.x, w.x, e.x)), fma(-o.x, w.y, fma(o.y, w.x, e.y)));
+    else if constexpr (DIR < 0 && ROT) v = mk(fma(o.y, w.x, fma(o.x, w.y, e.x)), fma(o.y, w.y, fma(-o.x, w.x, e.y)));
+    else v = mk(fma(o.x, w.y, fma(-o.y, w.x, e.x)), fma(o.y, w.y, fma(o.x, w.x, e.y)));
+    vm = mirror2(e, v);
+}
+
 // In-register DFT of R points, natural order in and out:  v[q] <- sum_r v[r] exp(DIR*2*pi*i*r*q/R)
 template <int R, int DIR> struct Dft;
 template <int DIR> struct Dft<1, DIR> {
@@ -106,8 +129,7 @@ template <int DIR> struct Dft<4, DIR> {
 };
 template <int R, int K, int DIR> struct Combine {   // v[k] = e[k] + W^k o[k], v[k+R/2] = e[k] - W^k o[k]
     __device__ __forceinline__ static void run(cd* v, const cd* e, const cd* o) {
-        const cd t = mul_root<R, K, DIR>(o[K]);
-        v[K] = e[K] + t; v[K + R / 2] = e[K] - t;
+        bfly_root<R, K, DIR>(e[K], o[K], v[K], v[K + R / 2]);
         if constexpr (K + 1 < R / 2) Combine<R, K + 1, DIR>::run(v, e, o);
     }
 };
@@ -119,6 +141,45 @@ template <int R, int DIR> struct Dft {
         Dft<R / 2, DIR>::run(e);
         Dft<R / 2, DIR>::run(o);
         Combine<R, 0, DIR>::run(v, e, o);
+    }
+};
+
+// ---------------------------------------------------------------------------------------------------
+// Twiddled DFT: v[q] <- sum_r (w^r v[r]) exp(DIR*2*pi*i*r*q/R) with the inter-stage twiddles w^r folded into the
+// butterflies.  Decimation in time: y[q] = E[q] + (w W_R^q) O[q], where E, O are the twiddled DFTs of size R/2 of
+// the even / odd inputs with base w^2.  Every butterfly then has exactly one run-time root and costs 6 FMA:
+// R/2 log2(R) * 6 operations (192 for R = 16) instead of 4 (R-1) for the twiddles plus the plain DFT (60 + 168).
+// Roots needed: w W_R^q for q < R/4 (the other quarter is the same entry rotated by -+i), then w^2 W_(R/2)^q, ...:
+// R/2 table entries (8 for R = 16) instead of R-1.
+// ---------------------------------------------------------------------------------------------------
+template <int R> struct TwCount { static constexpr int TOP = (R >= 4) ? R / 4 : 1, value = TOP + TwCount<R / 2>::value; };
+template <> struct TwCount<1> { static constexpr int TOP = 0, value = 0; };
+
+// w[] <- the roots of TDft<R>, base exponent m: w = exp(-2*pi*i*m/NT); tw[i*TWS] = exp(-2*pi*i*i/NT)
+template <int R, int NT, int TWS> __device__ __forceinline__ void load_tw(cd* w, const cd* __restrict__ tw, int m) {
+    if constexpr (R >= 2) {
+#pragma unroll
+        for (int q = 0; q < TwCount<R>::TOP; ++q) w[q] = __ldg(&tw[(m + q * (NT / R)) * TWS]);
+        load_tw<R / 2, NT, TWS>(w + TwCount<R>::TOP, tw, 2 * m);
+    }
+}
+template <int R, int DIR> struct TDft {
+    __device__ __forceinline__ static void run(cd* v, const cd* w) {
+        if constexpr (R == 2) {
+            const cd e = v[0], o = v[1];
+            bfly_tw<DIR, false>(e, o, w[0], v[0], v[1]);
+        } else {
+            cd e[R / 2], o[R / 2];
+#pragma unroll
+            for (int i = 0; i < R / 2; ++i) { e[i] = v[2 * i]; o[i] = v[2 * i + 1]; }
+            TDft<R / 2, DIR>::run(e, w + TwCount<R>::TOP);
+            TDft<R / 2, DIR>::run(o, w + TwCount<R>::TOP);
+#pragma unroll
+            for (int q = 0; q < R / 4; ++q) {
+                bfly_tw<DIR, false>(e[q], o[q], w[q], v[q], v[q + R / 2]);
+                bfly_tw<DIR, true>(e[q + R / 4], o[q + R / 4], w[q], v[q + R / 4], v[q + R / 4 + R / 2]);
+            }
+        }
     }
 };
 
@@ -166,14 +227,13 @@ __device__ __forceinline__ void fft_stage(cd (&v)[PlanInfo<NL>::E], int t, const
         cd u[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) u[r] = v[b + r * B];
-        if constexpr (NSTRIDE > 1) {
-#pragma unroll
-            for (int r = 1; r < R; ++r) {
-                const cd w = __ldg(&tw[(r * k * (NL / (NSTRIDE * R))) * TWS]);
-                u[r] = twmul<DIR>(u[r], w);
-            }
+        if constexpr (NSTRIDE > 1) {        // inter-stage twiddles w^r, w = exp(-+2 pi i k/(Ns R)), folded into the butterflies
+            cd w[TwCount<R>::value];
+            load_tw<R, NL, TWS>(w, tw, k * (NL / (NSTRIDE * R)));
+            TDft<R, DIR>::run(u, w);
+        } else {
+            Dft<R, DIR>::run(u);
         }
-        Dft<R, DIR>::run(u);
         if constexpr (LAST) {
 #pragma unroll
             for (int q = 0; q < R; ++q) v[b + q * B] = u[q];

@@ -10,14 +10,14 @@ constexpr int MAXF = 16;   // largest batch of fields one launch handles
 
 // Opt-in to more than 48 KB of dynamic shared memory, once per kernel instantiation AND per device (the attribute is a
 // per-device property of the function: a process that drives several GPUs must set it on each of them).
+// The cache is keyed by the kernel's ADDRESS (all instantiations of one template share the pointer type K, so a
+// function-local static keyed by K alone would configure only the first of them).
+bool dynamic_smem_seen(const void* kern, int dev);      // mhd_api.cu; returns true if (kern, dev) was already configured
 template <class K> inline void ensure_dynamic_smem(K kern, size_t smem) {
-    constexpr int MAX_DEV = 64;
-    static bool done[MAX_DEV] = {};
     int dev = 0;
     cudaGetDevice(&dev);
-    if (dev >= 0 && dev < MAX_DEV && done[dev]) return;
+    if (dynamic_smem_seen(reinterpret_cast<const void*>(kern), dev)) return;
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (dev >= 0 && dev < MAX_DEV) done[dev] = true;
 }
 
 // Physical constants of one context, passed by value to the point-wise kernels.
@@ -69,6 +69,22 @@ struct StridedArgs {
 };
 // dir = -1 forward, +1 inverse (unnormalised both ways)
 void launch_strided(int N, int dir, const StridedArgs& a, cudaStream_t st);
+
+// Sweep S5 as ONE launch (north_star (4): "the explicit time integrator fused into the last spectral
+// pass"): the in-core forward z pass of the 16 product fields in thread-block clusters of 16 — one CTA per field of a
+// (ky, kx tile) column — which keep the transformed rows in shared memory, meet at a cluster barrier and assemble R^
+// (i k, -k^2, mask) and the explicit update from each other's tiles through distributed shared memory.
+struct AssembleTail {
+    cd* U[8];
+    cd* Rold[8];
+    cd* rout[8];           // mode 0 only
+    int mode;              // as launch_assemble: 0 rout = R; 1 Euler update; 2 Adams-Bashforth 2 update
+    double dt;
+    Phys ph;
+};
+bool strided_assemble_supported(int N);
+void launch_strided_assemble(int N, int fields_per_cta, const StridedArgs& a, const AssembleTail& z, cudaStream_t st);
+int strided_assemble_max_clusters(int N, int fields_per_cta, const StridedArgs& a);   // occupancy query (bench / diagnostics)
 
 // ---- x passes ----------------------------------------------------------------------------------------------
 struct XArgs {

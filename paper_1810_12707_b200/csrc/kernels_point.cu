@@ -122,23 +122,10 @@ __global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 r
     cd R[8];
     if (m.inside) {
         const double kx = ph.k0 * m.nx, ky = ph.k0 * m.ny, kz = ph.k0 * m.nz;
-        const double k2 = kx * kx + ky * ky + kz * kz;
         cd u[8];
 #pragma unroll
         for (int f = 0; f < 8; ++f) u[f] = U.p[f][j];
-        const cd txx = pr.p[P_TXX][i], txy = pr.p[P_TXY][i], txz = pr.p[P_TXZ][i];
-        const cd tyy = pr.p[P_TYY][i], tyz = pr.p[P_TYZ][i], tzz = pr.p[P_TZZ][i];
-        const cd ex = pr.p[P_EX][i], ey = pr.p[P_EY][i], ez = pr.p[P_EZ][i];
-        // -i k.F = -(i kx Fx + i ky Fy + i kz Fz)
-        R[0] = mk(0, 0) - (imul(kx, u[1]) + imul(ky, u[2]) + imul(kz, u[3]));
-        R[1] = mk(0, 0) - (imul(kx, txx) + imul(ky, txy) + imul(kz, txz)) - (ph.mu * k2) * pr.p[P_UX][i];
-        R[2] = mk(0, 0) - (imul(kx, txy) + imul(ky, tyy) + imul(kz, tyz)) - (ph.mu * k2) * pr.p[P_UY][i];
-        R[3] = mk(0, 0) - (imul(kx, txz) + imul(ky, tyz) + imul(kz, tzz)) - (ph.mu * k2) * pr.p[P_UZ][i];
-        R[4] = mk(0, 0) - (imul(kx, pr.p[P_FEX][i]) + imul(ky, pr.p[P_FEY][i]) + imul(kz, pr.p[P_FEZ][i]))
-               - (ph.mu * k2) * pr.p[P_Q][i];
-        R[5] = imul(ky, ez) - imul(kz, ey) - (ph.eta * k2) * u[5];
-        R[6] = imul(kz, ex) - imul(kx, ez) - (ph.eta * k2) * u[6];
-        R[7] = imul(kx, ey) - imul(ky, ex) - (ph.eta * k2) * u[7];
+        rhs_mode([&](int s) { return pr.p[s][i]; }, u, kx, ky, kz, ph, R);
         if constexpr (VAR) {
         if (visc.p[0]) {         // variant: + d_j (2 nu rho S_ij) and + d_j (2 nu rho u_i S_ij)  (Eq. 11-12)
             const cd vxx = visc.p[0][j], vxy = visc.p[1][j], vxz = visc.p[2][j], vyy = visc.p[3][j], vyz = visc.p[4][j], vzz = visc.p[5][j];
@@ -161,10 +148,8 @@ __global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 r
         } else {
 #pragma unroll
             for (int f = 0; f < 8; ++f) {
-                cd inc;
-                if (mode == 1) inc = R[f];
-                else { const cd ro = Rold.p[f][j]; inc = mk(1.5 * R[f].x - 0.5 * ro.x, 1.5 * R[f].y - 0.5 * ro.y); }
-                U.p[f][j] = mk(u[f].x + dt * inc.x, u[f].y + dt * inc.y);
+                const cd ro = mode == 2 ? Rold.p[f][j] : mk(0, 0);
+                U.p[f][j] = updated(mode, dt, u[f], R[f], ro);
                 Rold.p[f][j] = R[f];
             }
         }

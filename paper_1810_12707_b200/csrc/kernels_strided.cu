@@ -10,6 +10,10 @@
 // identically zero are neither read nor written.
 #include "fft_core.cuh"
 #include "kernels.h"
+#include "physics.cuh"
+
+#include <cooperative_groups.h>
+namespace cg = cooperative_groups;
 
 namespace mhd {
 
@@ -112,6 +116,167 @@ strided_kernel(const __grid_constant__ StridedArgs a) {
             const bool keep = valid && (!a.out_rows || row <= kc || row >= N - kc);
             if (keep) out[(long long)row * a.in_row_stride] = v[m];
         }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// Sweep S5 in one launch: forward z pass (in-core, pruned) + assembly of R^ + explicit update (kernels.h AssembleTail).
+// Grid: x = (kx tile) * 16 + field, y = ky (pruned list); thread-block CLUSTERS of 16 along x, so that the 16 CTAs that
+// transform the 16 product fields of one (ky, kx tile) column are co-scheduled (hardware guarantee) and see each other's
+// shared memory.  Each CTA transforms its field (rows = kz) and leaves the rows inside the mask in its own tile; after a
+// cluster barrier every CTA assembles 1/16 of the rows, reading the 16 product values of a mode from the 16 tiles through
+// distributed shared memory.  The transformed products never reach L2 or HBM: sweep S5 reads 16 + 8 + 8 and writes 8 + 8
+// field sweeps, as SURVEY.md 8(d) counts it.
+// ---------------------------------------------------------------------------------------------------------------------
+// FPC = product fields per CTA (1 or 2) -> clusters of 16 / FPC CTAs.  Shared memory: the exchange tile [N][8] plus, for
+// FPC = 2, one compact tile [2kc+1][8] that keeps the first field's rows while the second field is transformed.
+template <int N, int FPC, int CC> struct S5Cfg {
+    static constexpr int C = CC, NK = 2 * (N / 3) + 1, CL = P_NOUT / FPC;
+    static constexpr int RPC = (NK + CL - 1) / CL;                  // kept rows assembled per CTA
+    static constexpr size_t SMEM = (size_t(N) * C + size_t(FPC - 1) * NK * C) * sizeof(cd);
+};
+
+template <int N, int FPC, int CC>
+__global__ void __launch_bounds__(StridedOcc<N, CC>::THREADS, StridedOcc<N, CC>::MINB)
+strided_assemble_kernel(const __grid_constant__ StridedArgs a, const __grid_constant__ AssembleTail z) {
+    typedef S5Cfg<N, FPC, CC> P;
+    constexpr int E = PlanInfo<N>::E, T = PlanInfo<N>::T, C = CC, NK = P::NK, CL = P::CL, RPC = P::RPC;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cd* sm = reinterpret_cast<cd*>(smem_raw);
+    cg::cluster_group cluster = cg::this_cluster();
+
+    const int tid = threadIdx.x;
+    const int c = tid % C, t = tid / C;
+    const int bx = blockIdx.x / CL, rank = blockIdx.x % CL;           // rank in the cluster
+    const int col = bx * C + c;
+    int o = blockIdx.y;
+    if (o >= a.outer_split) o += a.outer_skip;
+    const bool valid = col < a.ncols;
+    const int kc = a.kc;
+    const long long base = (long long)o * a.in_outer_stride + col;
+
+    // the state lines this CTA will update after the barrier: start them on their way to L2 now
+    if (c == 0 && bx * C <= kc) {
+        for (int ri = t; ri < RPC; ri += T) {
+            const int i = rank * RPC + ri;
+            if (i >= NK) break;
+            const int row = i <= kc ? i : i + (N - NK);
+            const long long line = base + (long long)row * a.in_row_stride;
+#pragma unroll
+            for (int g = 0; g < 8; ++g) {
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(z.U[g] + line));
+                if (z.mode == 2) asm volatile("prefetch.global.L2 [%0];" ::"l"(z.Rold[g] + line));
+            }
+        }
+    }
+#pragma unroll
+    for (int fi = 0; fi < FPC; ++fi) {
+        const int f = rank * FPC + fi;
+        cd v[E];
+        const cd* __restrict__ in = a.in[f] + base;
+#pragma unroll
+        for (int m = 0; m < E; ++m) v[m] = valid ? in[(long long)(t + T * m) * a.in_row_stride] : mk(0.0, 0.0);
+        if (fi > 0) __syncthreads();        // the previous field's compact rows have left the exchange tile
+        fft_line<N, -1, 1>(v, t, a.tw, sm, LayoutPlain{C, c});
+        __syncthreads();                    // every thread has gathered its last exchange: the tile is free
+        // kept rows, compact index i: the last field of the CTA stays in the exchange tile, earlier ones move behind it
+        cd* keep = (fi == FPC - 1) ? sm : sm + (size_t)N * C + (size_t)fi * NK * C;
+#pragma unroll
+        for (int m = 0; m < E; ++m) {
+            const int row = t + T * m;
+            if (row <= kc) keep[row * C + c] = v[m];
+            else if (row >= N - kc) keep[(row - (N - NK)) * C + c] = v[m];
+        }
+    }
+    cluster.sync();                         // all 16 product tiles of this column are in place
+    // ---- assembly: this CTA takes the kept rows [rank * RPC, (rank + 1) * RPC) --------------------------------------
+    if (valid && col <= kc) {
+        const int ny = o <= N / 2 ? o : o - N;
+        const double kxv = z.ph.k0 * col, kyv = z.ph.k0 * ny;
+        for (int ri = t; ri < RPC; ri += T) {
+            const int i = rank * RPC + ri;
+            if (i >= NK) break;
+            const int row = i <= kc ? i : i + (N - NK);
+            const int nz = row <= N / 2 ? row : row - N;
+            const long long idx = base + (long long)row * a.in_row_stride;
+            cd u[8], R[8];
+#pragma unroll
+            for (int g = 0; g < 8; ++g) u[g] = z.U[g][idx];
+            auto ld = [&](int s) {
+                const cd* tile = cluster.map_shared_rank(sm, s / FPC);
+                const int fi = s % FPC;
+                if (fi != FPC - 1) tile += (size_t)N * C + (size_t)fi * NK * C;
+                return tile[i * C + c];
+            };
+            rhs_mode(ld, u, kxv, kyv, z.ph.k0 * nz, z.ph, R);
+            if (z.mode == 0) {
+#pragma unroll
+                for (int g = 0; g < 8; ++g) z.rout[g][idx] = R[g];
+            } else {
+#pragma unroll
+                for (int g = 0; g < 8; ++g) {
+                    const cd ro = z.mode == 2 ? z.Rold[g][idx] : mk(0, 0);
+                    z.U[g][idx] = updated(z.mode, z.dt, u[g], R[g], ro);
+                    z.Rold[g][idx] = R[g];
+                }
+            }
+        }
+    }
+    cluster.sync();                         // nobody leaves while its tile may still be read
+}
+
+template <int N, int FPC, int CC> static void s5_configure(cudaLaunchConfig_t& cfg, cudaLaunchAttribute* attr, const StridedArgs& a,
+                                                   cudaStream_t st) {
+    typedef S5Cfg<N, FPC, CC> P;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (!dynamic_smem_seen(reinterpret_cast<const void*>(strided_assemble_kernel<N, FPC, CC>), dev)) {
+        cudaFuncSetAttribute(strided_assemble_kernel<N, FPC, CC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::SMEM);
+        // clusters of 16 are above the portable size of 8: a per-function, per-device opt-in
+        if (P::CL > 8) cudaFuncSetAttribute(strided_assemble_kernel<N, FPC, CC>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    }
+    cfg = cudaLaunchConfig_t{};
+    cfg.gridDim = dim3(((a.ncols + P::C - 1) / P::C) * P::CL, a.n_outer, 1);
+    cfg.blockDim = dim3(P::C * PlanInfo<N>::T, 1, 1);
+    cfg.dynamicSmemBytes = P::SMEM;
+    cfg.stream = st;
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = P::CL; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+}
+template <int N, int FPC, int CC> static void strided_assemble_one(const StridedArgs& a, const AssembleTail& z, cudaStream_t st) {
+    cudaLaunchConfig_t cfg; cudaLaunchAttribute attr[1];
+    s5_configure<N, FPC, CC>(cfg, attr, a, st);
+    cudaLaunchKernelEx(&cfg, strided_assemble_kernel<N, FPC, CC>, a, z);
+}
+template <int N, int FPC, int CC> static int s5_max_clusters(const StridedArgs& a) {
+    cudaLaunchConfig_t cfg; cudaLaunchAttribute attr[1];
+    s5_configure<N, FPC, CC>(cfg, attr, a, nullptr);
+    int n = 0;
+    if (cudaOccupancyMaxActiveClusters(&n, strided_assemble_kernel<N, FPC, CC>, &cfg) != cudaSuccess) { cudaGetLastError(); return -1; }
+    return n;
+}
+bool strided_assemble_supported(int N) { return N >= 64 && N <= 512; }
+// variant: 1 = one field per CTA (clusters of 16); 2 = two fields per CTA (clusters of 8, the portable size)
+void launch_strided_assemble(int N, int variant, const StridedArgs& a, const AssembleTail& z, cudaStream_t st) {
+#define S5_CASE(NN)                                                             \
+    case NN:                                                                    \
+        if (variant == 1) strided_assemble_one<NN, 1, 8>(a, z, st);             \
+        else strided_assemble_one<NN, 2, 8>(a, z, st);                          \
+        break;
+    switch (N) {
+        S5_CASE(64) S5_CASE(128) S5_CASE(256) S5_CASE(512)
+        default: break;
+    }
+#undef S5_CASE
+}
+int strided_assemble_max_clusters(int N, int variant, const StridedArgs& a) {
+    switch (N * 4 + variant) {
+        case 256 * 4 + 1: return s5_max_clusters<256, 1, 8>(a);
+        case 256 * 4 + 2: return s5_max_clusters<256, 2, 8>(a);
+        case 512 * 4 + 1: return s5_max_clusters<512, 1, 8>(a);
+        case 512 * 4 + 2: return s5_max_clusters<512, 2, 8>(a);
+        default: return -1;
     }
 }
 

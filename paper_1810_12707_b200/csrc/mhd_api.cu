@@ -10,7 +10,20 @@
 // No host round trip inside mhd_step: only kernel launches on the bound stream.
 #include "ctx.h"
 
+#include <mutex>
+#include <set>
+#include <utility>
+
 using namespace mhd;
+
+namespace mhd {
+bool dynamic_smem_seen(const void* kern, int dev) {
+    static std::mutex mu;
+    static std::set<std::pair<const void*, int>> seen;
+    std::lock_guard<std::mutex> lock(mu);
+    return !seen.insert(std::make_pair(kern, dev)).second;
+}
+}  // namespace mhd
 
 namespace {
 
@@ -115,7 +128,8 @@ namespace {
 
 // products W[0..15] <- state Uin (k-space); sweeps S1-S4 and the forward z pass of S5
 // breal != null (tracers, fused sweep only): the real-space B of Uin is also written there by sweep S3
-void products(mhd_ctx* c, cd* const Uin[8], double* const breal[3] = nullptr) {
+// s5a = false: the forward z pass is left to the caller (fused with the assembly: sweep S5 in one launch)
+void products(mhd_ctx* c, cd* const Uin[8], double* const breal[3] = nullptr, bool s5a = true) {
     const int N = c->N;
     const bool prune = c->opt_prune != 0;
     const SpecGeom g = c->geom();
@@ -164,7 +178,27 @@ void products(mhd_ctx* c, cd* const Uin[8], double* const breal[3] = nullptr) {
         }
         strided_pass(c, -1, 1, 16, c->W, c->W, c->hx(), c->hx(), prune, -1, 0, z0, nz);      // S4
     }
-    strided_pass(c, -1, 2, 16, c->W, c->W, c->hx(), c->hx(), prune);      // S5a
+    if (s5a) strided_pass(c, -1, 2, 16, c->W, c->W, c->hx(), c->hx(), prune);      // S5a
+}
+
+// sweep S5 in one launch: forward z pass of W[0..15] + assembly + update (kernels.h AssembleTail)
+void fused_s5(mhd_ctx* c, cd* const Uin[8], cd* const rout[8], int mode) {
+    const int N = c->N, kc = c->kc(), hx = c->hx();
+    StridedArgs a;
+    std::memset(&a, 0, sizeof(a));
+    for (int f = 0; f < 16; ++f) { a.in[f] = c->W[f]; a.out[f] = c->W[f]; }
+    a.tw = c->tw; a.kc = kc; a.nfields = 16; a.jfirst = -1;
+    a.ncols = std::min(kc + 1, hx);
+    a.in_row_stride = a.out_row_stride = (long long)N * hx; a.in_outer_stride = a.out_outer_stride = hx;
+    a.n_outer = 2 * kc + 1; a.outer_split = kc + 1; a.outer_skip = N - (2 * kc + 1);
+    a.in_rows = 0; a.out_rows = 1;
+    AssembleTail z;
+    std::memset(&z, 0, sizeof(z));
+    for (int f = 0; f < 8; ++f) { z.U[f] = Uin[f]; z.Rold[f] = c->Rold[f]; z.rout[f] = rout ? rout[f] : nullptr; }
+    z.mode = mode; z.dt = c->dt; z.ph = c->phys();
+    mhd_ctx::Scope s(c, F_S5);
+    launch_strided_assemble(N, c->opt_fuse_assemble, a, z, c->st);
+
 }
 
 // Variant MHD_OPT_STRESS (Eq. 3-4, 11-12): V_ij = 2 nu rho S_ij and Wv_j = u_i V_ij, transformed, for the assembly.
@@ -203,8 +237,12 @@ void rhs_spectral(mhd_ctx* c, cd* const Uin[8], cd* const rout[8], int mode, dou
     const bool stress = c->opt_stress != 0;
     const cd* visc[9] = {c->Y[0], c->Y[1], c->Y[2], c->Y[3], c->Y[4], c->Y[5], c->Y[6], c->Y[7], c->X[7]};
     if (stress) viscous_pass(c, Uin);                 // V^_ij, Wv^_j -> Y[0..7], X[7]   (before the products: uses X, Y)
-    products(c, Uin, breal);
     const bool forced = c->f0 != 0.0;
+    // default equation set on the pruned, fused path: sweep S5 is one launch
+    const bool one_s5 = c->opt_fuse_assemble != 0 && c->opt_fused != 0 && c->opt_prune != 0 && !stress && !forced &&
+                        c->cs2 <= 0.0 && c->evolve == 3 && strided_assemble_supported(c->N);
+    products(c, Uin, breal, !one_s5);
+    if (one_s5) { fused_s5(c, Uin, rout, mode); return; }
     SpecGeom gp = c->geom(); gp.pruned = 1;
     const cd* Uc[8];
     for (int f = 0; f < 8; ++f) Uc[f] = Uin[f];
@@ -374,6 +412,9 @@ int mhd_set_option(mhd_ctx* c, int option, int value) {
             c->opt_fused = value; return MHD_OK;
         case MHD_OPT_PRUNE: c->opt_prune = value ? 1 : 0; return MHD_OK;
         case MHD_OPT_FUSE_CURRENT: c->opt_fuse_current = value ? 1 : 0; return MHD_OK;
+        case MHD_OPT_FUSE_ASSEMBLE:
+            if (value < 0 || value > 2) return c->fail(MHD_ERR_INVALID_ARG, "fuse_assemble must be 0, 1 or 2");
+            c->opt_fuse_assemble = value; return MHD_OK;
         case MHD_OPT_INTEGRATOR:
             if (value < 0 || value > 2) return c->fail(MHD_ERR_INVALID_ARG, "integrator must be 0, 1 or 2");
             c->integrator = value; c->have_old = false; return MHD_OK;

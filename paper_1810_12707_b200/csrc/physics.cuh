@@ -50,4 +50,31 @@ __device__ __forceinline__ void flux_point(const double (&s)[S_NIN], double (&o)
 // i * k * a  for real k
 __device__ __forceinline__ cd imul(double k, cd a) { return mk(-k * a.y, k * a.x); }
 
+// R^ of one mode (default equation set) from the 16 transformed products, fetched through ld(slot), and the state u[8]:
+// derivative = multiplication by i k (PAPER.md L17 / L25), diffusion = -k^2 (Eq. 18-19).  One definition for
+// assemble_kernel and for the assembly tail of the fused forward z pass, so that both give bitwise the same numbers.
+template <class LD>
+__device__ __forceinline__ void rhs_mode(LD ld, const cd (&u)[8], double kx, double ky, double kz, const Phys& ph, cd (&R)[8]) {
+    const double k2 = kx * kx + ky * ky + kz * kz;
+    const cd txx = ld(P_TXX), txy = ld(P_TXY), txz = ld(P_TXZ);
+    const cd tyy = ld(P_TYY), tyz = ld(P_TYZ), tzz = ld(P_TZZ);
+    const cd ex = ld(P_EX), ey = ld(P_EY), ez = ld(P_EZ);
+    // -i k.F = -(i kx Fx + i ky Fy + i kz Fz)
+    R[0] = mk(0, 0) - (imul(kx, u[1]) + imul(ky, u[2]) + imul(kz, u[3]));
+    R[1] = mk(0, 0) - (imul(kx, txx) + imul(ky, txy) + imul(kz, txz)) - (ph.mu * k2) * ld(P_UX);
+    R[2] = mk(0, 0) - (imul(kx, txy) + imul(ky, tyy) + imul(kz, tyz)) - (ph.mu * k2) * ld(P_UY);
+    R[3] = mk(0, 0) - (imul(kx, txz) + imul(ky, tyz) + imul(kz, tzz)) - (ph.mu * k2) * ld(P_UZ);
+    R[4] = mk(0, 0) - (imul(kx, ld(P_FEX)) + imul(ky, ld(P_FEY)) + imul(kz, ld(P_FEZ))) - (ph.mu * k2) * ld(P_Q);
+    R[5] = imul(ky, ez) - imul(kz, ey) - (ph.eta * k2) * u[5];
+    R[6] = imul(kz, ex) - imul(kx, ez) - (ph.eta * k2) * u[6];
+    R[7] = imul(kx, ey) - imul(ky, ex) - (ph.eta * k2) * u[7];
+}
+// explicit update of one field of one mode: mode 1 Euler, 2 Adams-Bashforth 2 (R6)
+__device__ __forceinline__ cd updated(int mode, double dt, cd u, cd R, cd ro) {
+    cd inc;
+    if (mode == 1) inc = R;
+    else inc = mk(1.5 * R.x - 0.5 * ro.x, 1.5 * R.y - 0.5 * ro.y);
+    return mk(u.x + dt * inc.x, u.y + dt * inc.y);
+}
+
 }  // namespace mhd

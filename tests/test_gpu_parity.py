@@ -121,6 +121,58 @@ def test_rhs_random_state_128_both_fused_kernels(orc, MHD, fused, prune):
     check_rhs(o, g, N)
 
 
+@pytest.mark.parametrize("prune", [1, 0])
+def test_fused_sweep_generations_agree_256(MHD, prune):
+    """The two generations of the fused x sweep (MHD_OPT_FUSED = 1: register-resident real-FFT split; 2: generic tile) and
+    the unfused path (0), and sweep S5 as one launch (cluster kernel) or two (MHD_OPT_FUSE_ASSEMBLE), evaluate the same
+    right-hand side of a random 256^3 state at every grid point, with pruned and with full transforms."""
+    import torch
+    from paper_1810_12707_b200 import binding as b
+    N = 256
+    prim = [torch.from_numpy(p).cuda() for p in inputs.random_smooth_state(N, 21, kmax=6)]
+    ref = None
+    for fused, one_s5 in ((1, 1), (1, 0), (2, 1), (0, 0)):
+        g = MHD(N, mu=0.01, eta=0.02)
+        g.set_option(b.MHD_OPT_FUSED, fused)
+        g.set_option(b.MHD_OPT_FUSE_ASSEMBLE, one_s5)
+        g.set_option(b.MHD_OPT_PRUNE, prune)
+        g.set_fields(prim, "primitive")
+        R = g.rhs(where="device")
+        del g
+        if ref is None:
+            ref = R
+            continue
+        for f in range(8):
+            scale = float(torch.linalg.vector_norm(ref[f]))
+            assert float(torch.linalg.vector_norm(R[f] - ref[f])) <= 1e-12 * max(scale, 1.0), (fused, one_s5, NAMES[f])
+            assert float((R[f] - ref[f]).abs().max()) <= 1e-11 * max(float(ref[f].abs().max()), 1.0), (fused, one_s5, NAMES[f])
+        del R
+        torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("N,steps,variant", [(64, 7, 1), (128, 5, 2), (256, 4, 1), (256, 4, 2), (512, 3, 1), (512, 3, 2)])
+def test_one_launch_sweep_s5_is_bitwise_the_two_launch_path(MHD, N, steps, variant):
+    """Sweep S5 in one launch (forward z pass + assembly + update in clusters of 16 or 8 CTAs, MHD_OPT_FUSE_ASSEMBLE = 1 / 2)
+    gives bitwise the state of the two-launch path (forward z pass, then assemble_kernel): Euler start and AB2 steps."""
+    import torch
+    from paper_1810_12707_b200 import binding as b
+    cfg = inputs.config45(N) if N >= 256 else inputs.config3(N)
+    prim = [torch.from_numpy(p).cuda() for p in cfg.prim]
+    out = []
+    for one_s5 in (variant, 0):
+        g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+        g.set_option(b.MHD_OPT_FUSE_ASSEMBLE, one_s5)
+        g.set_fields(prim, "primitive")
+        l0 = g.launch_count()
+        g.step(steps)
+        per_step = (g.launch_count() - l0) / steps
+        assert per_step == (5 if one_s5 else 6)
+        out.append(g.get_fields(where="device"))
+        del g
+    for f in range(8):
+        assert torch.equal(out[0][f], out[1][f]), NAMES[f]
+
+
 @pytest.mark.parametrize("fused,prune", [(1, 1), (0, 1), (1, 0), (0, 0), (2, 1)])
 def test_rhs_random_state_32(orc, MHD, fused, prune):
     from paper_1810_12707_b200 import binding as b
@@ -578,14 +630,18 @@ def test_full_size_fft3d_plane_waves_every_mode(MHD, N):
     got = torch.view_as_complex(spec)
     err = got - E
     assert float(torch.linalg.vector_norm(err)) <= 1e-14 * float(torch.linalg.vector_norm(E))
-    assert float(err.abs().max()) <= 100 * eps * fnorm               # every single mode, incl. the 99.99 % that are zero
+    # every single mode: the 99.99 % that are exactly zero collect only the rounding noise of the sums (~ eps |f|_2), a
+    # populated mode additionally carries the relative error of its own coefficient (|E| = amp N^3 / 2 >> |f|_2)
+    zero = E == 0
+    assert float(err[zero].abs().max()) <= 100 * eps * fnorm
+    assert float((err[~zero].abs() / E[~zero].abs()).max()) <= 100 * eps
     # pruned forward transform: the modes inside the mask, everything else untouched
     spec_p = torch.full((N, N, H, 2), 7.0, dtype=torch.float64, device="cuda")
     g.fft3d_r2c([f], [spec_p], None, prune=True)
     n = torch.fft.fftfreq(N, 1.0 / N, device="cuda").round().long().abs()
     m3 = (n[:, None, None] <= kc) & (n[None, :, None] <= kc) & (torch.arange(H, device="cuda")[None, None, :] <= kc)
     gp = torch.view_as_complex(spec_p)
-    assert float((gp[m3] - E[m3]).abs().max()) <= 100 * eps * fnorm
+    assert float((gp[m3] - E[m3]).abs().max()) <= 100 * eps * max(fnorm, float(E.abs().max()))
     assert bool(torch.all(spec_p[~m3] == 7.0))
     # inverse: exact spectrum in, every grid point compared with the synthesised field
     out = torch.empty((N, N, N), dtype=torch.float64, device="cuda")
@@ -748,6 +804,10 @@ def test_config6_1024_maximum_size(MHD, placement):
     import torch
     from paper_1810_12707_b200 import binding as b
     nsteps = 10
+    gc.collect()
+    torch.cuda.empty_cache()
+    if hasattr(torch._C, "_host_emptyCache"):     # pinned blocks that earlier tests left in torch's caching host allocator
+        torch._C._host_emptyCache()
     c5 = inputs.config6(512)
     ref = MHD(c5.N, c5.L, c5.gamma, c5.mu, c5.eta, c5.dt)
     ref.set_fields(c5.prim, "primitive")
@@ -762,6 +822,11 @@ def test_config6_1024_maximum_size(MHD, placement):
     flags = b.MHD_FLAG_OUT_OF_CORE
     if placement == "host":
         flags |= b.MHD_FLAG_STATE_ON_HOST | b.MHD_FLAG_WORK_ON_HOST
+        # the initial fields (69 GB) wait in HBM, which this placement leaves almost empty, so that the host never holds
+        # them and the 103 GB pinned block at the same time
+        for f in range(8):
+            cfg.prim[f] = torch.from_numpy(cfg.prim[f]).cuda()
+        gc.collect()
     g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, flags=flags)
     if placement == "host":
         assert g.workspace_bytes < 16e9 and g.pinned_bytes > 100e9      # field storage is on the host, not in HBM
