@@ -7,10 +7,11 @@ A "step" is one explicit time step (one pass of the whole hot path: sweeps S1-S5
 config of BASELINE.json (config 5; `--size 256` gives config 4).  Inputs are seeded and synthetic.
   value        N^3 * K * n_gpus / (max over ranks of the device time of mhd_step(K)), state resident in HBM
   e2e          same metric through the C ABI with HOST (pinned) buffers: set_fields + step(K) + get_fields
-  roofline     dominant kernel family (the fused x sweep: fp64-issue bound -> "alu": fp64 instr/s vs the measured issue
-               rate; its HBM view under roofline.hbm), every family's algorithmic bytes / CUDA-event time vs the measured
-               HBM peak, and whole-step fractions
-  cpu_baseline the CPU oracle, as it stands, on a bounded sample (64^3 grid of the same config)
+  roofline     the dominant kernel family, SURVEY.md 8(d) style: algorithmic bytes per launch / CUDA-event time per launch
+               against the measured HBM copy peak (MEASURED_PEAKS.json); `alu` = the same kernel on FLOPS (8(d) count)
+               against twice the DFMA rate measured in this run; every family and the whole step beside it
+  size_256     the other size the metric is quoted on (config 4, 256^3), measured in the same run
+  cpu_baseline the CPU oracle, as it stands, on a bounded sample (128^3 grid of the same config), all cores and one thread
 Multi-GPU: the path does not shard without an all-to-all: `--gpus N` runs N independent
 replicas (weak scaling), one process per GPU under torchrun, timed as the max over ranks.
 `--impl reference` times the oracle (the reference arm of this tier) on the host cores of rank 0.
@@ -32,9 +33,7 @@ if ROOT not in sys.path:
 
 METRIC = "fp64 grid-point-steps/s"
 UNIT = "grid-point-steps/s"
-# fp64 instructions the fused x sweep executes per (y,z) line, from the committed ncu capture (profiles/r01b_ncu_full_*.md:
-# fp64 pipe busy fraction x 2 warp-instructions/clk/SM x active cycles); DESIGN.md section 6 derives the same figure by hand
-X_FUSED_FP64_INSTR_PER_LINE = {512: 312.0e3, 256: 141.3e3}
+TRAFFIC_FILE = os.path.join("profiles", "traffic_r02.json")   # ncu DRAM bytes per launch of the committed capture
 FALLBACK_HBM_GBS = 6650.0   # /opt/skills/guides/B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
 
 
@@ -111,7 +110,13 @@ def aggregate(ms_local: float, units_local: float, dist=None):
 # ----------------------------------------------------------------------------------------------------------------
 # algorithmic bytes per launch; one field-sweep = 8 B per grid point
 # ----------------------------------------------------------------------------------------------------------------
-def sweep_bytes(N: int, prune: bool, fuse_current: bool = True):
+def fused_flops_per_line(N: int) -> float:
+    """SURVEY.md 8(d) flop count of the fused x sweep per (y,z) line: 27 real line transforms at 2.5 N log2 N each
+    plus ~90 flop per grid point of point-wise products."""
+    return 27 * 2.5 * N * math.log2(N) + 90.0 * N
+
+
+def sweep_bytes(N: int, prune: bool, fuse_current: bool = True, fuse_s5: bool = False):
     """Per-family algorithmic bytes of ONE right-hand side: what the kernels must read + write."""
     kc = N // 3
     H = N // 2
@@ -125,8 +130,12 @@ def sweep_bytes(N: int, prune: bool, fuse_current: bool = True):
         b["build_current"] = (3 + 3) * f * ah * a * a
         b["strided_inverse"] = 11 * f * ah * (a * a + a) + 11 * f * ah * (a + 1.0)
     b["x_fused"] = (11 + 16) * f * ah
-    b["strided_forward"] = 16 * f * ah * (1.0 + a) + 16 * f * ah * (a + a * a)       # y pass, z pass
-    b["assemble"] = (16 + 8 + 8 + 8 + 8) * f * ah * a * a
+    if fuse_s5:          # sweep S5 in one launch: reads 16 z-full products + U^ + R^old, writes U^ + R^old
+        b["strided_forward"] = 16 * f * ah * (1.0 + a)                                # y pass
+        b["forward_z_assemble"] = 16 * f * ah * a + (8 + 8 + 8 + 8) * f * ah * a * a
+    else:
+        b["strided_forward"] = 16 * f * ah * (1.0 + a) + 16 * f * ah * (a + a * a)    # y pass, z pass
+        b["assemble"] = (16 + 8 + 8 + 8 + 8) * f * ah * a * a
     return b
 
 
@@ -168,19 +177,31 @@ def run_reference(args):
 
 
 def cpu_baseline(size):
+    """The oracle as it stands on a bounded sample: 128^3 grid of the same initial condition, all host cores (the headline
+    `value`) and one thread (single-thread and all-cores)."""
     import oracle
     from paper_1810_12707_b200 import inputs
-    n, steps = 128, 12
-    cfg = inputs.config45(n)
-    o = oracle.Oracle(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
-    o.set_fields(cfg.prim, "primitive")
-    o.step(1)
-    t0 = time.perf_counter()
-    o.step(steps)
-    dt = time.perf_counter() - t0
-    return {"value": n ** 3 * steps / dt, "unit": UNIT, "cores": oracle.get_threads(), "kind": "oracle",
+    all_cores = oracle.get_threads()
+    res = {}
+    for label, threads, n, steps in (("all_cores", all_cores, 128, 10), ("single_thread", 1, 64, 3)):
+        cfg = inputs.config45(n)
+        oracle.set_threads(threads)
+        o = oracle.Oracle(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
+        o.set_fields(cfg.prim, "primitive")
+        o.step(1)
+        t0 = time.perf_counter()
+        o.step(steps)
+        dt = time.perf_counter() - t0
+        res[label] = {"value": n ** 3 * steps / dt, "cores": threads, "steps": steps, "seconds": dt, "n": n}
+        o.close()
+    oracle.set_threads(all_cores)
+    a = res["all_cores"]
+    return {"value": a["value"], "unit": UNIT, "cores": a["cores"], "kind": "oracle",
             "sample": "config 4/5 initial condition on a %d^3 grid, %d AB2 steps, %.1f s (bounded sample of the %d^3 workload)"
-                      % (n, steps, dt, size)}
+                      % (a["n"], a["steps"], a["seconds"], size),
+            "single_thread": {"value": res["single_thread"]["value"], "cores": 1,
+                              "sample": "%d^3 grid, %d AB2 steps, %.1f s" % (res["single_thread"]["n"], res["single_thread"]["steps"],
+                                                                             res["single_thread"]["seconds"])}}
 
 
 def time_steps(g, torch, nsteps, dist):
@@ -198,7 +219,7 @@ def time_steps(g, torch, nsteps, dist):
     return e0.elapsed_time(e1)
 
 
-def fft_metric(g, torch, N, nf=8, reps=5):
+def fft_metric(g, torch, N, peak, nf=8, reps=5):
     """Stand-alone batched 3-D R2C + C2R (BASELINE.json: '3D FFT achieved HBM GB/s vs peak')."""
     H = N // 2
     real = [torch.randn((N, N, N), dtype=torch.float64, device=g.device) for _ in range(nf)]
@@ -215,23 +236,25 @@ def fft_metric(g, torch, N, nf=8, reps=5):
             e1.record(g.stream)
             torch.cuda.synchronize()
             ms = e0.elapsed_time(e1) / reps
-            out[name + ("_pruned" if prune else "")] = {"ms_per_field": ms / nf,
-                                                         "gbs_3pass_48B_per_pt": 48.0 * N ** 3 * nf / ms / 1e6,
+            gbs = 48.0 * N ** 3 * nf / ms / 1e6
+            out[name + ("_pruned" if prune else "")] = {"ms_per_field": ms / nf, "gbs_3pass_48B_per_pt": gbs,
+                                                         "frac_of_peak_3pass": gbs / peak,
                                                          "gbs_1r1w_16B_per_pt": 16.0 * N ** 3 * nf / ms / 1e6}
     # cuFFT (via torch.fft) as a timing reference only — never on the product path
     x = real[0]
     del spec, real                                       # cuFFT needs its own work area: give the memory back first
     y = torch.empty((N, N, H + 1), dtype=torch.complex128, device=g.device)
-    for _ in range(2):
+    for _ in range(3):
         torch.fft.rfftn(x, out=y)
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
-    for _ in range(reps):
+    for _ in range(4 * reps):
         torch.fft.rfftn(x, out=y)
     e1.record()
     torch.cuda.synchronize()
-    out["cufft_d2z_reference_ms_per_field"] = e0.elapsed_time(e1) / reps
+    out["cufft_d2z_reference_ms_per_field"] = e0.elapsed_time(e1) / (4 * reps)
+    out["accounting"] = "SURVEY.md 8(d): 3 passes x (8 B read + 8 B written) = 48 B per point and transform; peak = %.0f GB/s measured copy" % peak
     del y, x
     return out
 
@@ -291,6 +314,90 @@ def pcie_peaks(torch, device, nbytes=1 << 30, reps=4):
 
     run(True, True)
     return {"h2d_alone_gbs": run(True, False), "d2h_alone_gbs": run(False, True), "each_direction_when_both_gbs": run(True, True)}
+
+
+def hbm_peak():
+    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(peaks_path):
+        return float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def build_roofline(g, N, K, step_ms, prof, peak, peak_src, fuse_current=True, fuse_s5=False, in_core=True):
+    """per kernel family, algorithmic bytes per launch / CUDA-event time per launch against the HBM copy
+    peak; the dominant family (largest share of the step) is the top-level object."""
+    sb = sweep_bytes(N, prune=True, fuse_current=fuse_current, fuse_s5=fuse_s5)
+    fam = {}
+    for name, b in sb.items():
+        p = prof.get(name, {"ms": 0.0, "launches": 0})
+        if p["launches"] == 0:
+            continue
+        per_launch_bytes = b * K / p["launches"]
+        avg_ms = p["ms"] / p["launches"]
+        fam[name] = {"ms_per_step": p["ms"] / K, "launches_per_step": p["launches"] / K,
+                     "alg_bytes_per_launch": per_launch_bytes, "avg_launch_ms": avg_ms,
+                     "gbs": per_launch_bytes / avg_ms / 1e6, "frac_of_peak": per_launch_bytes / avg_ms / 1e6 / peak}
+    if not fam:
+        return None
+    dom = max(fam, key=lambda k: fam[k]["ms_per_step"])
+    alg_pruned = sum(sb.values())
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": fam[dom]["gbs"], "peak": peak, "unit": "GB/s",
+                "frac": fam[dom]["frac_of_peak"], "traffic": None, "peak_source": peak_src,
+                "share_of_step": fam[dom]["ms_per_step"] / step_ms,
+                "whole_step": {"alg_bytes_pruned": alg_pruned, "gbs_pruned": alg_pruned / step_ms / 1e6,
+                               "frac_pruned": alg_pruned / step_ms / 1e6 / peak,
+                               "alg_bytes_unpruned_1184B": unpruned_reference_bytes(N),
+                               "gbs_vs_1184B": unpruned_reference_bytes(N) / step_ms / 1e6,
+                               "frac_vs_1184B": unpruned_reference_bytes(N) / step_ms / 1e6 / peak,
+                               "frac_vs_1184B_nominal_8TBs": unpruned_reference_bytes(N) / step_ms / 1e6 / 8000.0},
+                "families": fam}
+    tpath = os.path.join(ROOT, TRAFFIC_FILE)
+    if os.path.exists(tpath):   # DRAM bytes per launch from the committed ncu capture: NOT measured in this run
+        try:
+            tj = json.load(open(tpath))
+            tr = tj.get(str(N), {})
+            roofline["traffic"] = tr.get(dom)
+            roofline["traffic_source"] = "%s (ncu dram__bytes_read + dram__bytes_write per launch, capture of commit %s; not measured in this run)" % (
+                TRAFFIC_FILE, tj.get("commit", "?"))
+            if in_core and all(k in tr for k in fam):
+                roofline["whole_step"]["dram_bytes_measured_ncu"] = sum(tr[k] * fam[k]["launches_per_step"] for k in fam)
+        except Exception:
+            pass
+    if "x_fused" in fam and in_core:
+        # the fused x sweep on FLOPS: SURVEY.md 8(d) count (27 x 2.5 N log2 N + 90 N per line) against twice the DFMA
+        # instruction rate of the fp64 pipe, measured in this run by a register-only FMA kernel (mhd_probe_fp64)
+        flops = fused_flops_per_line(N) * N * N
+        peak_f = 2.0 * g.probe_fp64()
+        ach = flops / (fam["x_fused"]["avg_launch_ms"] * 1e-3)
+        roofline["alu"] = {"bound": "alu", "kernel": "x_fused", "achieved": ach / 1e12, "peak": peak_f / 1e12, "unit": "TFLOP/s (fp64)",
+                           "frac": ach / peak_f, "flops_per_line": fused_flops_per_line(N),
+                           "flop_count": "SURVEY.md 8(d): 27 real line transforms x 2.5 N log2 N + 90 N point-wise, per (y,z) line",
+                           "peak_source": "2 x the DFMA rate of a register-only kernel measured in this run (mhd_probe_fp64); "
+                                          "64 lanes/clk/SM x 148 SMs x 1.965 GHz x 2 = %.1f TFLOP/s" % (148 * 64 * 1.965e9 * 2 / 1e12)}
+    return roofline
+
+
+def measure_other_size(MHD, inputs, torch, N, device, peak, peak_src, steps=50, warm=5):
+    """The second size the metric is quoted on, measured in the same run: value, ms per step, family fractions."""
+    cfg = inputs.config45(N)
+    g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, device=device)
+    g.set_fields([torch.from_numpy(p).to(device) for p in cfg.prim], "primitive")
+    g.step(warm)
+    g.profile_enable(True)
+    ms = time_steps(g, torch, steps, None)
+    prof = g.profile_get()
+    g.profile_enable(False)
+    r = build_roofline(g, N, steps, ms / steps, prof, peak, peak_src)
+    out = {"workload": "config4_abc_dynamo_%d^3" % N, "value": float(N) ** 3 * steps / (ms * 1e-3), "unit": UNIT,
+           "ms_per_step": ms / steps, "steps": steps, "warmup": warm,
+           "roofline": {k: r[k] for k in ("bound", "kernel", "achieved", "peak", "unit", "frac", "share_of_step", "traffic")},
+           "families": {k: {"ms_per_step": v["ms_per_step"], "frac_of_peak": v["frac_of_peak"]} for k, v in r["families"].items()},
+           "whole_step": r["whole_step"]}
+    if "alu" in r:
+        out["alu"] = {k: r["alu"][k] for k in ("achieved", "peak", "unit", "frac")}
+    del g
+    torch.cuda.empty_cache()
+    return out
 
 
 def run_ours(args):
@@ -386,62 +493,11 @@ def run_ours(args):
     value = units / (ms_max * 1e-3)
 
     # ---- roofline of the dominant kernel family ---------------------------------------------------------------
-    peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    if os.path.exists(peaks_path):
-        peak, peak_src = float(json.load(open(peaks_path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
-    else:
-        peak, peak_src = FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
-    sb = sweep_bytes(N, prune=True, fuse_current=opts.get(4, 1) != 0)
-    fam = {}
-    for name, b in sb.items():
-        p = prof.get(name, {"ms": 0.0, "launches": 0})
-        if p["launches"] == 0:
-            continue
-        per_launch_bytes = b * K / p["launches"]
-        avg_ms = p["ms"] / p["launches"]
-        fam[name] = {"ms_per_step": p["ms"] / K, "launches_per_step": p["launches"] / K,
-                     "alg_bytes_per_launch": per_launch_bytes, "avg_launch_ms": avg_ms,
-                     "gbs": per_launch_bytes / avg_ms / 1e6, "frac_of_peak": per_launch_bytes / avg_ms / 1e6 / peak}
-    dom = max(fam, key=lambda k: fam[k]["ms_per_step"]) if fam else None
-    step_ms_local = ms / K
-    alg_pruned = sum(sb.values())
-    roofline = None
-    if dom:
-        roofline = {"bound": "hbm", "kernel": dom, "achieved": fam[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                    "frac": fam[dom]["frac_of_peak"], "traffic": None, "peak_source": peak_src,
-                    "share_of_step": fam[dom]["ms_per_step"] / step_ms_local,
-                    "whole_step": {"alg_bytes_pruned": alg_pruned, "gbs_pruned": alg_pruned / step_ms_local / 1e6,
-                                   "frac_pruned": alg_pruned / step_ms_local / 1e6 / peak,
-                                   "alg_bytes_unpruned_1184B": unpruned_reference_bytes(N),
-                                   "gbs_vs_1184B": unpruned_reference_bytes(N) / step_ms_local / 1e6,
-                                   "frac_vs_1184B": unpruned_reference_bytes(N) / step_ms_local / 1e6 / peak,
-                                   "frac_vs_1184B_nominal_8TBs": unpruned_reference_bytes(N) / step_ms_local / 1e6 / 8000.0},
-                    "families": fam}
-        tpath = os.path.join(ROOT, "profiles", "traffic_r01.json")
-        if os.path.exists(tpath):   # DRAM bytes per launch from the committed ncu --set full capture
-            try:
-                tr = json.load(open(tpath)).get(str(N), {})
-                roofline["traffic"] = tr.get(dom)
-                if not flags and all(k in tr for k in fam):
-                    # measured DRAM bytes of one whole step (ncu) beside the algorithmic bytes
-                    roofline["whole_step"]["dram_bytes_measured_ncu"] = sum(tr[k] * fam[k]["launches_per_step"] for k in fam)
-            except Exception:
-                pass
-        if dom == "x_fused" and N in X_FUSED_FP64_INSTR_PER_LINE and not flags:
-            # The dominant kernel is bound by fp64 issue, not by HBM: its roofline is the ALU one —
-            # fp64 instructions per second against the issue rate of the fp64 pipe.  The B200 guides give no fp64 unit
-            # count, so the peak is MEASURED in this run (register-only DFMA kernel); the figure derived
-            # from 64 lanes/clk/SM x 148 SMs x 1.965 GHz is given beside it.  The HBM view of the same kernel is kept.
-            peak_i = g.probe_fp64()
-            ach_i = X_FUSED_FP64_INSTR_PER_LINE[N] * N * N / (fam["x_fused"]["avg_launch_ms"] * 1e-3)
-            hbm_view = {k: roofline[k] for k in ("bound", "achieved", "peak", "unit", "frac", "peak_source")}
-            roofline.update({"bound": "alu", "achieved": ach_i / 1e9, "peak": peak_i / 1e9, "unit": "Ginstr/s (fp64 pipe)",
-                             "frac": ach_i / peak_i,
-                             "peak_source": "measured in this run: register-only DFMA kernel (mhd_probe_fp64)",
-                             "peak_derived_64_lanes_per_clk_per_sm": 148 * 64 * 1.965,
-                             "frac_vs_derived_peak": ach_i / (148 * 64 * 1.965e9),
-                             "instr_per_line": X_FUSED_FP64_INSTR_PER_LINE[N], "hbm": hbm_view})
-            roofline["alu"] = {k: roofline[k] for k in ("bound", "kernel", "achieved", "peak", "unit", "frac", "peak_source")}
+    peak, peak_src = hbm_peak()
+    fuse_s5 = opts.get(7, 0) != 0
+    roofline = build_roofline(g, N, K, ms / K, prof, peak, peak_src, fuse_current=opts.get(4, 1) != 0, fuse_s5=fuse_s5,
+                              in_core=not flags)
+    alg_pruned = sum(sweep_bytes(N, True, opts.get(4, 1) != 0, fuse_s5).values())
 
     # ---- end to end through the C ABI with host buffers ----------------------------------------------------------
     e2e = None
@@ -465,9 +521,13 @@ def run_ours(args):
     extra = {}
     if rank == 0 and not args.no_fft and not flags:
         host = None
-        extra["fft3d"] = fft_metric(g, torch, N)
+        extra["fft3d"] = fft_metric(g, torch, N, peak)
     if rank == 0 and args.tracers > 0 and not flags:
         extra["tracers"] = tracer_metric(g, torch, N, cfg.L, args.tracers, K, ms / K)
+    if rank == 0 and world == 1 and not flags and N == 512 and not args.no_256 and not opts:
+        g = None
+        torch.cuda.empty_cache()
+        extra["size_256"] = measure_other_size(MHD, inputs, torch, 256, "cuda:%d" % local_rank, peak, peak_src)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
         cpu = cpu_baseline(N)
@@ -478,7 +538,7 @@ def run_ours(args):
                 "dtype": "f64", "data": "synthetic",
                 "config": {"workload": ("config6_turbulence_out_of_core_%d^3" % N) if N == 1024 else
                            "config%d_abc_dynamo_%d^3" % (5 if N == 512 else 4, N), "N": N, "dt": cfg.dt, "placement": args.placement,
-                           "mu": cfg.mu, "eta": cfg.eta, "integrator": "AB2", "fused": 1, "pruned": 1,
+                           "mu": cfg.mu, "eta": cfg.eta, "integrator": "AB2", "options": opts, "pruned": 1,
                            "parallelism": ("slab decomposition x%d" if args.decompose else "replicas x%d") % world,
                            "l2": "no flush: one step streams %.1f GB, far beyond the 126 MB L2" % (alg_pruned / 1e9)},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "out_of_core": ooc,
@@ -506,6 +566,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-fft", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-256", action="store_true", help="skip the 256^3 measurement that the default 512^3 run adds")
     ap.add_argument("--decompose", action="store_true",
                     help="with --gpus N under torchrun: ONE problem decomposed over the N GPUs (ky bricks / z slabs, two NCCL "
                          "all-to-alls per step) instead of N replicas; with N = 1 it measures the pack / unpack overhead")

@@ -21,6 +21,7 @@ MHD_HOST, MHD_DEVICE = 0, 1
 MHD_CONSERVATIVE, MHD_PRIMITIVE = 0, 1
 MHD_OPT_FUSED, MHD_OPT_PRUNE, MHD_OPT_INTEGRATOR, MHD_OPT_FUSE_CURRENT, MHD_OPT_OOC_BRICK, MHD_OPT_OOC_SLAB = 1, 2, 3, 4, 5, 6
 MHD_OPT_FUSE_ASSEMBLE = 7
+MHD_OPT_TMA = 13
 MHD_FLAG_OUT_OF_CORE, MHD_FLAG_STATE_ON_HOST, MHD_FLAG_WORK_ON_HOST = 1, 2, 4
 
 

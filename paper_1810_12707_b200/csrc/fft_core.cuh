@@ -213,13 +213,23 @@ struct LayoutSwz {          // tile[n][SL] with the low 3 slot bits XOR-swizzled
     __device__ __forceinline__ int operator()(int n) const { return n * SL + (slot ^ (n & 7)); }
 };
 
+// barrier policies of the exchange: the whole CTA, or a named barrier shared by one group of warps (several
+// independent transforms per CTA: the TMA-pipelined strided passes)
+struct BlockSync {
+    __device__ __forceinline__ void operator()() const { __syncthreads(); }
+};
+struct GroupSync {
+    int id, nthreads;       // barrier 1..15, threads of the group (multiple of 32)
+    __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
+};
+
 // one stage: butterflies on registers; non-final stages scatter to shared memory and gather back
-template <int NL, int R, int NSTRIDE /*Ns*/, bool LAST, bool FIRST, int DIR, int TWS, class Layout>
+template <int NL, int R, int NSTRIDE /*Ns*/, bool LAST, bool FIRST, int DIR, int TWS, class Layout, class Sync>
 __device__ __forceinline__ void fft_stage(cd (&v)[PlanInfo<NL>::E], int t, const cd* __restrict__ tw, cd* sm,
-                                          const Layout& L) {
+                                          const Layout& L, const Sync& sync) {
     constexpr int E = PlanInfo<NL>::E, T = PlanInfo<NL>::T, B = E / R;
     static_assert(E % R == 0, "radix must divide the points per thread");
-    if constexpr (!LAST && !FIRST) __syncthreads();   // every thread has gathered the previous exchange
+    if constexpr (!LAST && !FIRST) sync();   // every thread has gathered the previous exchange
 #pragma unroll
     for (int b = 0; b < B; ++b) {
         const int j = t + b * T;
@@ -244,7 +254,7 @@ __device__ __forceinline__ void fft_stage(cd (&v)[PlanInfo<NL>::E], int t, const
         }
     }
     if constexpr (!LAST) {
-        __syncthreads();
+        sync();
 #pragma unroll
         for (int m = 0; m < E; ++m) v[m] = sm[L(t + T * m)];
     }
@@ -252,20 +262,20 @@ __device__ __forceinline__ void fft_stage(cd (&v)[PlanInfo<NL>::E], int t, const
 
 // Whole line transform on registers.  On entry v[m] = x[t + T*m]; on exit v[m] = X[t + T*m] with
 // X[q] = sum_n x[n] exp(DIR*2*pi*i*n*q/NL) (unnormalised).  `sm` is the exchange tile (must be free on entry;
-// all threads of the block must call).  tw[m*TWS] = exp(-2*pi*i*m/NL).
-template <int NL, int DIR, int TWS, class Layout>
+// all threads of the block — or of the group that `sync` joins — must call).  tw[m*TWS] = exp(-2*pi*i*m/NL).
+template <int NL, int DIR, int TWS, class Layout, class Sync = BlockSync>
 __device__ __forceinline__ void fft_line(cd (&v)[PlanInfo<NL>::E], int t, const cd* __restrict__ tw, cd* sm,
-                                         const Layout& L) {
+                                         const Layout& L, const Sync& sync = Sync()) {
     typedef Plan<NL> P;
     if constexpr (P::NS == 1) {
-        fft_stage<NL, P::R0, 1, true, true, DIR, TWS>(v, t, tw, sm, L);
+        fft_stage<NL, P::R0, 1, true, true, DIR, TWS>(v, t, tw, sm, L, sync);
     } else if constexpr (P::NS == 2) {
-        fft_stage<NL, P::R0, 1, false, true, DIR, TWS>(v, t, tw, sm, L);
-        fft_stage<NL, P::R1, P::R0, true, false, DIR, TWS>(v, t, tw, sm, L);
+        fft_stage<NL, P::R0, 1, false, true, DIR, TWS>(v, t, tw, sm, L, sync);
+        fft_stage<NL, P::R1, P::R0, true, false, DIR, TWS>(v, t, tw, sm, L, sync);
     } else {
-        fft_stage<NL, P::R0, 1, false, true, DIR, TWS>(v, t, tw, sm, L);
-        fft_stage<NL, P::R1, P::R0, false, false, DIR, TWS>(v, t, tw, sm, L);
-        fft_stage<NL, P::R2, P::R0 * P::R1, true, false, DIR, TWS>(v, t, tw, sm, L);
+        fft_stage<NL, P::R0, 1, false, true, DIR, TWS>(v, t, tw, sm, L, sync);
+        fft_stage<NL, P::R1, P::R0, false, false, DIR, TWS>(v, t, tw, sm, L, sync);
+        fft_stage<NL, P::R2, P::R0 * P::R1, true, false, DIR, TWS>(v, t, tw, sm, L, sync);
     }
 }
 

@@ -70,6 +70,19 @@ struct StridedArgs {
 // dir = -1 forward, +1 inverse (unnormalised both ways)
 void launch_strided(int N, int dir, const StridedArgs& a, cudaStream_t st);
 
+// The same in-core passes as a persistent, TMA-fed pipeline (kernels_strided_tma.cu): N = 128, 256, 512, arrays that are
+// field buffers of the workspace (tensor maps are built over it at bind time), no fused current, no peer stores.
+struct StridedTma {
+    const void* maps = nullptr;    // 4 CUtensorMap: (rows = y | z) x (box rows = kc + 1 | N / 2), or null: not available
+    const void* base = nullptr;    // first field buffer
+    size_t stride_bytes = 0;       // distance between field buffers
+    int nbuf = 0;                  // number of field buffers
+    int sms = 0;                   // CTAs of the persistent grid (= multiprocessors of the device)
+};
+bool strided_tma_supported(int N);
+bool strided_tma_build_maps(int N, void* base, size_t stride_bytes, int nbuf, void* maps_out);
+bool launch_strided_tma(int N, int dir, const StridedArgs& a, const StridedTma& tm, cudaStream_t st);   // false: not eligible
+
 // Sweep S5 as ONE launch (north_star (4): "the explicit time integrator fused into the last spectral
 // pass"): the in-core forward z pass of the 16 product fields in thread-block clusters of 16 — one CTA per field of a
 // (ky, kx tile) column — which keep the transformed rows in shared memory, meet at a cluster barrier and assemble R^

@@ -56,7 +56,9 @@ void strided_pass(mhd_ctx* c, int dir, int axis, int nf, const cd* const in[], c
         a.in_rows = (prune && dir > 0) ? 1 : 0;     // inverse: input rows outside the mask are zero
         a.out_rows = (prune && dir < 0) ? 1 : 0;    // forward: output rows outside the mask are not needed
         mhd_ctx::Scope s(c, dir > 0 ? F_STRIDED_INV : F_STRIDED_FWD);
-        launch_strided(N, dir, a, c->st);
+        // MHD_OPT_TMA: 1 = where it measured at least as fast (N = 512), 2 = wherever the pipeline exists, 0 = never
+        const bool tma = (c->opt_tma == 2 || (c->opt_tma == 1 && N == 512)) && zoff == 0;
+        if (!(tma && launch_strided_tma(N, dir, a, c->tma, c->st))) launch_strided(N, dir, a, c->st);
         done += nb;
     }
 }
@@ -398,6 +400,13 @@ int mhd_bind(mhd_ctx* c, void* dev_workspace, size_t bytes, void* cuda_stream, u
     launch_twiddle_table(c->N, c->tw, c->st);
     launch_x_fused2_tables(c->N, c->ftw, c->st);
     c->launches += 2;
+    c->tma = StridedTma();
+    if (strided_tma_supported(c->N) && strided_tma_build_maps(c->N, fp, fb, NFIELD_BUFS, c->tmaps)) {
+        int dev = 0, sms = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        c->tma.maps = c->tmaps; c->tma.base = fp; c->tma.stride_bytes = fb; c->tma.nbuf = NFIELD_BUFS; c->tma.sms = sms;
+    }
     int rc = check_cuda(c, "bind");
     if (rc) return rc;
     c->bound = true; c->have_fields = false; c->have_old = false; c->step = 0;
@@ -412,6 +421,9 @@ int mhd_set_option(mhd_ctx* c, int option, int value) {
             c->opt_fused = value; return MHD_OK;
         case MHD_OPT_PRUNE: c->opt_prune = value ? 1 : 0; return MHD_OK;
         case MHD_OPT_FUSE_CURRENT: c->opt_fuse_current = value ? 1 : 0; return MHD_OK;
+        case MHD_OPT_TMA:
+            if (value < 0 || value > 2) return c->fail(MHD_ERR_INVALID_ARG, "tma must be 0, 1 or 2");
+            c->opt_tma = value; return MHD_OK;
         case MHD_OPT_FUSE_ASSEMBLE:
             if (value < 0 || value > 2) return c->fail(MHD_ERR_INVALID_ARG, "fuse_assemble must be 0, 1 or 2");
             c->opt_fuse_assemble = value; return MHD_OK;
