@@ -323,7 +323,7 @@ def hbm_peak():
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
-def build_roofline(g, N, K, step_ms, prof, peak, peak_src, fuse_current=True, fuse_s5=False, in_core=True):
+def build_roofline(g, N, K, step_ms, prof, peak, peak_src, fuse_current=True, fuse_s5=False, in_core=True, rhs_per_step=1):
     """per kernel family, algorithmic bytes per launch / CUDA-event time per launch against the HBM copy
     peak; the dominant family (largest share of the step) is the top-level object."""
     sb = sweep_bytes(N, prune=True, fuse_current=fuse_current, fuse_s5=fuse_s5)
@@ -332,7 +332,7 @@ def build_roofline(g, N, K, step_ms, prof, peak, peak_src, fuse_current=True, fu
         p = prof.get(name, {"ms": 0.0, "launches": 0})
         if p["launches"] == 0:
             continue
-        per_launch_bytes = b * K / p["launches"]
+        per_launch_bytes = b * rhs_per_step * K / p["launches"]
         avg_ms = p["ms"] / p["launches"]
         fam[name] = {"ms_per_step": p["ms"] / K, "launches_per_step": p["launches"] / K,
                      "alg_bytes_per_launch": per_launch_bytes, "avg_launch_ms": avg_ms,
@@ -340,7 +340,7 @@ def build_roofline(g, N, K, step_ms, prof, peak, peak_src, fuse_current=True, fu
     if not fam:
         return None
     dom = max(fam, key=lambda k: fam[k]["ms_per_step"])
-    alg_pruned = sum(sb.values())
+    alg_pruned = sum(sb.values()) * rhs_per_step
     roofline = {"bound": "hbm", "kernel": dom, "achieved": fam[dom]["gbs"], "peak": peak, "unit": "GB/s",
                 "frac": fam[dom]["frac_of_peak"], "traffic": None, "peak_source": peak_src,
                 "share_of_step": fam[dom]["ms_per_step"] / step_ms,
@@ -448,6 +448,9 @@ def run_ours(args):
     host = [torch.from_numpy(p).pin_memory() if pin_inputs else torch.from_numpy(p) for p in cfg.prim]
     cfg.prim = None
     opts = {}
+    integ = {"ab2": 0, "rk4": 1, "pc": 2}[args.integrator]
+    if integ:
+        g.set_option(3, integ)      # MHD_OPT_INTEGRATOR
     for kv in args.option:
         k, v = kv.split("=")
         opts[int(k)] = int(v)
@@ -496,8 +499,8 @@ def run_ours(args):
     peak, peak_src = hbm_peak()
     fuse_s5 = opts.get(7, 0) != 0
     roofline = build_roofline(g, N, K, ms / K, prof, peak, peak_src, fuse_current=opts.get(4, 1) != 0, fuse_s5=fuse_s5,
-                              in_core=not flags)
-    alg_pruned = sum(sweep_bytes(N, True, opts.get(4, 1) != 0, fuse_s5).values())
+                              in_core=not flags, rhs_per_step={"ab2": 1, "rk4": 4, "pc": 2}[args.integrator])
+    alg_pruned = sum(sweep_bytes(N, True, opts.get(4, 1) != 0, fuse_s5).values()) * {"ab2": 1, "rk4": 4, "pc": 2}[args.integrator]
 
     # ---- end to end through the C ABI with host buffers ----------------------------------------------------------
     e2e = None
@@ -524,7 +527,7 @@ def run_ours(args):
         extra["fft3d"] = fft_metric(g, torch, N, peak)
     if rank == 0 and args.tracers > 0 and not flags:
         extra["tracers"] = tracer_metric(g, torch, N, cfg.L, args.tracers, K, ms / K)
-    if rank == 0 and world == 1 and not flags and N == 512 and not args.no_256 and not opts:
+    if rank == 0 and world == 1 and not flags and N == 512 and not args.no_256 and not opts and not integ:
         g = None
         torch.cuda.empty_cache()
         extra["size_256"] = measure_other_size(MHD, inputs, torch, 256, "cuda:%d" % local_rank, peak, peak_src)
@@ -538,7 +541,8 @@ def run_ours(args):
                 "dtype": "f64", "data": "synthetic",
                 "config": {"workload": ("config6_turbulence_out_of_core_%d^3" % N) if N == 1024 else
                            "config%d_abc_dynamo_%d^3" % (5 if N == 512 else 4, N), "N": N, "dt": cfg.dt, "placement": args.placement,
-                           "mu": cfg.mu, "eta": cfg.eta, "integrator": "AB2", "options": opts, "pruned": 1,
+                           "mu": cfg.mu, "eta": cfg.eta, "integrator": args.integrator.upper(), "rhs_per_step": {"ab2": 1, "rk4": 4, "pc": 2}[args.integrator],
+                           "options": opts, "pruned": 1,
                            "parallelism": ("slab decomposition x%d" if args.decompose else "replicas x%d") % world,
                            "l2": "no flush: one step streams %.1f GB, far beyond the 126 MB L2" % (alg_pruned / 1e9)},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "out_of_core": ooc,
@@ -572,6 +576,8 @@ def main():
                          "all-to-alls per step) instead of N replicas; with N = 1 it measures the pack / unpack overhead")
     ap.add_argument("--packed-exchange", action="store_true",
                     help="--decompose: pack -> NCCL all_to_all_single -> unpack instead of direct peer stores")
+    ap.add_argument("--integrator", default="ab2", choices=["ab2", "rk4", "pc"],
+                    help="time integrator (PAPER.md L25, Table I): Adams-Bashforth 2 (the metric's), RK4, predictor-corrector")
     ap.add_argument("--tracers", type=int, default=0, metavar="NP",
                     help="also measure NP tracer particles (PAPER.md Sec. VI): frozen-field pushes/s and the step overhead")
     ap.add_argument("--option", action="append", default=[], metavar="ID=VALUE",

@@ -151,12 +151,21 @@ struct SpecGeom {
 };
 // J^ = M i k x B^
 void launch_build_current(const SpecGeom& g, const cd* const B[3], cd* const J[3], Phys ph, cudaStream_t st);
+// One stage of a multi-stage integrator in low-storage form (mode 3; RK4 and the predictor-corrector, Table I
+// L39): with the stage slope R just assembled,  first: U0 <- U;  acc <- acc + b_acc R (first: b_acc R);  U <- U0 + c_next R;
+// last stage instead: U <- U0 + acc + b_acc R.  One pass over the modes per stage, no separate linear-combination kernels.
+struct StageUpdate {
+    cd* U0[8];
+    cd* acc[8];
+    double c_next, b_acc;
+    int first, last;
+};
 // R^ from the 16 transformed product fields and the state; mode 0: write R^ to rout only;
-// mode 1: Euler update U += dt R, Rold = R; mode 2: AB2 update U += dt(1.5 R - 0.5 Rold), Rold = R
+// mode 1: Euler update U += dt R, Rold = R; mode 2: AB2 update U += dt(1.5 R - 0.5 Rold), Rold = R; mode 3: `stage`
 // force (or null): 4 arrays F^_x, F^_y, F^_z, (m.f)^ added to R_m and R_E (launch_forcing below)
 void launch_assemble(const SpecGeom& g, const cd* const prod[16], cd* const U[8], cd* const Rold[8],
                      cd* const rout[8], int mode, double dt, Phys ph, cudaStream_t st, const cd* const force[4] = nullptr,
-                     const cd* const visc[9] = nullptr);   // visc: V^xx,xy,xz,yy,yz,zz, Wv^x,y,z: R_m += i k_j V^_ij, R_E += i k.Wv^
+                     const cd* const visc[9] = nullptr, const StageUpdate* stage = nullptr);   // visc: V^xx,xy,xz,yy,yz,zz, Wv^x,y,z: R_m += i k_j V^_ij, R_E += i k.Wv^
 // full stress tensor variant (Eq. 3-4, 11-12): u = m/rho in real space; S^ (xx,xy,xz,yy,yz,zz) from u^;
 // V_ij = 2 nu rho S_ij (in place over S) and Wv_j = u_i V_ij in real space
 void launch_velocity_real(long long n, const double* rho, const double* const m[3], double* const u[3], cudaStream_t st);

@@ -115,7 +115,7 @@ struct PtrC9 { const cd* p[9]; };
 // its register budget; VAR = true: all variants of DESIGN.md section 13
 template <bool VAR>
 __global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 rout, int mode, double dt, Phys ph, PtrC4 force,
-                                PtrC9 visc) {
+                                PtrC9 visc, StageUpdate sg) {
     ModeIt m;
     if (!mode_of_thread(g, m)) return;
     const long long i = m.idx, j = m.sidx;     // products / state
@@ -145,6 +145,19 @@ __global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 r
         if (mode == 0) {
 #pragma unroll
             for (int f = 0; f < 8; ++f) rout.p[f][i] = R[f];     // work-array geometry (may alias the products)
+        } else if (mode == 3) {      // one stage of RK4 / predictor-corrector, low-storage form (kernels.h StageUpdate)
+#pragma unroll
+            for (int f = 0; f < 8; ++f) {
+                const cd u0 = sg.first ? u[f] : sg.U0[f][j];
+                const cd a = sg.first ? mk(0, 0) : sg.acc[f][j];
+                if (sg.first) sg.U0[f][j] = u[f];
+                const cd an = mk(a.x + sg.b_acc * R[f].x, a.y + sg.b_acc * R[f].y);
+                if (sg.last) U.p[f][j] = mk(u0.x + an.x, u0.y + an.y);
+                else {
+                    sg.acc[f][j] = an;
+                    U.p[f][j] = mk(u0.x + sg.c_next * R[f].x, u0.y + sg.c_next * R[f].y);
+                }
+            }
         } else {
 #pragma unroll
             for (int f = 0; f < 8; ++f) {
@@ -160,15 +173,17 @@ __global__ void assemble_kernel(SpecGeom g, PtrC16 pr, Ptr8 U, Ptr8 Rold, Ptr8 r
 }
 void launch_assemble(const SpecGeom& g, const cd* const prod[16], cd* const U[8], cd* const Rold[8],
                      cd* const rout[8], int mode, double dt, Phys ph, cudaStream_t st, const cd* const force[4],
-                     const cd* const visc[9]) {
+                     const cd* const visc[9], const StageUpdate* stage) {
     PtrC16 p; Ptr8 u, ro, rr; PtrC4 fc; PtrC9 vc;
     for (int f = 0; f < 9; ++f) vc.p[f] = visc ? visc[f] : nullptr;
     for (int f = 0; f < 4; ++f) fc.p[f] = force ? force[f] : nullptr;
     for (int f = 0; f < 16; ++f) p.p[f] = prod[f];
     for (int f = 0; f < 8; ++f) { u.p[f] = U[f]; ro.p[f] = Rold ? Rold[f] : nullptr; rr.p[f] = rout ? rout[f] : nullptr; }
     const bool var = force || visc || ph.cs2 > 0.0 || ph.evolve != 3;
-    if (var) assemble_kernel<true><<<mode_grid(g, kt_for(g)), kt_for(g), 0, st>>>(g, p, u, ro, rr, mode, dt, ph, fc, vc);
-    else assemble_kernel<false><<<mode_grid(g, kt_for(g)), kt_for(g), 0, st>>>(g, p, u, ro, rr, mode, dt, ph, fc, vc);
+    StageUpdate sg = StageUpdate();
+    if (stage) sg = *stage;
+    if (var) assemble_kernel<true><<<mode_grid(g, kt_for(g)), kt_for(g), 0, st>>>(g, p, u, ro, rr, mode, dt, ph, fc, vc, sg);
+    else assemble_kernel<false><<<mode_grid(g, kt_for(g)), kt_for(g), 0, st>>>(g, p, u, ro, rr, mode, dt, ph, fc, vc, sg);
 }
 
 // ---- full stress tensor variant (Eq. 3-4, 11-12) -------------------------------------------------------

@@ -235,14 +235,15 @@ void viscous_pass(mhd_ctx* c, cd* const Uin[8]) {
 }
 
 // R^(Uin) -> rout (mode 0) or explicit update of Uin / Rold (mode 1 Euler, 2 AB2)
-void rhs_spectral(mhd_ctx* c, cd* const Uin[8], cd* const rout[8], int mode, double* const breal[3] = nullptr) {
+void rhs_spectral(mhd_ctx* c, cd* const Uin[8], cd* const rout[8], int mode, double* const breal[3] = nullptr,
+                  const StageUpdate* stage = nullptr) {
     const bool stress = c->opt_stress != 0;
     const cd* visc[9] = {c->Y[0], c->Y[1], c->Y[2], c->Y[3], c->Y[4], c->Y[5], c->Y[6], c->Y[7], c->X[7]};
     if (stress) viscous_pass(c, Uin);                 // V^_ij, Wv^_j -> Y[0..7], X[7]   (before the products: uses X, Y)
     const bool forced = c->f0 != 0.0;
     // default equation set on the pruned, fused path: sweep S5 is one launch
     const bool one_s5 = c->opt_fuse_assemble != 0 && c->opt_fused != 0 && c->opt_prune != 0 && !stress && !forced &&
-                        c->cs2 <= 0.0 && c->evolve == 3 && strided_assemble_supported(c->N);
+                        c->cs2 <= 0.0 && c->evolve == 3 && mode != 3 && strided_assemble_supported(c->N);
     products(c, Uin, breal, !one_s5);
     if (one_s5) { fused_s5(c, Uin, rout, mode); return; }
     SpecGeom gp = c->geom(); gp.pruned = 1;
@@ -259,7 +260,7 @@ void rhs_spectral(mhd_ctx* c, cd* const Uin[8], cd* const rout[8], int mode, dou
         if (stress) ph.mu = 0.0;                      // the viscous terms come from `visc`, not from mu k^2 u^
         mhd_ctx::Scope s(c, F_ASSEMBLE);
         launch_assemble(c->geom(), c->W, Uin, c->Rold, rout, mode, c->dt, ph, c->st, (forced && mode != 0) ? force : nullptr,
-                        stress ? visc : nullptr);
+                        stress ? visc : nullptr, stage);
     }
     if (forced && mode == 0) {      // U^ is not modified: add F^ to the assembled R^ (X, Y may hold integrator stages)
         mhd_ctx::Scope s(c, F_POINT);
@@ -534,37 +535,23 @@ int mhd_step(mhd_ctx* c, int nsteps) {
             rhs_spectral(c, c->U, nullptr, c->have_old ? 2 : 1, emit ? Breal : nullptr);
             if (emit) tracers_push_with(c, Breal, 1);
             c->have_old = true;
-        } else if (c->integrator == 1) {                // classical RK4
-            // U0 = Rold, acc = Y, k = X, stage state in U
-            const cd* Uc[8]; const cd* Xc[8]; const cd* U0c[8]; const cd* Yc[8];
-            for (int f = 0; f < 8; ++f) { Uc[f] = c->U[f]; Xc[f] = c->X[f]; U0c[f] = c->Rold[f]; Yc[f] = c->Y[f]; }
+        } else {
+            // RK4 and the predictor-corrector (Heun: U* = U + dt R(U); U+ = U + dt/2 (R(U) + R(U*))) in low-storage
+            // form: each stage's assembly pass also accumulates the slope and forms the next stage state (StageUpdate);
+            // U0 lives in the R^old buffers, the accumulator in Y
             const double dt = c->dt;
-            auto ax = [&](double a, cd* const y[], double b, const cd* const x[]) { mhd_ctx::Scope sc(c, F_AXPBY); launch_axpby(gp, 8, a, y, b, x, c->st); };
-            ax(0.0, c->Rold, 1.0, Uc);                  // U0 = U
-            rhs_spectral(c, c->U, c->X, 0);             // k1
-            ax(0.0, c->Y, dt / 6.0, Xc);                // acc = dt/6 k1
-            ax(0.0, c->U, 1.0, U0c); ax(1.0, c->U, 0.5 * dt, Xc);
-            rhs_spectral(c, c->U, c->X, 0);             // k2
-            ax(1.0, c->Y, dt / 3.0, Xc);
-            ax(0.0, c->U, 1.0, U0c); ax(1.0, c->U, 0.5 * dt, Xc);
-            rhs_spectral(c, c->U, c->X, 0);             // k3
-            ax(1.0, c->Y, dt / 3.0, Xc);
-            ax(0.0, c->U, 1.0, U0c); ax(1.0, c->U, dt, Xc);
-            rhs_spectral(c, c->U, c->X, 0);             // k4
-            ax(1.0, c->Y, dt / 6.0, Xc);
-            ax(0.0, c->U, 1.0, U0c); ax(1.0, c->U, 1.0, Yc);
-        } else {                                        // predictor-corrector (Heun): U* = U + dt R(U); U+ = U + dt/2 (R(U) + R(U*))
-            const cd* Uc[8]; const cd* Xc[8]; const cd* U0c[8]; const cd* Yc[8];
-            for (int f = 0; f < 8; ++f) { Uc[f] = c->U[f]; Xc[f] = c->X[f]; U0c[f] = c->Rold[f]; Yc[f] = c->Y[f]; }
-            const double dt = c->dt;
-            auto ax = [&](double a, cd* const y[], double b, const cd* const x[]) { mhd_ctx::Scope sc(c, F_AXPBY); launch_axpby(gp, 8, a, y, b, x, c->st); };
-            ax(0.0, c->Rold, 1.0, Uc);                  // U0 = U
-            rhs_spectral(c, c->U, c->X, 0);             // R(U)
-            ax(0.0, c->Y, 0.5 * dt, Xc);
-            ax(1.0, c->U, dt, Xc);                      // predictor
-            rhs_spectral(c, c->U, c->X, 0);             // R(U*)
-            ax(1.0, c->Y, 0.5 * dt, Xc);
-            ax(0.0, c->U, 1.0, U0c); ax(1.0, c->U, 1.0, Yc);
+            const double rk4[4][2] = {{0.5 * dt, dt / 6.0}, {0.5 * dt, dt / 3.0}, {dt, dt / 3.0}, {0.0, dt / 6.0}};
+            const double heun[2][2] = {{dt, 0.5 * dt}, {0.0, 0.5 * dt}};
+            const int ns = c->integrator == 1 ? 4 : 2;
+            for (int k = 0; k < ns; ++k) {
+                StageUpdate sg;
+                std::memset(&sg, 0, sizeof(sg));
+                for (int f = 0; f < 8; ++f) { sg.U0[f] = c->Rold[f]; sg.acc[f] = c->Y[f]; }
+                sg.c_next = c->integrator == 1 ? rk4[k][0] : heun[k][0];
+                sg.b_acc = c->integrator == 1 ? rk4[k][1] : heun[k][1];
+                sg.first = k == 0; sg.last = k == ns - 1;
+                rhs_spectral(c, c->U, nullptr, 3, nullptr, &sg);
+            }
         }
         ++c->step;
     }
