@@ -56,6 +56,9 @@ extern "C" {
  * staging buffers on side streams.  Placement flags need MHD_FLAG_OUT_OF_CORE.           */
 #define MHD_FLAG_OUT_OF_CORE 1u   /* chunked pipeline on compact storage; with no placement flag everything stays in HBM */
 #define MHD_FLAG_STATE_ON_HOST 2u /* U^ and the Adams-Bashforth history live in pinned host memory                      */
+#define MHD_FLAG_STAGE_STORAGE 8u /* chunked pipeline: also allocate the 8 compact accumulator arrays that the multi-stage
+                                     integrators (MHD_OPT_INTEGRATOR = 1 RK4, 2 predictor-corrector) need beside U^ and the
+                                     R^old arrays (which then hold the state at the start of the step): +50 % state storage  */
 #define MHD_FLAG_WORK_ON_HOST 4u  /* the 16 work fields between the z and y passes live in pinned host memory           */
 #define MHD_FLAG_RANKS(g) ((unsigned)((g) - 1) << 4) /* slab decomposition over g = 1..8 GPUs with PER-RANK storage: the context
                                      allocates only one rank's share (1/g of the state, 2/g of the work arrays: a brick-shaped

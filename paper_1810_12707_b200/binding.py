@@ -23,6 +23,7 @@ MHD_OPT_FUSED, MHD_OPT_PRUNE, MHD_OPT_INTEGRATOR, MHD_OPT_FUSE_CURRENT, MHD_OPT_
 MHD_OPT_FUSE_ASSEMBLE = 7
 MHD_OPT_TMA = 13
 MHD_FLAG_OUT_OF_CORE, MHD_FLAG_STATE_ON_HOST, MHD_FLAG_WORK_ON_HOST = 1, 2, 4
+MHD_FLAG_STAGE_STORAGE = 8
 
 
 def MHD_FLAG_BUDGET_MIB(m):

@@ -74,6 +74,8 @@ struct mhd_ctx {
         bool on = false, state_host = false, work_host = false;
         int nzc = 0, nyc = 0, nxp = 0;           // compact extents: 2kc+1, 2kc+1, kc+1 rounded up to 8
         cd *Uc[8], *Rc[8];                       // compact state / history [nzc][nyc][nxp]
+        cd* Ac[8] = {};                          // MHD_FLAG_STAGE_STORAGE: accumulator of the multi-stage integrators
+        bool stage_storage = false;
         // work arrays between the z and y passes.  Unified layout (one context holds everything): WzB = WzS = [N][nyc][nxp].
         // Per-rank layout (MHD_FLAG_RANKS, `split`): WzB = [N][ny_max][nxp] holds all z of the rank's ky share (stages A, C),
         // WzS = [nz_max][nyc][nxp] all ky of its z share (stage B); the state arrays are [nzc][ny_max][nxp]

@@ -345,7 +345,7 @@ int mhd_init(mhd_ctx** out, int N, double L, double gamma, double mu, double eta
 }
 
 static bool flags_valid(unsigned flags) {
-    if ((flags & 0x88u) != 0) return false;                                 // unknown bits
+    if ((flags & 0x80u) != 0) return false;                                 // unknown bits
     if ((flags & 0x70u) && (flags & (MHD_FLAG_STATE_ON_HOST | MHD_FLAG_WORK_ON_HOST))) return false;   // per-rank storage lives in HBM
     if (!(flags & MHD_FLAG_OUT_OF_CORE)) return flags == 0;                 // placement / budget need the chunked pipeline
     return true;

@@ -34,6 +34,7 @@ struct OocSizes {
     size_t tw_off, ftw_off, state_off, work_off, stage_off, stage_total, part_off, part_bytes, res_off, total;
     size_t per_ky, per_z;         // staging bytes per ky column of a brick / per z plane of a slab
     bool state_host, work_host;
+    int nstate;                   // compact state-shaped arrays: U^ 8 + R^old 8 (+ 8 accumulators with MHD_FLAG_STAGE_STORAGE)
     size_t pinned_total;
 };
 
@@ -48,6 +49,7 @@ bool ooc_sizes(int N, unsigned flags, OocSizes& s) {
     s.kc = N / 3; s.nzc = 2 * s.kc + 1; s.nyc = s.nzc; s.nxp = (s.kc + 1 + 7) / 8 * 8; s.hx = N / 2;
     s.state_host = (flags & MHD_FLAG_STATE_ON_HOST) != 0;
     s.work_host = (flags & MHD_FLAG_WORK_ON_HOST) != 0;
+    s.nstate = (flags & MHD_FLAG_STAGE_STORAGE) ? 24 : 16;
     s.ranks = (int)((flags >> 4) & 7u) + 1;
     if (s.ranks > 1 && (s.state_host || s.work_host || s.ranks > s.nyc || s.ranks > N)) return false;
     s.ny_max = (s.nyc + s.ranks - 1) / s.ranks; s.nz_max = (N + s.ranks - 1) / s.ranks;
@@ -58,7 +60,7 @@ bool ooc_sizes(int N, unsigned flags, OocSizes& s) {
     size_t off = 0;
     s.tw_off = off; off += align_up((size_t)N * sizeof(cd));
     s.ftw_off = off; off += align_up((size_t)(4 * N + 64) * sizeof(cd));
-    s.state_off = off; if (!s.state_host) off += 16 * s.cbytes;
+    s.state_off = off; if (!s.state_host) off += (size_t)s.nstate * s.cbytes;
     s.work_off = off; if (!s.work_host) off += 16 * s.wbytes;
     s.slab_off = off; off += 16 * s.sbytes;
     s.part_bytes = align_up((size_t)(diag_partial_doubles() + absmax_partial_doubles() + spectrum_partial_doubles(ns)) * sizeof(double));
@@ -68,7 +70,7 @@ bool ooc_sizes(int N, unsigned flags, OocSizes& s) {
     // 9 compact columns of scratch (R^ of mhd_rhs / the divergence of mhd_diagnostics); per z plane of a slab: the
     // 16 full-pitch planes of the x sweep plus the compact in (11) and out (16) planes when the work lives on the host
     const size_t col = (size_t)s.nxp * sizeof(cd);
-    s.per_ky = ((s.work_host ? 16 * (size_t)N : 0) + (s.state_host ? 16 * (size_t)s.nzc : 0) + 9 * (size_t)s.nzc) * col + 64 * 256;
+    s.per_ky = ((s.work_host ? 16 * (size_t)N : 0) + (s.state_host ? (size_t)s.nstate * s.nzc : 0) + 9 * (size_t)s.nzc) * col + 64 * 256;
     s.per_z = 16 * (size_t)N * s.hx * sizeof(cd) + (s.work_host ? 27 * (size_t)s.nyc * col : 0) + 64 * 256;
     const size_t min_set = std::max(s.per_ky, s.per_z);
     const size_t want_set = std::max(s.per_ky * (size_t)std::min(s.kc + 1, 16), s.per_z * (size_t)std::min(N, 8));
@@ -80,7 +82,7 @@ bool ooc_sizes(int N, unsigned flags, OocSizes& s) {
     }
     s.stage_off = off; s.stage_total = NBUF * align_up(set); off += s.stage_total;
     s.total = off;
-    s.pinned_total = (s.state_host ? 16 * s.cbytes : 0) + (s.work_host ? 16 * s.wbytes : 0);
+    s.pinned_total = (s.state_host ? (size_t)s.nstate * s.cbytes : 0) + (s.work_host ? 16 * s.wbytes : 0);
     return true;
 }
 
@@ -399,7 +401,7 @@ int stage_slabs(mhd_ctx* c, SlabKind kind, const SlabIO& io) {
 //      mode 0 (mhd_rhs): R^ replaces the first 8 work fields and is inverse-z-transformed on the spot.
 //      next_inverse (modes 1, 2): stage A of the NEXT step runs on the freshly updated brick while it is still on the
 //      device (the z pass is local to a brick), which saves one host->device pass over U^ per step ----------------------
-int stage_forward_z_assemble(mhd_ctx* c, int mode, bool next_inverse) {
+int stage_forward_z_assemble(mhd_ctx* c, int mode, bool next_inverse, const StageUpdate* sg = nullptr) {
     Ooc& o = c->ooc;
     stage_begin(c);
     const auto chunks = brick_chunks(c);
@@ -409,15 +411,22 @@ int stage_forward_z_assemble(mhd_ctx* c, int mode, bool next_inverse) {
         Chunk ch = chunk_begin(c, (int)i, h2d);
         View w = work_view(c, ch, 16, y0, ny, true);
         View u = state_view(c, ch, o.Uc, 8, y0, ny, true);
-        View r;
-        if (mode != 0) r = state_view(c, ch, o.Rc, 8, y0, ny, mode == 2);
+        View r, acc;
+        if (mode != 0) r = state_view(c, ch, o.Rc, 8, y0, ny, mode == 2 || (mode == 3 && !sg->first));
+        if (mode == 3) acc = state_view(c, ch, o.Ac, 8, y0, ny, !sg->first);      // (the last stage only reads it)
         if (ch.overflow) return overflow(c);
         if (h2d) chunk_h2d_done(c, ch);
         gen_pass(c, -1, 16, w.p, w.p, w.rs, o.nxp, 0, w.rs, o.nxp, 2, ny);          // in place: rows compacted
         const SpecGeom g = brick_geom(c, y0, ny, w.rs, u.rs);
         {
             mhd_ctx::Scope s(c, F_ASSEMBLE);
-            launch_assemble(g, w.p, u.p, mode != 0 ? r.p : nullptr, mode == 0 ? w.p : nullptr, mode, c->dt, c->phys(), c->st);
+            StageUpdate st3 = StageUpdate();
+            if (mode == 3) {        // multi-stage integrators: U0 in the R^old arrays, accumulator in Ac (brick views)
+                st3 = *sg;
+                for (int f = 0; f < 8; ++f) { st3.U0[f] = r.p[f]; st3.acc[f] = acc.p[f]; }
+            }
+            launch_assemble(g, w.p, u.p, mode != 0 ? r.p : nullptr, mode == 0 ? w.p : nullptr, mode, c->dt, c->phys(), c->st, nullptr,
+                            nullptr, mode == 3 ? &st3 : nullptr);
         }
         if (mode == 0) gen_pass(c, +1, 8, w.p, w.p, w.rs, o.nxp, 2, w.rs, o.nxp, 0, ny);
         if (mode != 0 && next_inverse) {
@@ -431,7 +440,9 @@ int stage_forward_z_assemble(mhd_ctx* c, int mode, bool next_inverse) {
         if (d2h) {
             if (mode == 0) work_store(c, w, 8, y0);
             else {
-                state_store(c, u, o.Uc, 8, y0); state_store(c, r, o.Rc, 8, y0);
+                state_store(c, u, o.Uc, 8, y0);
+                if (mode != 3 || sg->first) state_store(c, r, o.Rc, 8, y0);
+                if (mode == 3 && !sg->last) state_store(c, acc, o.Ac, 8, y0);
                 if (next_inverse) work_store(c, w, 11, y0);
             }
             chunk_d2h_done(c, ch);
@@ -523,8 +534,9 @@ int ooc_bind(mhd_ctx* c, char* base, size_t bytes, char* pinned, size_t pinned_b
     c->tw = reinterpret_cast<cd*>(base + s.tw_off);
     c->ftw = reinterpret_cast<cd*>(base + s.ftw_off);
     char* hp = pinned;
-    for (int f = 0; f < 16; ++f) {
-        cd*& dst = f < 8 ? o.Uc[f] : o.Rc[f - 8];
+    o.stage_storage = s.nstate > 16;
+    for (int f = 0; f < s.nstate; ++f) {
+        cd*& dst = f < 8 ? o.Uc[f] : (f < 16 ? o.Rc[f - 8] : o.Ac[f - 16]);
         if (s.state_host) { dst = reinterpret_cast<cd*>(hp); hp += s.cbytes; }
         else dst = reinterpret_cast<cd*>(base + s.state_off + (size_t)f * s.cbytes);
     }
@@ -632,14 +644,36 @@ int ooc_rhs(mhd_ctx* c, int where, double* const out[8]) {
 
 int ooc_step(mhd_ctx* c, int nsteps) {
     if (c->ooc.world > 1) return c->fail(MHD_ERR_INVALID_ARG, "decomposed context: drive the step with mhd_dist_phase and the exchanges");
-    if (c->integrator != 0) return c->fail(MHD_ERR_INVALID_ARG, "the chunked pipeline implements Adams-Bashforth only");
+    if (c->integrator != 0 && !c->ooc.stage_storage)
+        return c->fail(MHD_ERR_INVALID_ARG, "RK4 / predictor-corrector on the chunked pipeline need MHD_FLAG_STAGE_STORAGE at mhd_bind");
     if (int vrc = ooc_variant_check(c)) return vrc;
+    bool have_inverse_z = false;        // stage A of the next right-hand side already ran on the bricks of the last stage C
     for (int s = 0; s < nsteps; ++s) {
-        int rc = ooc_products(c, s > 0);
-        if (rc) return rc;
-        rc = stage_forward_z_assemble(c, c->have_old ? 2 : 1, s + 1 < nsteps);
-        if (rc) return rc;
-        c->have_old = true;
+        if (c->integrator == 0) {
+            int rc = ooc_products(c, have_inverse_z);
+            if (rc) return rc;
+            have_inverse_z = s + 1 < nsteps;
+            rc = stage_forward_z_assemble(c, c->have_old ? 2 : 1, have_inverse_z);
+            if (rc) return rc;
+            c->have_old = true;
+        } else {                        // RK4 / predictor-corrector, low-storage stages (kernels.h StageUpdate; mhd_api.cu mhd_step)
+            const double dt = c->dt;
+            const double rk4[4][2] = {{0.5 * dt, dt / 6.0}, {0.5 * dt, dt / 3.0}, {dt, dt / 3.0}, {0.0, dt / 6.0}};
+            const double heun[2][2] = {{dt, 0.5 * dt}, {0.0, 0.5 * dt}};
+            const int ns = c->integrator == 1 ? 4 : 2;
+            for (int k = 0; k < ns; ++k) {
+                StageUpdate sg = StageUpdate();
+                sg.c_next = c->integrator == 1 ? rk4[k][0] : heun[k][0];
+                sg.b_acc = c->integrator == 1 ? rk4[k][1] : heun[k][1];
+                sg.first = k == 0; sg.last = k == ns - 1;
+                int rc = ooc_products(c, have_inverse_z);
+                if (rc) return rc;
+                have_inverse_z = !(sg.last && s + 1 == nsteps);
+                rc = stage_forward_z_assemble(c, 3, have_inverse_z, &sg);
+                if (rc) return rc;
+            }
+            c->have_old = false;        // the R^old arrays now hold U0, not a slope
+        }
         ++c->step;
     }
     return check_cuda(c, "step (chunked)");

@@ -772,6 +772,33 @@ def test_chunked_pipeline_matches_in_core(orc, MHD, flags, N, brick, slab):
     assert dg["step"] == 4 and abs(dg["max_divb"] - dr["max_divb"]) <= 1e-12 + 1e-6 * dr["max_divb"]
 
 
+@pytest.mark.parametrize("integ", [1, 2])
+@pytest.mark.parametrize("flags,N,brick,slab", [(0, 64, 0, 0), (6, 32, 4, 5), (2, 64, 7, 9)])
+def test_chunked_pipeline_rk4_and_predictor_corrector(MHD, integ, flags, N, brick, slab):
+    """RK4 and the predictor-corrector (Table I) on the chunked pipeline (MHD_FLAG_STAGE_STORAGE reserves the
+    accumulator arrays): same low-storage stages as in core, so the states agree to roundoff, in HBM and with the state /
+    work arrays streamed from pinned host memory; without the flag the call is refused."""
+    from paper_1810_12707_b200 import binding as b
+    cfg = inputs.Config("random", N, 2 * math.pi, 5 / 3, 0.01, 0.02, 1e-3, 1, inputs.random_smooth_state(N, 23, kmax=4))
+    ref, g = _ooc_pair(MHD, cfg, flags | b.MHD_FLAG_STAGE_STORAGE, brick, slab)
+    ref.set_option(b.MHD_OPT_INTEGRATOR, integ)
+    g.set_option(b.MHD_OPT_INTEGRATOR, integ)
+    g.step(1); g.step(2)
+    ref.step(3)
+    for a, r in zip(g.get_fields(), ref.get_fields()):
+        assert rel_l2(a, r) <= 1e-13
+    assert g.diagnostics()["step"] == 3
+    # back to Adams-Bashforth on the same context: Euler restart (the R^old arrays held U0)
+    g.set_option(b.MHD_OPT_INTEGRATOR, 0); ref.set_option(b.MHD_OPT_INTEGRATOR, 0)
+    g.step(2); ref.step(2)
+    for a, r in zip(g.get_fields(), ref.get_fields()):
+        assert rel_l2(a, r) <= 1e-13
+    _, plain = _ooc_pair(MHD, cfg, flags, brick, slab)
+    plain.set_option(b.MHD_OPT_INTEGRATOR, integ)
+    with pytest.raises(RuntimeError, match="MHD_FLAG_STAGE_STORAGE"):
+        plain.step(1)
+
+
 def test_chunked_pipeline_device_pointers_and_spectrum(MHD):
     import torch
     from paper_1810_12707_b200 import binding as b
