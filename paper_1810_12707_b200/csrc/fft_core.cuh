@@ -78,23 +78,24 @@ template <int R, int K, int DIR> __device__ __forceinline__ cd mul_rootN(cd a) {
 // ---------------------------------------------------------------------------------------------------
 __device__ __forceinline__ cd mirror2(cd e, cd v) { return mk(fma(2.0, e.x, -v.x), fma(2.0, e.y, -v.y)); }
 
-// constant root W = exp(DIR * 2*pi*i * K/R), 0 <= K < R/2, R in {2,4,8,16}
+// constant root W = exp(DIR * 2*pi*i * K/R), 0 <= K < R/2, R in {2,4,8,16,32}
 template <int R, int K, int DIR> __device__ __forceinline__ void bfly_root(cd e, cd o, cd& v, cd& vm) {
-    constexpr int K16 = K * (16 / R);
+    constexpr int K32 = K * (32 / R);
     constexpr double SQH = 0.70710678118654752440;   // sqrt(1/2)
-    constexpr double C8 = 0.92387953251128675613;    // cos(pi/8)
-    constexpr double S8 = 0.38268343236508977173;    // sin(pi/8)
-    if constexpr (K16 == 0) { v = e + o; vm = e - o; }
-    else if constexpr (K16 == 4) { const cd t = mul_mi<DIR>(o); v = e + t; vm = e - t; }
-    else if constexpr (K16 == 2) {          // W = SQH (1 + sg i):  W o = SQH (o.x - sg o.y, o.y + sg o.x)
+    // cos / sin (pi m / 16), m = 0..8
+    constexpr double CS[9] = {1.0, 0.98078528040323044913, 0.92387953251128675613, 0.83146961230254523708, SQH,
+                              0.55557023301960222474, 0.38268343236508977173, 0.19509032201612826785, 0.0};
+    if constexpr (K32 == 0) { v = e + o; vm = e - o; }
+    else if constexpr (K32 == 8) { const cd t = mul_mi<DIR>(o); v = e + t; vm = e - t; }
+    else if constexpr (K32 == 4) {          // W = SQH (1 + sg i):  W o = SQH (o.x - sg o.y, o.y + sg o.x)
         const double dx = (DIR < 0) ? o.x + o.y : o.x - o.y, dy = (DIR < 0) ? o.y - o.x : o.y + o.x;
         v = mk(fma(SQH, dx, e.x), fma(SQH, dy, e.y)); vm = mk(fma(-SQH, dx, e.x), fma(-SQH, dy, e.y));
-    } else if constexpr (K16 == 6) {        // W = SQH (-1 + sg i): W o = SQH (-(o.x + sg o.y), sg o.x - o.y)
+    } else if constexpr (K32 == 12) {       // W = SQH (-1 + sg i): W o = SQH (-(o.x + sg o.y), sg o.x - o.y)
         const double dx = (DIR < 0) ? o.x - o.y : o.x + o.y, dy = (DIR < 0) ? -o.x - o.y : o.x - o.y;
         v = mk(fma(-SQH, dx, e.x), fma(SQH, dy, e.y)); vm = mk(fma(SQH, dx, e.x), fma(-SQH, dy, e.y));
-    } else {
-        constexpr double wr = (K16 == 1) ? C8 : (K16 == 3) ? S8 : (K16 == 5) ? -S8 : -C8;
-        constexpr double wi = ((DIR < 0) ? -1.0 : 1.0) * ((K16 == 1 || K16 == 7) ? S8 : C8);
+    } else {                                // angle 2 pi K32 / 32 = pi K32 / 16 in (0, pi)
+        constexpr double wr = (K32 < 8) ? CS[K32] : -CS[16 - K32];
+        constexpr double wi = ((DIR < 0) ? -1.0 : 1.0) * ((K32 < 8) ? CS[8 - K32] : CS[K32 - 8]);
         v = mk(fma(-o.y, wi, fma(o.x, wr, e.x)), fma(o.y, wr, fma(o.x, wi, e.y)));
         vm = mirror2(e, v);
     }

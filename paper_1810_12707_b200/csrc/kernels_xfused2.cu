@@ -1,4 +1,4 @@
-// kernels_xfused2.cu — sweep S3, second generation: the fused real-axis kernel for N = 128, 256, 512.
+// kernels_xfused2.cu — sweep S3, second generation: the fused real-axis kernel for N = 128, 256, 512, 1024.
 //
 // Per (y,z) line: C2R of 11 half-spectrum lines, 16 flux products, R2C of the 16 products.  Compared with the
 // generic tile version (kernels_x.cu) this kernel
@@ -24,6 +24,7 @@ template <int H> struct FPlan;
 template <> struct FPlan<64>  { static constexpr int R0 = 8,  R1 = 8;  };
 template <> struct FPlan<128> { static constexpr int R0 = 8,  R1 = 16; };
 template <> struct FPlan<256> { static constexpr int R0 = 16, R1 = 16; };
+template <> struct FPlan<512> { static constexpr int R0 = 16, R1 = 32; };   // N = 1024: 128 KB tile, one CTA per SM
 
 template <int H> struct F2 {
     static constexpr int R0 = FPlan<H>::R0, R1 = FPlan<H>::R1;
@@ -108,7 +109,7 @@ __device__ __forceinline__ void r2c_pair(cd& Zk, cd& Zm, cd w) {
 }
 
 template <int N>
-__global__ void __launch_bounds__(F2<N / 2>::THREADS, (N / 2 == 256) ? 3 : 4)
+__global__ void __launch_bounds__(F2<N / 2>::THREADS, (N / 2 == 512) ? 1 : (N / 2 == 256) ? 3 : 4)
 x_fused2_kernel(const __grid_constant__ FusedXArgs a) {
     constexpr int H = N / 2;
     typedef F2<H> P;
@@ -271,13 +272,14 @@ template <int N> static void fused2_one(const FusedXArgs& a, cudaStream_t st) {
     x_fused2_kernel<N><<<(unsigned)a.nlines, P::THREADS, P::SMEM, st>>>(a);
 }
 
-bool x_fused2_supported(int N) { return N == 128 || N == 256 || N == 512; }
+bool x_fused2_supported(int N) { return N == 128 || N == 256 || N == 512 || N == 1024; }
 
 int x_fused2_table_entries(int N) {
     switch (N) {
         case 128: return FTab<64>::SIZE;
         case 256: return FTab<128>::SIZE;
         case 512: return FTab<256>::SIZE;
+        case 1024: return FTab<512>::SIZE;
         default: return 0;
     }
 }
@@ -289,6 +291,7 @@ void launch_x_fused2_tables(int N, cd* tab, cudaStream_t st) {
         case 128: fused_twiddle_kernel<64><<<blocks, 128, 0, st>>>(tab); break;
         case 256: fused_twiddle_kernel<128><<<blocks, 128, 0, st>>>(tab); break;
         case 512: fused_twiddle_kernel<256><<<blocks, 128, 0, st>>>(tab); break;
+        case 1024: fused_twiddle_kernel<512><<<blocks, 128, 0, st>>>(tab); break;
         default: break;
     }
 }
@@ -298,6 +301,7 @@ void launch_x_fused2(int N, const FusedXArgs& a, cudaStream_t st) {
         case 128: fused2_one<128>(a, st); break;
         case 256: fused2_one<256>(a, st); break;
         case 512: fused2_one<512>(a, st); break;
+        case 1024: fused2_one<1024>(a, st); break;
         default: break;
     }
 }
