@@ -157,12 +157,12 @@ def test_partition_is_balanced_and_counts_match():
 
 def test_algorithmic_bytes_match_the_measured_dram_traffic():
     """bench.sweep_bytes (the algorithmic bytes behind every roofline fraction) against the DRAM bytes per launch that
-    ncu measured (profiles/traffic_r01.json, from the committed captures): equal to within 4 %, i.e. no
+    ncu measured (profiles/traffic_r02.json, from the committed captures): equal to within 4 %, i.e. no
     kernel re-reads what it should stream once, and the accounting does not flatter the fractions."""
     import json
     sys.path.insert(0, ROOT)
     import bench
-    traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic_r01.json")))
+    traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic_r02.json")))
     for N in (256, 512):
         sb = bench.sweep_bytes(N, prune=True)
         launches = {"strided_inverse": 2, "strided_forward": 2, "x_fused": 1, "assemble": 1}
