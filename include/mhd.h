@@ -84,11 +84,11 @@ extern "C" {
                                 two-launch result; measured slower on B200, so the default is
                                 0: forward z pass and assembly as two launches                                 */
 
-#define MHD_OPT_TMA 13 /* the in-core y / z passes (all but the pass that builds J^ on load) as a persistent pipeline fed by the
-                          tensor-memory accelerator (cp.async.bulk.tensor into a ring of shared-memory tiles, mbarrier
-                          completion): 1 (default): at N = 512, where it measured at least as fast; 2: wherever it exists
-                          (N = 128, 256, 512); 0: never — every CTA loads its tile into registers itself.  Bitwise
-                          the same results either way                                                              */
+#define MHD_OPT_TMA 13 /* 1: the in-core y / z passes (N = 128, 256, 512; all but the pass that builds J^ on load) run as a
+                          persistent pipeline fed by the tensor-memory accelerator (cp.async.bulk.tensor into a ring of
+                          shared-memory tiles, mbarrier completion); 0 (default): every CTA loads its tile into registers
+                          itself — measured faster at every size.  Same results to roundoff
+                          (bitwise at N = 128, 256, where both use the same butterfly plan)                         */
 
 #define MHD_OPT_OOC_BRICK 5 /* chunked pipeline: largest number of ky columns per brick (0 = what the staging allows) */
 #define MHD_OPT_OOC_SLAB 6  /* chunked pipeline: largest number of z planes per slab  (0 = what the staging allows) */

@@ -65,7 +65,7 @@ struct mhd_ctx {
     cd* ftw = nullptr;     // lane-contiguous tables of the fused x sweep
     alignas(64) unsigned char tmaps[4 * 128];   // CUtensorMap x 4 over the field buffers (TMA-fed strided passes)
     StridedTma tma;
-    int opt_tma = 1;       // MHD_OPT_TMA
+    int opt_tma = 0;       // MHD_OPT_TMA
     cd *U[8], *Rold[8], *W[16], *X[8], *Y[8], *nyq[3];
     double *scratch = nullptr, *res = nullptr;
     // chunked ("out-of-core") pipeline, see ooc.cu

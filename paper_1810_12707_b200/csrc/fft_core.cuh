@@ -198,8 +198,12 @@ template <> struct Plan<256>  { static constexpr int NS = 2, R0 = 16, R1 = 16, R
 template <> struct Plan<512>  { static constexpr int NS = 3, R0 = 8,  R1 = 8,  R2 = 8, E = 16; };
 template <> struct Plan<1024> { static constexpr int NS = 3, R0 = 16, R1 = 8,  R2 = 8, E = 16; };
 
-template <int NL> struct PlanInfo {
-    typedef Plan<NL> P;
+// alternative plan of the 512-point strided passes: ONE shared-memory exchange instead of two (32 points per thread,
+// radix 32 then radix 16); chosen per kernel through the PL parameter below
+struct Plan512x { static constexpr int NS = 2, R0 = 32, R1 = 16, R2 = 1, E = 32; };
+
+template <int NL, class PL = Plan<NL>> struct PlanInfo {
+    typedef PL P;
     static constexpr int E = P::E;
     static constexpr int T = NL / E;    // threads per line
 };
@@ -225,10 +229,10 @@ struct GroupSync {
 };
 
 // one stage: butterflies on registers; non-final stages scatter to shared memory and gather back
-template <int NL, int R, int NSTRIDE /*Ns*/, bool LAST, bool FIRST, int DIR, int TWS, class Layout, class Sync>
-__device__ __forceinline__ void fft_stage(cd (&v)[PlanInfo<NL>::E], int t, const cd* __restrict__ tw, cd* sm,
+template <int NL, int R, int NSTRIDE /*Ns*/, bool LAST, bool FIRST, int DIR, int TWS, class PL, class Layout, class Sync>
+__device__ __forceinline__ void fft_stage(cd (&v)[PL::E], int t, const cd* __restrict__ tw, cd* sm,
                                           const Layout& L, const Sync& sync) {
-    constexpr int E = PlanInfo<NL>::E, T = PlanInfo<NL>::T, B = E / R;
+    constexpr int E = PL::E, T = NL / PL::E, B = E / R;
     static_assert(E % R == 0, "radix must divide the points per thread");
     if constexpr (!LAST && !FIRST) sync();   // every thread has gathered the previous exchange
 #pragma unroll
@@ -264,19 +268,18 @@ __device__ __forceinline__ void fft_stage(cd (&v)[PlanInfo<NL>::E], int t, const
 // Whole line transform on registers.  On entry v[m] = x[t + T*m]; on exit v[m] = X[t + T*m] with
 // X[q] = sum_n x[n] exp(DIR*2*pi*i*n*q/NL) (unnormalised).  `sm` is the exchange tile (must be free on entry;
 // all threads of the block — or of the group that `sync` joins — must call).  tw[m*TWS] = exp(-2*pi*i*m/NL).
-template <int NL, int DIR, int TWS, class Layout, class Sync = BlockSync>
-__device__ __forceinline__ void fft_line(cd (&v)[PlanInfo<NL>::E], int t, const cd* __restrict__ tw, cd* sm,
+template <int NL, int DIR, int TWS, class Layout, class Sync = BlockSync, class P = Plan<NL>>
+__device__ __forceinline__ void fft_line(cd (&v)[P::E], int t, const cd* __restrict__ tw, cd* sm,
                                          const Layout& L, const Sync& sync = Sync()) {
-    typedef Plan<NL> P;
     if constexpr (P::NS == 1) {
-        fft_stage<NL, P::R0, 1, true, true, DIR, TWS>(v, t, tw, sm, L, sync);
+        fft_stage<NL, P::R0, 1, true, true, DIR, TWS, P>(v, t, tw, sm, L, sync);
     } else if constexpr (P::NS == 2) {
-        fft_stage<NL, P::R0, 1, false, true, DIR, TWS>(v, t, tw, sm, L, sync);
-        fft_stage<NL, P::R1, P::R0, true, false, DIR, TWS>(v, t, tw, sm, L, sync);
+        fft_stage<NL, P::R0, 1, false, true, DIR, TWS, P>(v, t, tw, sm, L, sync);
+        fft_stage<NL, P::R1, P::R0, true, false, DIR, TWS, P>(v, t, tw, sm, L, sync);
     } else {
-        fft_stage<NL, P::R0, 1, false, true, DIR, TWS>(v, t, tw, sm, L, sync);
-        fft_stage<NL, P::R1, P::R0, false, false, DIR, TWS>(v, t, tw, sm, L, sync);
-        fft_stage<NL, P::R2, P::R0 * P::R1, true, false, DIR, TWS>(v, t, tw, sm, L, sync);
+        fft_stage<NL, P::R0, 1, false, true, DIR, TWS, P>(v, t, tw, sm, L, sync);
+        fft_stage<NL, P::R1, P::R0, false, false, DIR, TWS, P>(v, t, tw, sm, L, sync);
+        fft_stage<NL, P::R2, P::R0 * P::R1, true, false, DIR, TWS, P>(v, t, tw, sm, L, sync);
     }
 }
 

@@ -13,6 +13,7 @@
 #include "physics.cuh"
 
 #include <cooperative_groups.h>
+#include <cstdlib>
 namespace cg = cooperative_groups;
 
 namespace mhd {
@@ -34,11 +35,20 @@ template <int N, int C> struct StridedOcc {
     static constexpr int THREADS = C * PlanInfo<N>::T;
     static constexpr int MINB = (512 / THREADS) < 1 ? 1 : ((512 / THREADS) > 8 ? 8 : (512 / THREADS));
 };
+// line plan of the register-fed kernel: N = 512 with 8 columns uses the one-exchange plan (32 points per thread, radix 32 x 16,
+// 128 threads and <= 168 registers: three 64 KB tiles per SM instead of two, one shared-memory round trip instead of two)
+template <int N, int C> struct SPlan { typedef Plan<N> type; static constexpr int MINB = StridedOcc<N, C>::MINB; };
+#ifndef MHD_STRIDED_512_TWO_EXCHANGES
+template <> struct SPlan<512, 8> { typedef Plan512x type; static constexpr int MINB = 3; };
+// (the same idea at N = 1024 — radix 32 x 32, 4-column tiles, three CTAs per SM — measured slower: 51.7 + 70.0 ms against
+// 48.1 + 67.2 ms per step of the chunked pipeline; the twiddled radix-32 stage needs 16 table roots and spills)
+#endif
 
 template <int N, int DIR, int C, bool GEN, bool FJ>
-__global__ void __launch_bounds__(StridedOcc<N, C>::THREADS, StridedOcc<N, C>::MINB)
+__global__ void __launch_bounds__(C * (N / SPlan<N, C>::type::E), SPlan<N, C>::MINB)
 strided_kernel(const __grid_constant__ StridedArgs a) {
-    constexpr int E = PlanInfo<N>::E, T = PlanInfo<N>::T;
+    typedef typename SPlan<N, C>::type PL;
+    constexpr int E = PL::E, T = N / PL::E;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cd* sm = reinterpret_cast<cd*>(smem_raw);
 
@@ -92,7 +102,7 @@ strided_kernel(const __grid_constant__ StridedArgs a) {
             }
         }
     }
-    fft_line<N, DIR, 1>(v, t, a.tw, sm, LayoutPlain{C, c});
+    fft_line<N, DIR, 1, LayoutPlain, BlockSync, PL>(v, t, a.tw, sm, LayoutPlain{C, c});
     if (GEN) {
         cd* __restrict__ out = a.out[f] + (long long)o * a.out_outer_stride + col;
 #pragma unroll
@@ -137,10 +147,11 @@ template <int N, int FPC, int CC> struct S5Cfg {
 };
 
 template <int N, int FPC, int CC>
-__global__ void __launch_bounds__(StridedOcc<N, CC>::THREADS, StridedOcc<N, CC>::MINB)
+__global__ void __launch_bounds__(CC * (N / SPlan<N, CC>::type::E), SPlan<N, CC>::MINB)
 strided_assemble_kernel(const __grid_constant__ StridedArgs a, const __grid_constant__ AssembleTail z) {
     typedef S5Cfg<N, FPC, CC> P;
-    constexpr int E = PlanInfo<N>::E, T = PlanInfo<N>::T, C = CC, NK = P::NK, CL = P::CL, RPC = P::RPC;
+    typedef typename SPlan<N, CC>::type PL;      // same butterfly plan as the two-launch path: bitwise the same numbers
+    constexpr int E = PL::E, T = N / PL::E, C = CC, NK = P::NK, CL = P::CL, RPC = P::RPC;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cd* sm = reinterpret_cast<cd*>(smem_raw);
     cg::cluster_group cluster = cg::this_cluster();
@@ -177,7 +188,7 @@ strided_assemble_kernel(const __grid_constant__ StridedArgs a, const __grid_cons
 #pragma unroll
         for (int m = 0; m < E; ++m) v[m] = valid ? in[(long long)(t + T * m) * a.in_row_stride] : mk(0.0, 0.0);
         if (fi > 0) __syncthreads();        // the previous field's compact rows have left the exchange tile
-        fft_line<N, -1, 1>(v, t, a.tw, sm, LayoutPlain{C, c});
+        fft_line<N, -1, 1, LayoutPlain, BlockSync, PL>(v, t, a.tw, sm, LayoutPlain{C, c});
         __syncthreads();                    // every thread has gathered its last exchange: the tile is free
         // kept rows, compact index i: the last field of the CTA stays in the exchange tile, earlier ones move behind it
         cd* keep = (fi == FPC - 1) ? sm : sm + (size_t)N * C + (size_t)fi * NK * C;
@@ -237,7 +248,7 @@ template <int N, int FPC, int CC> static void s5_configure(cudaLaunchConfig_t& c
     }
     cfg = cudaLaunchConfig_t{};
     cfg.gridDim = dim3(((a.ncols + P::C - 1) / P::C) * P::CL, a.n_outer, 1);
-    cfg.blockDim = dim3(P::C * PlanInfo<N>::T, 1, 1);
+    cfg.blockDim = dim3(P::C * (N / SPlan<N, CC>::type::E), 1, 1);
     cfg.dynamicSmemBytes = P::SMEM;
     cfg.stream = st;
     attr[0].id = cudaLaunchAttributeClusterDimension;
@@ -281,7 +292,7 @@ int strided_assemble_max_clusters(int N, int variant, const StridedArgs& a) {
 }
 
 template <int N, int DIR, int C, bool GEN, bool FJ> static void launch_one(const StridedArgs& a, cudaStream_t st) {
-    constexpr int threads = C * PlanInfo<N>::T;
+    constexpr int threads = C * (N / SPlan<N, C>::type::E);
     constexpr size_t smem = size_t(N) * C * sizeof(cd);
     ensure_dynamic_smem(strided_kernel<N, DIR, C, GEN, FJ>, smem);
     dim3 grid((a.ncols + C - 1) / C, a.n_outer, a.nfields);

@@ -56,8 +56,7 @@ void strided_pass(mhd_ctx* c, int dir, int axis, int nf, const cd* const in[], c
         a.in_rows = (prune && dir > 0) ? 1 : 0;     // inverse: input rows outside the mask are zero
         a.out_rows = (prune && dir < 0) ? 1 : 0;    // forward: output rows outside the mask are not needed
         mhd_ctx::Scope s(c, dir > 0 ? F_STRIDED_INV : F_STRIDED_FWD);
-        // MHD_OPT_TMA: 1 = where it measured at least as fast (N = 512), 2 = wherever the pipeline exists, 0 = never
-        const bool tma = (c->opt_tma == 2 || (c->opt_tma == 1 && N == 512)) && zoff == 0;
+        const bool tma = c->opt_tma != 0 && zoff == 0;      // MHD_OPT_TMA (opt-in: measured slower than the register-fed kernel)
         if (!(tma && launch_strided_tma(N, dir, a, c->tma, c->st))) launch_strided(N, dir, a, c->st);
         done += nb;
     }
@@ -423,8 +422,7 @@ int mhd_set_option(mhd_ctx* c, int option, int value) {
         case MHD_OPT_PRUNE: c->opt_prune = value ? 1 : 0; return MHD_OK;
         case MHD_OPT_FUSE_CURRENT: c->opt_fuse_current = value ? 1 : 0; return MHD_OK;
         case MHD_OPT_TMA:
-            if (value < 0 || value > 2) return c->fail(MHD_ERR_INVALID_ARG, "tma must be 0, 1 or 2");
-            c->opt_tma = value; return MHD_OK;
+            c->opt_tma = value ? 1 : 0; return MHD_OK;
         case MHD_OPT_FUSE_ASSEMBLE:
             if (value < 0 || value > 2) return c->fail(MHD_ERR_INVALID_ARG, "fuse_assemble must be 0, 1 or 2");
             c->opt_fuse_assemble = value; return MHD_OK;

