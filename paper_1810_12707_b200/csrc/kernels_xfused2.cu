@@ -109,7 +109,7 @@ __device__ __forceinline__ void r2c_pair(cd& Zk, cd& Zm, cd w) {
 }
 
 template <int N>
-__global__ void __launch_bounds__(F2<N / 2>::THREADS, (N / 2 == 512) ? 1 : (N / 2 == 256) ? 3 : 4)
+__global__ void __launch_bounds__(F2<N / 2>::THREADS, (N / 2 == 512) ? 1 : (N / 2 == 256) ? 3 : 5)
 x_fused2_kernel(const __grid_constant__ FusedXArgs a) {
     constexpr int H = N / 2;
     typedef F2<H> P;
