@@ -399,7 +399,8 @@ void launch_sqrt_rho_u(long long n, const double* const U[8], double* const w[3]
     sqrt_rho_u_kernel<<<ew_blocks(n, 256), 256, 0, st>>>(n, a, b);
 }
 
-// ---- reductions: fixed grid, fixed tree order -> bitwise reproducible -------------------------------------
+// ---- reductions: fixed grid, fixed tree order -> bitwise reproducible (the scalar diagnostics; the shell spectra below
+//      bin with shared-memory atomicAdd inside a block: reproducible to roundoff only) ---------------------------------
 constexpr int RB = 1024;     // blocks of the first stage
 constexpr int RT = 256;      // threads per block
 constexpr int NRED = 10;     // ke, me, ie, mass, momx, momy, momz, etot (sums); rho_min, p_min
