@@ -196,8 +196,12 @@ int mhd_fft3d_c2r(mhd_ctx *ctx, int nfields, double *const spec[], double *const
  *   of u = m/rho of the current state (L241; needs mhd_set_fields first).
  * While tracers are set, every step of mhd_step() first pushes them once with dt and the B of the state at the START
  * of that step (t_n), then advances the fields.  mhd_tracers_push() pushes nsteps times in the B of the current state
- * without advancing the fields (one kernel; the gather benchmark).  Not available on an out-of-core context. */
+ * without advancing the fields (one kernel; the gather benchmark).
+ * Chunked (MHD_FLAG_OUT_OF_CORE) contexts: the buffer of mhd_tracers_bind must be mhd_tracers_bytes(np) +
+ * mhd_tracers_field_bytes(ctx) long — the tracers then keep their own real-space copies of B (and of rho, m for the
+ * initial velocity), filled slab by slab at the start of every step; not available on a decomposed context. */
 size_t mhd_tracers_bytes(long long np);
+size_t mhd_tracers_field_bytes(const mhd_ctx *ctx);   /* 0 for in-core contexts */
 int mhd_tracers_bind(mhd_ctx *ctx, long long np, void *dev_buffer, size_t bytes);   /* np = 0 detaches */
 int mhd_tracers_set(mhd_ctx *ctx, int where, const double *const pos[3], const double *const vel[3]);
 int mhd_tracers_get(mhd_ctx *ctx, int where, double *const pos[3], double *const vel[3]);

@@ -37,7 +37,7 @@ ERRORS = {-1: "MHD_ERR_INVALID_ARG", -2: "MHD_ERR_NOT_BOUND", -3: "MHD_ERR_NO_FI
 SYMBOLS = ["mhd_init", "mhd_workspace_bytes", "mhd_pinned_bytes", "mhd_bind", "mhd_set_option", "mhd_set_fields",
            "mhd_rhs", "mhd_step", "mhd_get_fields", "mhd_diagnostics", "mhd_nspec", "mhd_fft3d_r2c",
            "mhd_fft3d_c2r", "mhd_launch_count", "mhd_transfer_bytes", "mhd_profile_enable", "mhd_profile_get", "mhd_last_error",
-           "mhd_destroy", "mhd_tracers_bytes", "mhd_tracers_bind", "mhd_tracers_set", "mhd_tracers_get",
+           "mhd_destroy", "mhd_tracers_bytes", "mhd_tracers_field_bytes", "mhd_tracers_bind", "mhd_tracers_set", "mhd_tracers_get",
            "mhd_tracers_push", "mhd_set_param", "mhd_probe_fp64", "mhd_dist_config", "mhd_dist_phase",
            "mhd_dist_counts", "mhd_dist_pack", "mhd_dist_unpack", "mhd_dist_ranges", "mhd_dist_peers",
            "mhd_dist_enable_peer_access"]
@@ -80,6 +80,8 @@ def lib():
     L.mhd_fft3d_c2r.argtypes = [C.c_void_p, C.c_int, P8, P8, C.c_int]
     L.mhd_tracers_bytes.argtypes = [C.c_longlong]
     L.mhd_tracers_bytes.restype = C.c_size_t
+    L.mhd_tracers_field_bytes.argtypes = [C.c_void_p]
+    L.mhd_tracers_field_bytes.restype = C.c_size_t
     L.mhd_tracers_bind.argtypes = [C.c_void_p, C.c_longlong, C.c_void_p, C.c_size_t]
     L.mhd_tracers_set.argtypes = [C.c_void_p, C.c_int, P8, P8]
     L.mhd_tracers_get.argtypes = [C.c_void_p, C.c_int, P8, P8]
@@ -285,7 +287,7 @@ class MHD:
         torch = self.torch
         n = int(pos[0].numel() if isinstance(pos[0], torch.Tensor) else np.asarray(pos[0]).size)
         if getattr(self, "_ntr", 0) != n:
-            nbytes = int(self._L.mhd_tracers_bytes(n))
+            nbytes = int(self._L.mhd_tracers_bytes(n)) + int(self._L.mhd_tracers_field_bytes(self._h))
             with torch.cuda.device(self.device):
                 self._trbuf = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
             base = (self._trbuf.data_ptr() + 255) // 256 * 256

@@ -113,6 +113,7 @@ struct mhd_ctx {
         double* alt[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
         long long *id = nullptr, *alt_id = nullptr;
         unsigned *hist = nullptr, *key = nullptr, *rank = nullptr;
+        double* field[4] = {nullptr, nullptr, nullptr, nullptr};   // chunked contexts: real-space field copies (B; rho, m)
         bool sorted = false;           // storage order != id order
         int since_sort = 0;            // pushes since the last sort
     } tr;
@@ -176,6 +177,7 @@ int ooc_set_fields(mhd_ctx* c, int kind, int where, const double* const f[8]);
 int ooc_get_fields(mhd_ctx* c, int kind, int where, double* const out[8]);
 int ooc_rhs(mhd_ctx* c, int where, double* const out[8]);
 int ooc_step(mhd_ctx* c, int nsteps);
+int ooc_real_fields(mhd_ctx* c, double* const out[8]);
 int ooc_diagnostics(mhd_ctx* c, mhd_diag* d, double* spec_kin, double* spec_mag, int nspec);
 int ooc_dist_config(mhd_ctx* c, int rank, int world);
 int ooc_dist_phase(mhd_ctx* c, int phase, int arg);

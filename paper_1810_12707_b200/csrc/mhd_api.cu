@@ -279,6 +279,12 @@ bool tracers_active(const mhd_ctx* c) { return c->tr.np > 0 && c->tr.set; }
 bool tracers_fused_emit(const mhd_ctx* c) { return c->opt_fused == 1 && x_fused2_supported(c->N) && c->integrator == 0; }
 // real-space B of the current state -> X[0..2] by a separate pruned inverse transform (U^ is left intact)
 void tracers_real_B(mhd_ctx* c, double* Breal[3]) {
+    if (c->ooc.on) {            // chunked pipeline: the slab stage of mhd_get_fields, B only, into the tracers' own arrays
+        double* out[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, c->tr.field[0], c->tr.field[1], c->tr.field[2]};
+        for (int d = 0; d < 3; ++d) Breal[d] = c->tr.field[d];
+        ooc_real_fields(c, out);
+        return;
+    }
     const cd* spec[3] = {c->U[5], c->U[6], c->U[7]};
     cd* work[3] = {c->X[0], c->X[1], c->X[2]};
     for (int d = 0; d < 3; ++d) Breal[d] = reinterpret_cast<double*>(c->X[d]);
@@ -519,7 +525,16 @@ int mhd_step(mhd_ctx* c, int nsteps) {
     if (!c || nsteps < 0) return MHD_ERR_INVALID_ARG;
     if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
     if (!c->have_fields) return c->fail(MHD_ERR_NO_FIELDS, "mhd_set_fields has not been called");
-    if (c->ooc.on) return ooc_step(c, nsteps);
+    if (c->ooc.on) {
+        if (!tracers_active(c)) return ooc_step(c, nsteps);
+        for (int s = 0; s < nsteps; ++s) {      // tracers feel the B of the state at the start of each step
+            double* Breal[3];
+            tracers_real_B(c, Breal);
+            tracers_push_with(c, Breal, 1);
+            if (int rc = ooc_step(c, 1)) return rc;
+        }
+        return check_cuda(c, "step (chunked, tracers)");
+    }
     const SpecGeom g = c->geom();
     SpecGeom gp = g; gp.pruned = 1;
     if (c->opt_stress && c->integrator != 0) return c->fail(MHD_ERR_INVALID_ARG, "the stress-tensor variant is implemented for Adams-Bashforth only");
@@ -643,6 +658,10 @@ int mhd_fft3d_c2r(mhd_ctx* c, int nfields, double* const spec[], double* const r
 
 // 12 particle arrays (two sets: the spatial sort ping-pongs), 2 id arrays, key + rank, 2^20 histogram bins
 static size_t tracer_hist_bytes() { return align_up(((size_t)1 << 20) * sizeof(unsigned)); }
+size_t mhd_tracers_field_bytes(const mhd_ctx* c) {
+    if (!c || !c->ooc.on) return 0;
+    return 4 * align_up((size_t)c->n3() * sizeof(double));
+}
 size_t mhd_tracers_bytes(long long np) {
     if (np <= 0) return 0;
     return 14 * align_up((size_t)np * sizeof(double)) + 2 * align_up((size_t)np * sizeof(unsigned)) + tracer_hist_bytes();
@@ -651,11 +670,11 @@ size_t mhd_tracers_bytes(long long np) {
 int mhd_tracers_bind(mhd_ctx* c, long long np, void* dev_buffer, size_t bytes) {
     if (!c || np < 0) return MHD_ERR_INVALID_ARG;
     if (!c->bound) return c->fail(MHD_ERR_NOT_BOUND, "mhd_bind has not been called");
-    if (c->ooc.on) return c->fail(MHD_ERR_INVALID_ARG, "tracers need an in-core context");
+    if (c->ooc.on && c->ooc.world > 1) return c->fail(MHD_ERR_INVALID_ARG, "tracers are not available on a decomposed context");
     c->tr = mhd_ctx::Tracers();
     if (np == 0) return MHD_OK;
     if (!dev_buffer || ((uintptr_t)dev_buffer & 255) != 0) return c->fail(MHD_ERR_INVALID_ARG, "tracer buffer must be 256-byte aligned");
-    if (bytes < mhd_tracers_bytes(np)) return c->fail(MHD_ERR_NOMEM, "tracer buffer too small");
+    if (bytes < mhd_tracers_bytes(np) + mhd_tracers_field_bytes(c)) return c->fail(MHD_ERR_NOMEM, "tracer buffer too small");
     if (np >= ((long long)1 << 32)) return c->fail(MHD_ERR_INVALID_ARG, "at most 2^32 - 1 tracers");
     const size_t stride = align_up((size_t)np * sizeof(double)), istride = align_up((size_t)np * sizeof(unsigned));
     char* b = static_cast<char*>(dev_buffer);
@@ -669,6 +688,9 @@ int mhd_tracers_bind(mhd_ctx* c, long long np, void* dev_buffer, size_t bytes) {
     c->tr.key = reinterpret_cast<unsigned*>(b + 14 * stride);
     c->tr.rank = reinterpret_cast<unsigned*>(b + 14 * stride + istride);
     c->tr.hist = reinterpret_cast<unsigned*>(b + 14 * stride + 2 * istride);
+    if (c->ooc.on)          // chunked context: the real-space field copies follow the particle storage
+        for (int f = 0; f < 4; ++f)
+            c->tr.field[f] = reinterpret_cast<double*>(b + mhd_tracers_bytes(np) + (size_t)f * align_up((size_t)c->n3() * sizeof(double)));
     c->tr.np = np;
     return MHD_OK;
 }
@@ -688,7 +710,13 @@ int mhd_tracers_set(mhd_ctx* c, int where, const double* const pos[3], const dou
     }
     { mhd_ctx::Scope s(c, F_TRACERS, 2); launch_tracer_wrap(tracer_args(c, nullptr, 0), c->st); launch_tracer_iota(c->tr.np, c->tr.id, c->st); }
     c->tr.sorted = false; c->tr.since_sort = 0;
-    if (!vel) {      // v0 = CIC of u = m/rho (L241): real-space rho, m of the current state -> X[0..3]
+    if (!vel && c->ooc.on) {     // chunked context: real-space rho, m through the slab stage into the tracers' field arrays
+        double* out[8] = {c->tr.field[0], c->tr.field[1], c->tr.field[2], c->tr.field[3], nullptr, nullptr, nullptr, nullptr};
+        if (int rc = ooc_real_fields(c, out)) return rc;
+        const double* m[3] = {c->tr.field[1], c->tr.field[2], c->tr.field[3]};
+        mhd_ctx::Scope s(c, F_TRACERS);
+        launch_tracer_init_velocity(tracer_args(c, nullptr, 0), c->tr.field[0], m, c->st);
+    } else if (!vel) {      // v0 = CIC of u = m/rho (L241): real-space rho, m of the current state -> X[0..3]
         const cd* spec[4] = {c->U[0], c->U[1], c->U[2], c->U[3]};
         cd* work[4] = {c->X[0], c->X[1], c->X[2], c->X[3]};
         double* real[4];

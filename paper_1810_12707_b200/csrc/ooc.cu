@@ -372,7 +372,8 @@ int stage_slabs(mhd_ctx* c, SlabKind kind, const SlabIO& io) {
             if (io.kind == MHD_PRIMITIVE) { mhd_ctx::Scope s(c, F_POINT); launch_cons_to_prim(nlines * N, real, c->gamma, c->st); }
             if (io.user_out && io.where == MHD_DEVICE)
                 for (int f = 0; f < 8; ++f)
-                    cudaMemcpyAsync(io.user_out[f] + (size_t)z0 * plane_r, real[f], (size_t)zc * plane_r * sizeof(double), cudaMemcpyDeviceToDevice, c->st);
+                    if (io.user_out[f])
+                        cudaMemcpyAsync(io.user_out[f] + (size_t)z0 * plane_r, real[f], (size_t)zc * plane_r * sizeof(double), cudaMemcpyDeviceToDevice, c->st);
         } else {             // SLAB_FROM_REAL
             if (io.kind == MHD_PRIMITIVE) { mhd_ctx::Scope s(c, F_POINT); launch_prim_to_cons(nlines * N, real, c->gamma, c->st); }
             XArgs a; std::memset(&a, 0, sizeof(a));
@@ -389,7 +390,8 @@ int stage_slabs(mhd_ctx* c, SlabKind kind, const SlabIO& io) {
             if (io.nout > 0 && o.work_host)
                 for (int f = 0; f < io.nout; ++f) d2h_1d(c, o.WzS[f] + (size_t)z0 * plane_c, out[f], (size_t)zc * plane_c * sizeof(cd));
             if (user_d2h)
-                for (int f = 0; f < 8; ++f) d2h_1d(c, io.user_out[f] + (size_t)z0 * plane_r, real[f], (size_t)zc * plane_r * sizeof(double));
+                for (int f = 0; f < 8; ++f)
+                    if (io.user_out[f]) d2h_1d(c, io.user_out[f] + (size_t)z0 * plane_r, real[f], (size_t)zc * plane_r * sizeof(double));
             chunk_d2h_done(c, ch);
         }
     }
@@ -608,6 +610,17 @@ int ooc_get_fields(mhd_ctx* c, int kind, int where, double* const out[8]) {
     if (rc) return rc;
     if (where == MHD_HOST) cudaStreamSynchronize(c->st);
     return check_cuda(c, "get_fields (chunked)");
+}
+
+// real-space conservative fields of the current state into DEVICE arrays; out[f] == null: field f is not wanted
+// (tracers: B for the push, rho and m for the initial velocity)
+int ooc_real_fields(mhd_ctx* c, double* const out[8]) {
+    if (c->ooc.world > 1) return c->fail(MHD_ERR_INVALID_ARG, "not available on a decomposed context");
+    int rc = stage_inverse_z(c, c->ooc.Uc, false);
+    if (rc) return rc;
+    SlabIO io; io.nin = 8; io.nout = 0; io.kind = MHD_CONSERVATIVE; io.where = MHD_DEVICE; io.user_out = out;
+    rc = stage_slabs(c, SLAB_TO_REAL, io);
+    return rc ? rc : check_cuda(c, "real fields (chunked)");
 }
 
 static int ooc_products(mhd_ctx* c, bool have_inverse_z = false) {
