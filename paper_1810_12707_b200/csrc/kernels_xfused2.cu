@@ -46,8 +46,10 @@ template <int H> __device__ __forceinline__ int tidx(int row, int slot) { return
 // (ncu on the first cut of this kernel: 3.4x more L1 load sectors than data because of scattered table reads).
 //   TA[r][t] = exp(-2 pi i (jA(t) + r R1)/N)      split / merge factor of the rows of butterfly jA
 //   TB[r][t] = exp(-2 pi i (jB(t) + r R1)/N)      same for butterfly jB (used by t = 0 only)
-//   TS[b][r][t] = exp(-2 pi i r (t + b T)/H)      second inverse stage
-//   TF[w][r][t] = exp(-2 pi i r j_w(t)/H)         last forward stage, w = 0: jA, 1: jB
+//   TS[b][e][t] = root e of the twiddle-folded radix-R1 butterfly j = t + b T of the second inverse stage
+//                 (fft_core.cuh TDft: exp(-2 pi i 2^l (j + q R0)/H) for level l, position q)
+//   TF[e][t]    = root e of the twiddle-folded radix-R0 butterfly jA = t of the last forward stage; the roots of its mirror
+//                 butterfly jB = R1 - jA follow from them (mirror_roots); lane 0's jB = R1/2 has its own: TF[NR0 T + e]
 template <int H> struct FTab {
     typedef F2<H> P;
     static constexpr int TA = 0;
@@ -56,6 +58,32 @@ template <int H> struct FTab {
     static constexpr int TF = TS + H;
     static constexpr int SIZE = TF + 2 * P::R0 * P::T;
 };
+
+// root e of TDft<R> for a butterfly with k = j mod Ns: exp(-2 pi i (2^l (k + q Ns)) / (Ns R)), (l, q) = position of e
+__device__ inline void root_fraction(int R, int e, int k, int Ns, long long* num, int* den) {
+    int Rl = R, l = 0;
+    for (;;) {
+        const int top = Rl >= 4 ? Rl / 4 : 1;
+        if (e < top) break;
+        e -= top; Rl /= 2; ++l;
+    }
+    *num = ((long long)k + (long long)e * Ns) << l;
+    *den = Ns * R;
+}
+// roots of the mirror butterfly R1 - j (base exp(-2 pi i/R0) conj(w)) from those of butterfly j: level by level the entry
+// a quarter turn away, conjugated and rotated — sign flips and swaps only
+template <int R> __device__ __forceinline__ void mirror_roots(const cd* wa, cd* wb) {
+    if constexpr (R >= 2) {
+        constexpr int TOP = TwCount<R>::TOP;
+        if constexpr (R >= 4) {
+#pragma unroll
+            for (int q = 0; q < TOP; ++q) { const cd a = wa[TOP - 1 - q]; wb[q] = mk(-a.y, -a.x); }
+        } else {
+            wb[0] = mk(-wa[0].x, wa[0].y);
+        }
+        mirror_roots<R / 2>(wa + TOP, wb + TOP);
+    }
+}
 
 template <int H> __global__ void fused_twiddle_kernel(cd* tab) {
     typedef F2<H> P;
@@ -68,14 +96,17 @@ template <int H> __global__ void fused_twiddle_kernel(cd* tab) {
         const int j = which == 0 ? t : (t == 0 ? R1 / 2 : R1 - t);
         num = j + r * R1; den = N;
     } else if (i < FTab<H>::TF) {                // TS
-        const int k = i - FTab<H>::TS, b = k / (R1 * T), r = (k % (R1 * T)) / T, t = k % T;
-        num = (long long)r * (t + b * T); den = H;
-        (void)NB;
+        constexpr int NR1 = TwCount<R1>::value;
+        const int k = i - FTab<H>::TS;
+        if (k >= NB * NR1 * T) { tab[i] = mk(0.0, 0.0); return; }
+        const int b = k / (NR1 * T), e = (k % (NR1 * T)) / T, t = k % T;
+        root_fraction(R1, e, t + b * T, R0, &num, &den);
     } else {                                     // TF
-        const int k = i - FTab<H>::TF, which = k / (R0 * T), r = (k % (R0 * T)) / T, t = k % T;
-        const int j = which == 0 ? t : (t == 0 ? R1 / 2 : R1 - t);
-        num = (long long)r * j; den = H;
-        if (which == 0 && t == 0) { num = r; den = 2 * R0; }      // lane 0: exp(-2 pi i r/(2 R0)) = w_H^(r R1/2)
+        constexpr int NR0 = TwCount<R0>::value;
+        const int k = i - FTab<H>::TF;
+        if (k < NR0 * T) root_fraction(R0, k / T, k % T, R1, &num, &den);
+        else if (k < NR0 * T + NR0) root_fraction(R0, k - NR0 * T, R1 / 2, R1, &num, &den);
+        else { tab[i] = mk(0.0, 0.0); return; }
     }
     double sn, cs;
     sincospi(2.0 * (double)(num % den) / (double)den, &sn, &cs);
@@ -174,9 +205,10 @@ x_fused2_kernel(const __grid_constant__ FusedXArgs a) {
             cd u[R1];
 #pragma unroll
             for (int r = 0; r < R1; ++r) u[r] = sm[tidx<H>(j + r * R0, slot)];
+            cd w[TwCount<R1>::value];
 #pragma unroll
-            for (int r = 1; r < R1; ++r) u[r] = twmul<+1>(u[r], __ldg(&tab[FT::TS + (b * R1 + r) * T + t]));
-            Dft<R1, +1>::run(u);
+            for (int e = 0; e < TwCount<R1>::value; ++e) w[e] = __ldg(&tab[FT::TS + (b * TwCount<R1>::value + e) * T + t]);
+            TDft<R1, +1>::run(u, w);
 #pragma unroll
             for (int q = 0; q < R1; ++q) sm[tidx<H>(j + q * R0, slot)] = u[q];
         }
@@ -226,16 +258,21 @@ x_fused2_kernel(const __grid_constant__ FusedXArgs a) {
             za[r] = sm[tidx<H>(r + jA * R0, slot)];      // Y[r][jA]
             zb[r] = sm[tidx<H>(r + jB * R0, slot)];
         }
-        // w^(r jB) = exp(-2 pi i r/R0) * conj(w^(r jA)) for jB = R1 - jA; lane t = 0 (jA = 0, jB = R1/2) finds
-        // exp(-2 pi i r/(2 R0)) in its TF entry instead and skips the (unit) factor of za
-        static_for<1, R0>([&](auto rc) {
-            constexpr int r = decltype(rc)::value;
-            const cd w = __ldg(&tab[FT::TF + r * T + t]);
-            if (t != 0) za[r] = twmul<-1>(za[r], w);
-            zb[r] = mul_rootN<R0, r, -1>(twmul<+1>(zb[r], w));
-        });
-        Dft<R0, -1>::run(za);
-        Dft<R0, -1>::run(zb);
+        // twiddle-folded butterflies: the roots of jA come from the table (lane 0: jA = 0, plain roots of unity), those of
+        // jB = R1 - jA by mirror_roots; lane 0 (jB = R1/2) reads its own
+        {
+            constexpr int NR0 = TwCount<R0>::value;
+            cd wa[NR0], wb[NR0];
+#pragma unroll
+            for (int e = 0; e < NR0; ++e) wa[e] = __ldg(&tab[FT::TF + e * T + t]);
+            mirror_roots<R0>(wa, wb);
+            if (t == 0) {
+#pragma unroll
+                for (int e = 0; e < NR0; ++e) wb[e] = __ldg(&tab[FT::TF + NR0 * T + e]);
+            }
+            TDft<R0, -1>::run(za, wa);
+            TDft<R0, -1>::run(zb, wb);
+        }
         // za[q] = Z[jA + q*R1], zb[q] = Z[jB + q*R1]
         if (t != 0) {
             const cd w0 = __ldg(&tab[FT::TA + t]);
