@@ -131,12 +131,13 @@ __device__ __forceinline__ void c2r_pair(cd& A, cd& B, cd ws, double scale) {
     B = mk(fma(scale, Sx, q), fma(-scale, Sy, p));
 }
 // R2C merge of one mirror pair: Zk = Z[k], Zm = Z[H-k]:  X[k] -> Zk, X[H-k] -> Zm
-__device__ __forceinline__ void r2c_pair(cd& Zk, cd& Zm, cd w) {
+// wh = w / 2: the halving rides on the twiddle and on four FMAs
+__device__ __forceinline__ void r2c_pair(cd& Zk, cd& Zm, cd wh) {
     const double Sx = Zk.x + Zm.x, Sy = Zk.y - Zm.y;
     const double Dx = Zk.x - Zm.x, Dy = Zk.y + Zm.y;
-    const double gx = w.x * Dx - w.y * Dy, gy = w.x * Dy + w.y * Dx;
-    Zk = mk(0.5 * (Sx + gy), 0.5 * (Sy - gx));
-    Zm = mk(0.5 * (Sx - gy), -0.5 * (Sy + gx));
+    const double gx = fma(wh.x, Dx, -(wh.y * Dy)), gy = fma(wh.x, Dy, wh.y * Dx);
+    Zk = mk(fma(0.5, Sx, gy), fma(0.5, Sy, -gx));
+    Zm = mk(fma(0.5, Sx, -gy), fma(-0.5, Sy, -gx));
 }
 
 template <int N>
@@ -275,7 +276,7 @@ x_fused2_kernel(const __grid_constant__ FusedXArgs a) {
         }
         // za[q] = Z[jA + q*R1], zb[q] = Z[jB + q*R1]
         if (t != 0) {
-            const cd w0 = __ldg(&tab[FT::TA + t]);
+            const cd w0 = 0.5 * __ldg(&tab[FT::TA + t]);
             static_for<0, R0>([&](auto qc) {
                 constexpr int q = decltype(qc)::value;
                 r2c_pair(za[q], zb[R0 - 1 - q], mul_rootN<2 * R0, q, -1>(w0));
@@ -283,8 +284,8 @@ x_fused2_kernel(const __grid_constant__ FusedXArgs a) {
         } else {
             za[0] = mk(za[0].x + za[0].y, 0.0);                         // k = 0 (Nyquist partner dropped)
             za[R0 / 2] = mk(za[R0 / 2].x, -za[R0 / 2].y);               // k = H/2
-            const cd one = mk(1.0, 0.0);
-            const cd wh = __ldg(&tab[FT::TB]);
+            const cd one = mk(0.5, 0.0);
+            const cd wh = 0.5 * __ldg(&tab[FT::TB]);
             static_for<1, R0 / 2>([&](auto qc) {
                 constexpr int q = decltype(qc)::value;
                 r2c_pair(za[q], za[R0 - q], mul_rootN<2 * R0, q, -1>(one));
