@@ -9,6 +9,22 @@
 extern "C" {
 #endif
 
+/* A/B switches for mhd_set_option(): alternative kernels that were built, are parity-tested and measured SLOWER than the
+ * defaults on B200 (DESIGN.md section 6 has the numbers).  They exist so that the measurements can be repeated; they are
+ * not part of the method's interface. */
+#define MHD_OPT_FUSE_ASSEMBLE 7 /* sweep S5 (in-core contexts, default equation set, N = 64..512) as ONE launch: the forward z
+                                pass runs in thread-block clusters — 1: 16 CTAs, one per product field; 2: 8 CTAs, two
+                                fields each — that keep the transformed rows in shared memory and assemble R^ and the
+                                explicit update from each other's tiles (distributed shared memory).  Bitwise the
+                                two-launch result; measured slower on B200, so the default is
+                                0: forward z pass and assembly as two launches                                 */
+
+#define MHD_OPT_TMA 13 /* 1: the in-core y / z passes (N = 128, 256, 512; all but the pass that builds J^ on load) run as a
+                          persistent pipeline fed by the tensor-memory accelerator (cp.async.bulk.tensor into a ring of
+                          shared-memory tiles, mbarrier completion); 0 (default): every CTA loads its tile into registers
+                          itself — measured faster at every size.  Same results to roundoff
+                          (bitwise at N = 128, 256, where both use the same butterfly plan)                         */
+
 /* Measurement helper for the bench (not part of the method): fp64 instructions per second of a register-only DFMA
  * kernel on the current device = the issue ceiling of the fp64 pipe ("measure it with an FMA
  * micro-benchmark"); flop/s of pure-FMA code is twice that. */
