@@ -129,8 +129,9 @@ size_t mhd_pinned_bytes(int N, unsigned flags);
  * cuda_stream: a cudaStream_t (NULL = legacy default stream); pinned_host/pinned_bytes: page-locked host
  * memory, 256-byte aligned, >= mhd_pinned_bytes(N, flags), for the host-resident classes of the chunked pipeline
  * (NULL/0 otherwise); the caller keeps it alive like the workspace.  Builds the twiddle tables (device work).
- * A context bound with MHD_FLAG_OUT_OF_CORE implements every call except mhd_fft3d_*, the kinetic spectrum of
- * mhd_diagnostics (needs an unpruned transform) and the RK4 / predictor-corrector integrators. */
+ * A context bound with MHD_FLAG_OUT_OF_CORE implements every call — including tracers, and the RK4 / predictor-corrector
+ * integrators when MHD_FLAG_STAGE_STORAGE was given — except mhd_fft3d_*, the kinetic spectrum of mhd_diagnostics (needs an
+ * unpruned transform) and the forcing / stress-tensor variants (refused with MHD_ERR_INVALID_ARG). */
 int mhd_bind(mhd_ctx *ctx, void *dev_workspace, size_t bytes, void *cuda_stream, unsigned flags,
              void *pinned_host, size_t pinned_bytes);
 
