@@ -160,6 +160,35 @@ int mhd_get_fields(mhd_ctx *ctx, int kind, int where, double *const out[8]);
 int mhd_diagnostics(mhd_ctx *ctx, mhd_diag *d, double *spec_kin, double *spec_mag, int nspec);
 int mhd_nspec(int N);
 
+/* ---- Diagnostics without a workspace -------------------------------------------------------------------------------
+ * The scalar part of mhd_diagnostics (energies "per grid"; R8) for callers that can
+ * give the library no device memory at all.  Everything above needs mhd_bind() and therefore a caller that can allocate
+ * a workspace.  Some cannot: a monitoring or check-pointing hook that is only handed the eight field pointers of a solver
+ * it does not own; a plug-in inside an application that reserved all of HBM for its own arena and exposes no allocator;
+ * a health check that runs while another thread captures a CUDA graph, where cudaMalloc / cudaFree (which synchronise the
+ * device) must not be called.  This one call needs no mhd_ctx and performs NO allocation of any kind (no cudaMalloc,
+ * cudaFree, or library routine that allocates): the 80 KB of block partials that the two-stage reduction keeps between its
+ * kernels live in a static __device__ array of libmhd.so, which every GPU that loads the library holds until the process
+ * exits.
+ *   n        grid points per field, 1 <= n <= MHD_NOALLOC_MAX_POINTS (2^30 = 1024^3, the library's largest grid); larger n is
+ *            refused with MHD_ERR_INVALID_ARG and a message — the static array is fixed at 1024 blocks x 10 partials;
+ *   gamma    adiabatic index > 1;
+ *   dev_U    host array of 8 DEVICE pointers, conservative order (rho, mx, my, mz, E, Bx, By, Bz), n doubles each, read only;
+ *   dev_out  DEVICE pointer to 10 doubles, written: ke, me, ie, mass, mom[0..2], etot (volume means as in mhd_diag),
+ *            rho_min, p_min.  Bit for bit what mhd_diagnostics() reports for the same real-space arrays;
+ *   cuda_stream  a cudaStream_t (NULL = legacy default stream); the two kernels are enqueued there and the call returns
+ *            without synchronising; pointers belong to the current device;
+ *   errbuf   optional host buffer (errbuf_len bytes) that receives a description when the return value is not MHD_OK.
+ * Set-up: the FIRST call on each device looks up the device address of the static array (cudaGetSymbolAddress, with that
+ * device current) and caches it; make that first call at start-up, before any stream capture begins.
+ * Sharing: all calls on one GPU — from any thread, stream or context — use the same array.  It keeps the previous call's
+ * partials; the first kernel overwrites every entry, so nothing needs clearing, but two calls whose kernels overlap on
+ * the GPU (different streams, no ordering between them) race on it and return garbage.  Order them, e.g. by using one
+ * stream. */
+#define MHD_NOALLOC_MAX_POINTS (1LL << 30)
+int mhd_energy_means_noalloc(long long n, double gamma, const double *const dev_U[8], double *dev_out,
+                             void *cuda_stream, char *errbuf, size_t errbuf_len);
+
 /* Stand-alone batched 3-D real FFT on DEVICE buffers (the FFT metric of BASELINE.json).
  *   r2c: real[i] (N^3 doubles) -> spec[i]: N*N*(N/2) complex doubles [kz][ky][kx], kx = 0..N/2-1, unnormalised
  *        forward transform F(n) = sum_x f(x) exp(-i k.x); the Nyquist column kx = N/2 goes to nyq[i]

@@ -40,7 +40,7 @@ SYMBOLS = ["mhd_init", "mhd_workspace_bytes", "mhd_pinned_bytes", "mhd_bind", "m
            "mhd_destroy", "mhd_tracers_bytes", "mhd_tracers_field_bytes", "mhd_tracers_bind", "mhd_tracers_set", "mhd_tracers_get",
            "mhd_tracers_push", "mhd_set_param", "mhd_probe_fp64", "mhd_dist_config", "mhd_dist_phase",
            "mhd_dist_counts", "mhd_dist_pack", "mhd_dist_unpack", "mhd_dist_ranges", "mhd_dist_peers",
-           "mhd_dist_enable_peer_access"]
+           "mhd_dist_enable_peer_access", "mhd_energy_means_noalloc"]
 
 
 class MhdDiag(C.Structure):
@@ -96,6 +96,7 @@ def lib():
     L.mhd_last_error.argtypes = [C.c_void_p]
     L.mhd_last_error.restype = C.c_char_p
     L.mhd_destroy.argtypes = [C.c_void_p]
+    L.mhd_energy_means_noalloc.argtypes = [C.c_longlong, C.c_double, P8, C.c_void_p, C.c_void_p, C.c_char_p, C.c_size_t]
     _lib = L
     return L
 
@@ -105,6 +106,27 @@ def _ptr_array(ptrs):
     for i, p in enumerate(ptrs):
         a[i] = p
     return a
+
+
+NOALLOC_MAX_POINTS = 1 << 30
+NOALLOC_KEYS = ("ke", "me", "ie", "mass", "momx", "momy", "momz", "etot", "rho_min", "p_min")
+
+
+def energy_means_noalloc(fields, gamma, out, stream=None):
+    """mhd_energy_means_noalloc (include/mhd.h): scalar diagnostics of 8 real-space conservative fields for callers that
+    cannot allocate device memory.  `fields`: 8 contiguous float64 CUDA tensors of equal size; `out`: a float64 CUDA tensor
+    of 10 elements that the caller already owns (this wrapper allocates nothing on the device either); `stream`: a
+    torch.cuda.Stream or None for the current one.  Asynchronous: read `out` after synchronising the stream."""
+    import torch
+    assert len(fields) == 8 and all(f.is_cuda and f.dtype == torch.float64 and f.is_contiguous() for f in fields)
+    assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() >= 10
+    st = stream if stream is not None else torch.cuda.current_stream(fields[0].device)
+    err = C.create_string_buffer(256)
+    with torch.cuda.device(fields[0].device):
+        rc = lib().mhd_energy_means_noalloc(fields[0].numel(), float(gamma), _ptr_array([f.data_ptr() for f in fields]),
+                                            out.data_ptr(), st.cuda_stream, err, len(err))
+    if rc != MHD_OK:
+        raise RuntimeError("libmhd: %s: %s" % (ERRORS.get(rc, rc), err.value.decode()))
 
 
 class MHD:
