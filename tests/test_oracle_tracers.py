@@ -265,3 +265,46 @@ def test_tp12_crossing_zero_with_negative_velocity():
     assert abs(p[0][0] - 0.75) <= 1e-13 and abs(p[1][0] - 1.5) <= 1e-13
     for c in range(3):
         assert 0.0 <= p[c][0] < L
+
+
+def test_tp13_initial_velocity_is_cic_of_the_grid_point_velocity_with_nonuniform_density():
+    """Reading T3 (the tracers start with the fluid velocity) on a NON-uniform density: the oracle's own
+    attach path (orc_tracers_set with no velocities) interpolates u = m/rho formed AT THE GRID POINTS.  With
+    rho = 1.5 + 0.5 cos x, u = (a sin x, b cos 2y, c) every conservative field is band-limited (the projection of
+    set_fields leaves it alone), the fields do not depend on z, and Eq. 20 reduces to linear interpolation between the
+    neighbouring grid values: v0_x = (1-w_x) a sin x_i + w_x a sin x_{i+1}, v0_y likewise in y, v0_z = c.
+    The tempting alternatives differ at the 1e-2 level and fail: CIC(m)/CIC(rho), m without the division, and a rho taken
+    from a neighbouring corner (TP9's uniform rho cannot tell these apart)."""
+    N = 16
+    h = L / N
+    a, b, c = 0.7, -0.4, 0.25
+    x = np.arange(N) * h
+    X = np.broadcast_to(x[None, None, :], (N, N, N))
+    Y = np.broadcast_to(x[None, :, None], (N, N, N))
+    rho = 1.5 + 0.5 * np.cos(X)
+    prim = [rho, a * np.sin(X), b * np.cos(2 * Y), np.full((N, N, N), c), np.full((N, N, N), 2.0),
+            np.full((N, N, N), 0.1), np.full((N, N, N), 0.2), np.full((N, N, N), 0.3)]
+    o = oracle.Oracle(N, L, 5.0 / 3.0, 0.0, 0.0, 1e-3)
+    o.set_fields([np.ascontiguousarray(p) for p in prim], "primitive")
+    rng = np.random.default_rng(13)
+    pos = rand_pos(200, rng)
+    o.tracers_set(pos)
+    _, v0 = o.tracers_get()
+
+    def lin(f, s):                       # linear interpolation of the periodic grid function f(x_i) at positions s
+        i = np.floor(s / h).astype(int)
+        w = s / h - i
+        return (1 - w) * f(x[i % N]) + w * f(x[(i + 1) % N])
+
+    want = [lin(lambda t: a * np.sin(t), pos[0]), lin(lambda t: b * np.cos(2 * t), pos[1]), np.full(200, c)]
+    for k in range(3):
+        assert np.max(np.abs(v0[k] - want[k])) <= 1e-13, k
+    # what the wrong readings would give (x component): all are far from `want`
+    rho_f = lambda t: 1.5 + 0.5 * np.cos(t)
+    m_f = lambda t: rho_f(t) * a * np.sin(t)
+    ratio_of_means = lin(m_f, pos[0]) / lin(rho_f, pos[0])
+    momentum = lin(m_f, pos[0])
+    shifted = lin(lambda t: m_f(t) / rho_f(t + h), pos[0])
+    for wrong in (ratio_of_means, momentum, shifted):
+        assert np.max(np.abs(wrong - want[0])) >= 5e-3
+        assert np.max(np.abs(v0[0] - wrong)) >= 5e-3
