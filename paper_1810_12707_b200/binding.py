@@ -20,7 +20,7 @@ MHD_OK = 0
 MHD_HOST, MHD_DEVICE = 0, 1
 MHD_CONSERVATIVE, MHD_PRIMITIVE = 0, 1
 MHD_OPT_FUSED, MHD_OPT_PRUNE, MHD_OPT_INTEGRATOR, MHD_OPT_FUSE_CURRENT, MHD_OPT_OOC_BRICK, MHD_OPT_OOC_SLAB = 1, 2, 3, 4, 5, 6
-MHD_OPT_FUSE_ASSEMBLE = 7
+MHD_OPT_FUSE_ASSEMBLE = 14
 MHD_OPT_TMA = 13
 MHD_FLAG_OUT_OF_CORE, MHD_FLAG_STATE_ON_HOST, MHD_FLAG_WORK_ON_HOST = 1, 2, 4
 MHD_FLAG_STAGE_STORAGE = 8
@@ -40,7 +40,7 @@ SYMBOLS = ["mhd_init", "mhd_workspace_bytes", "mhd_pinned_bytes", "mhd_bind", "m
            "mhd_destroy", "mhd_tracers_bytes", "mhd_tracers_field_bytes", "mhd_tracers_bind", "mhd_tracers_set", "mhd_tracers_get",
            "mhd_tracers_push", "mhd_set_param", "mhd_probe_fp64", "mhd_dist_config", "mhd_dist_phase",
            "mhd_dist_counts", "mhd_dist_pack", "mhd_dist_unpack", "mhd_dist_ranges", "mhd_dist_peers",
-           "mhd_dist_enable_peer_access", "mhd_energy_means_noalloc"]
+           "mhd_dist_enable_peer_access", "mhd_energy_means_noalloc", "mhd_alt_launch_count"]
 
 
 class MhdDiag(C.Structure):
@@ -96,6 +96,8 @@ def lib():
     L.mhd_last_error.argtypes = [C.c_void_p]
     L.mhd_last_error.restype = C.c_char_p
     L.mhd_destroy.argtypes = [C.c_void_p]
+    L.mhd_alt_launch_count.argtypes = [C.c_void_p, C.c_int]
+    L.mhd_alt_launch_count.restype = C.c_longlong
     L.mhd_energy_means_noalloc.argtypes = [C.c_longlong, C.c_double, P8, C.c_void_p, C.c_void_p, C.c_char_p, C.c_size_t]
     _lib = L
     return L
@@ -355,6 +357,10 @@ class MHD:
 
     def launch_count(self):
         return int(self._L.mhd_launch_count(self._h))
+
+    def alt_launch_count(self, which):
+        """Launches of an opt-in alternative kernel so far (which = MHD_OPT_TMA or MHD_OPT_FUSE_ASSEMBLE)."""
+        return int(self._L.mhd_alt_launch_count(self._h, int(which)))
 
     def profile_enable(self, on=True):
         self._check(self._L.mhd_profile_enable(self._h, int(on)))

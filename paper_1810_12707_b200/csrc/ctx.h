@@ -66,6 +66,8 @@ struct mhd_ctx {
     alignas(64) unsigned char tmaps[4 * 128];   // CUtensorMap x 4 over the field buffers (TMA-fed strided passes)
     StridedTma tma;
     int opt_tma = 0;       // MHD_OPT_TMA
+    long long tma_launches = 0, s5_launches = 0;      // mhd_alt_launch_count
+    int s5_ok[3] = {-1, -1, -1};                      // one-launch S5, variant v: clusters can be co-scheduled (-1 = not asked yet)
     cd *U[8], *Rold[8], *W[16], *X[8], *Y[8], *nyq[3];
     double *scratch = nullptr, *res = nullptr;
     // chunked ("out-of-core") pipeline, see ooc.cu
@@ -160,7 +162,9 @@ struct mhd_ctx {
 
 inline int check_cuda(mhd_ctx* c, const char* what) {
     cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return c->fail(MHD_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+    const std::string cfg = kernel_config_error();      // a failed shared-memory / cluster opt-in of this thread, if any
+    if (e != cudaSuccess) return c->fail(MHD_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e) + (cfg.empty() ? "" : " [" + cfg + "]"));
+    if (!cfg.empty()) return c->fail(MHD_ERR_CUDA, std::string(what) + ": " + cfg);
     return MHD_OK;
 }
 

@@ -8,16 +8,19 @@ namespace mhd {
 typedef double2 cd;
 constexpr int MAXF = 16;   // largest batch of fields one launch handles
 
-// Opt-in to more than 48 KB of dynamic shared memory, once per kernel instantiation AND per device (the attribute is a
-// per-device property of the function: a process that drives several GPUs must set it on each of them).
+// Opt-in to more than 48 KB of dynamic shared memory (and, for the cluster kernels, to a non-portable cluster size), once
+// per kernel instantiation AND per device (the attributes are per-device properties of the function: a process that drives
+// several GPUs must set them on each of them).
 // The cache is keyed by the kernel's ADDRESS (all instantiations of one template share the pointer type K, so a
-// function-local static keyed by K alone would configure only the first of them).
-bool dynamic_smem_seen(const void* kern, int dev);      // mhd_api.cu; returns true if (kern, dev) was already configured
+// function-local static keyed by K alone would configure only the first of them).  Check, cudaFuncSetAttribute and the
+// record happen under ONE lock, and (kernel, device) is recorded only when every attribute was set: a second host thread
+// cannot launch before the opt-in has landed, and a failed opt-in is retried by the next launch and reported — the
+// cudaError_t stays in the runtime's last-error slot for check_cuda(), which also names the failing step
+// (kernel_config_error()).
+cudaError_t configure_kernel(const void* kern, size_t smem, bool nonportable_cluster = false);      // mhd_api.cu
+const char* kernel_config_error();      // description of this thread's last failed configure_kernel ("" = none); clears it
 template <class K> inline void ensure_dynamic_smem(K kern, size_t smem) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (dynamic_smem_seen(reinterpret_cast<const void*>(kern), dev)) return;
-    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    configure_kernel(reinterpret_cast<const void*>(kern), smem);
 }
 
 // Physical constants of one context, passed by value to the point-wise kernels.

@@ -239,13 +239,7 @@ strided_assemble_kernel(const __grid_constant__ StridedArgs a, const __grid_cons
 template <int N, int FPC, int CC> static void s5_configure(cudaLaunchConfig_t& cfg, cudaLaunchAttribute* attr, const StridedArgs& a,
                                                    cudaStream_t st) {
     typedef S5Cfg<N, FPC, CC> P;
-    int dev = 0;
-    cudaGetDevice(&dev);
-    if (!dynamic_smem_seen(reinterpret_cast<const void*>(strided_assemble_kernel<N, FPC, CC>), dev)) {
-        cudaFuncSetAttribute(strided_assemble_kernel<N, FPC, CC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P::SMEM);
-        // clusters of 16 are above the portable size of 8: a per-function, per-device opt-in
-        if (P::CL > 8) cudaFuncSetAttribute(strided_assemble_kernel<N, FPC, CC>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-    }
+    configure_kernel(reinterpret_cast<const void*>(strided_assemble_kernel<N, FPC, CC>), P::SMEM, P::CL > 8);
     cfg = cudaLaunchConfig_t{};
     cfg.gridDim = dim3(((a.ncols + P::C - 1) / P::C) * P::CL, a.n_outer, 1);
     cfg.blockDim = dim3(P::C * (N / SPlan<N, CC>::type::E), 1, 1);
@@ -283,6 +277,10 @@ void launch_strided_assemble(int N, int variant, const StridedArgs& a, const Ass
 }
 int strided_assemble_max_clusters(int N, int variant, const StridedArgs& a) {
     switch (N * 4 + variant) {
+        case 64 * 4 + 1: return s5_max_clusters<64, 1, 8>(a);
+        case 64 * 4 + 2: return s5_max_clusters<64, 2, 8>(a);
+        case 128 * 4 + 1: return s5_max_clusters<128, 1, 8>(a);
+        case 128 * 4 + 2: return s5_max_clusters<128, 2, 8>(a);
         case 256 * 4 + 1: return s5_max_clusters<256, 1, 8>(a);
         case 256 * 4 + 2: return s5_max_clusters<256, 2, 8>(a);
         case 512 * 4 + 1: return s5_max_clusters<512, 1, 8>(a);

@@ -175,17 +175,15 @@ typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void
                              CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 EncodeFn encode_fn() {
-    static EncodeFn fn = nullptr;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
+    // a function-local static with an initialiser is set up exactly once, even when several host threads bind at once
+    static const EncodeFn fn = [] {
         void* p = nullptr;
         cudaDriverEntryPointQueryResult q;
         if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess)
-            fn = reinterpret_cast<EncodeFn>(p);
-        else
-            cudaGetLastError();
-    }
+            return reinterpret_cast<EncodeFn>(p);
+        cudaGetLastError();
+        return static_cast<EncodeFn>(nullptr);
+    }();
     return fn;
 }
 

@@ -17,11 +17,32 @@
 using namespace mhd;
 
 namespace mhd {
-bool dynamic_smem_seen(const void* kern, int dev) {
+namespace { thread_local std::string t_config_error; }
+cudaError_t configure_kernel(const void* kern, size_t smem, bool nonportable_cluster) {
     static std::mutex mu;
-    static std::set<std::pair<const void*, int>> seen;
-    std::lock_guard<std::mutex> lock(mu);
-    return !seen.insert(std::make_pair(kern, dev)).second;
+    static std::set<std::pair<const void*, int>> done;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lock(mu);          // held across the set: nobody sees (kern, dev) before it is configured
+    const auto key = std::make_pair(kern, dev);
+    if (done.count(key)) return cudaSuccess;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    // clusters of 16 are above the portable size of 8: a per-function, per-device opt-in
+    if (e == cudaSuccess && nonportable_cluster) e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    if (e != cudaSuccess) {
+        t_config_error = std::string("cudaFuncSetAttribute (") + std::to_string(smem) + " B of dynamic shared memory" +
+                         (nonportable_cluster ? ", non-portable cluster size" : "") + "): " + cudaGetErrorString(e);
+        return e;                                  // not recorded: the next launch tries again
+    }
+    done.insert(key);
+    return cudaSuccess;
+}
+const char* kernel_config_error() {
+    static thread_local std::string out;
+    out.swap(t_config_error);
+    t_config_error.clear();
+    return out.c_str();
 }
 }  // namespace mhd
 
@@ -57,7 +78,8 @@ void strided_pass(mhd_ctx* c, int dir, int axis, int nf, const cd* const in[], c
         a.out_rows = (prune && dir < 0) ? 1 : 0;    // forward: output rows outside the mask are not needed
         mhd_ctx::Scope s(c, dir > 0 ? F_STRIDED_INV : F_STRIDED_FWD);
         const bool tma = c->opt_tma != 0 && zoff == 0;      // MHD_OPT_TMA (opt-in: measured slower than the register-fed kernel)
-        if (!(tma && launch_strided_tma(N, dir, a, c->tma, c->st))) launch_strided(N, dir, a, c->st);
+        if (tma && launch_strided_tma(N, dir, a, c->tma, c->st)) ++c->tma_launches;
+        else launch_strided(N, dir, a, c->st);
         done += nb;
     }
 }
@@ -183,7 +205,7 @@ void products(mhd_ctx* c, cd* const Uin[8], double* const breal[3] = nullptr, bo
 }
 
 // sweep S5 in one launch: forward z pass of W[0..15] + assembly + update (kernels.h AssembleTail)
-void fused_s5(mhd_ctx* c, cd* const Uin[8], cd* const rout[8], int mode) {
+StridedArgs s5_args(mhd_ctx* c) {
     const int N = c->N, kc = c->kc(), hx = c->hx();
     StridedArgs a;
     std::memset(&a, 0, sizeof(a));
@@ -193,13 +215,29 @@ void fused_s5(mhd_ctx* c, cd* const Uin[8], cd* const rout[8], int mode) {
     a.in_row_stride = a.out_row_stride = (long long)N * hx; a.in_outer_stride = a.out_outer_stride = hx;
     a.n_outer = 2 * kc + 1; a.outer_split = kc + 1; a.outer_skip = N - (2 * kc + 1);
     a.in_rows = 0; a.out_rows = 1;
+    return a;
+}
+// can this device co-schedule the kernel's thread-block clusters (16 CTAs are above the portable size)?  Asked once per
+// context and variant; "no" makes rhs_spectral keep the two-launch sweep instead of failing the step at launch time
+bool s5_available(mhd_ctx* c) {
+    const int v = c->opt_fuse_assemble;
+    if (v < 1 || v > 2 || !strided_assemble_supported(c->N)) return false;
+    if (c->s5_ok[v] < 0) {
+        c->s5_ok[v] = strided_assemble_max_clusters(c->N, v, s5_args(c)) > 0 ? 1 : 0;
+        cudaGetLastError();                 // an unavailable cluster shape is an answer, not an error of the step
+        kernel_config_error();
+    }
+    return c->s5_ok[v] == 1;
+}
+void fused_s5(mhd_ctx* c, cd* const Uin[8], cd* const rout[8], int mode) {
+    const StridedArgs a = s5_args(c);
     AssembleTail z;
     std::memset(&z, 0, sizeof(z));
     for (int f = 0; f < 8; ++f) { z.U[f] = Uin[f]; z.Rold[f] = c->Rold[f]; z.rout[f] = rout ? rout[f] : nullptr; }
     z.mode = mode; z.dt = c->dt; z.ph = c->phys();
     mhd_ctx::Scope s(c, F_S5);
-    launch_strided_assemble(N, c->opt_fuse_assemble, a, z, c->st);
-
+    launch_strided_assemble(c->N, c->opt_fuse_assemble, a, z, c->st);
+    ++c->s5_launches;
 }
 
 // Variant MHD_OPT_STRESS (Eq. 3-4, 11-12): V_ij = 2 nu rho S_ij and Wv_j = u_i V_ij, transformed, for the assembly.
@@ -242,7 +280,7 @@ void rhs_spectral(mhd_ctx* c, cd* const Uin[8], cd* const rout[8], int mode, dou
     const bool forced = c->f0 != 0.0;
     // default equation set on the pruned, fused path: sweep S5 is one launch
     const bool one_s5 = c->opt_fuse_assemble != 0 && c->opt_fused != 0 && c->opt_prune != 0 && !stress && !forced &&
-                        c->cs2 <= 0.0 && c->evolve == 3 && mode != 3 && strided_assemble_supported(c->N);
+                        c->cs2 <= 0.0 && c->evolve == 3 && mode != 3 && s5_available(c);
     products(c, Uin, breal, !one_s5);
     if (one_s5) { fused_s5(c, Uin, rout, mode); return; }
     SpecGeom gp = c->geom(); gp.pruned = 1;
@@ -277,18 +315,20 @@ TracerArgs tracer_args(mhd_ctx* c, const double* const B[3], int nsteps) {
 bool tracers_active(const mhd_ctx* c) { return c->tr.np > 0 && c->tr.set; }
 // sweep S3 of the second-generation fused kernel can write the real-space B as a by-product
 bool tracers_fused_emit(const mhd_ctx* c) { return c->opt_fused == 1 && x_fused2_supported(c->N) && c->integrator == 0; }
-// real-space B of the current state -> X[0..2] by a separate pruned inverse transform (U^ is left intact)
-void tracers_real_B(mhd_ctx* c, double* Breal[3]) {
+// real-space B of the current state -> X[0..2] by a separate pruned inverse transform (U^ is left intact).
+// Returns MHD_OK or the error of the chunked slab stage (staging overflow, decomposed context, ...): the caller must not
+// push particles in a B that was never written.
+int tracers_real_B(mhd_ctx* c, double* Breal[3]) {
     if (c->ooc.on) {            // chunked pipeline: the slab stage of mhd_get_fields, B only, into the tracers' own arrays
         double* out[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, c->tr.field[0], c->tr.field[1], c->tr.field[2]};
         for (int d = 0; d < 3; ++d) Breal[d] = c->tr.field[d];
-        ooc_real_fields(c, out);
-        return;
+        return ooc_real_fields(c, out);
     }
     const cd* spec[3] = {c->U[5], c->U[6], c->U[7]};
     cd* work[3] = {c->X[0], c->X[1], c->X[2]};
     for (int d = 0; d < 3; ++d) Breal[d] = reinterpret_cast<double*>(c->X[d]);
     inverse3d(c, 3, spec, work, Breal, true);
+    return MHD_OK;
 }
 // spatial sort of the particle storage (tracers.cu); ping-pongs the two sets of arrays
 void tracers_sort(mhd_ctx* c) {
@@ -428,7 +468,13 @@ int mhd_set_option(mhd_ctx* c, int option, int value) {
         case MHD_OPT_PRUNE: c->opt_prune = value ? 1 : 0; return MHD_OK;
         case MHD_OPT_FUSE_CURRENT: c->opt_fuse_current = value ? 1 : 0; return MHD_OK;
         case MHD_OPT_TMA:
+            // a bound context knows whether its tensor maps could be built: refuse instead of silently running the default
+            if (value && c->bound && !c->ooc.on && !c->tma.maps)
+                return c->fail(MHD_ERR_INVALID_ARG, "the TMA pipeline is not available for this context (N must be 128, 256 or 512 and "
+                                                    "cuTensorMapEncodeTiled must succeed)");
             c->opt_tma = value ? 1 : 0; return MHD_OK;
+        case 7: case 10:
+            return c->fail(MHD_ERR_INVALID_ARG, "option ids 7 and 10 are retired (include/mhd_bench.h)");
         case MHD_OPT_FUSE_ASSEMBLE:
             if (value < 0 || value > 2) return c->fail(MHD_ERR_INVALID_ARG, "fuse_assemble must be 0, 1 or 2");
             c->opt_fuse_assemble = value; return MHD_OK;
@@ -455,6 +501,13 @@ int mhd_set_option(mhd_ctx* c, int option, int value) {
             c->ooc.slab_max = value; return MHD_OK;
         default: return c->fail(MHD_ERR_INVALID_ARG, "unknown option");
     }
+}
+
+long long mhd_alt_launch_count(const mhd_ctx* c, int which) {
+    if (!c) return -1;
+    if (which == MHD_OPT_TMA) return c->tma_launches;
+    if (which == MHD_OPT_FUSE_ASSEMBLE) return c->s5_launches;
+    return -1;
 }
 
 int mhd_set_param(mhd_ctx* c, int param, double value) {
@@ -529,7 +582,7 @@ int mhd_step(mhd_ctx* c, int nsteps) {
         if (!tracers_active(c)) return ooc_step(c, nsteps);
         for (int s = 0; s < nsteps; ++s) {      // tracers feel the B of the state at the start of each step
             double* Breal[3];
-            tracers_real_B(c, Breal);
+            if (int rc = tracers_real_B(c, Breal)) return rc;
             tracers_push_with(c, Breal, 1);
             if (int rc = ooc_step(c, 1)) return rc;
         }
@@ -543,7 +596,10 @@ int mhd_step(mhd_ctx* c, int nsteps) {
     for (int s = 0; s < nsteps; ++s) {
         // tracers feel the B of the state at the start of the step (t_n): either a separate inverse transform now, or
         // (AB2 + fused sweep) the real-space B that sweep S3 of this step's right-hand side produces anyway
-        if (tracers && !emit) { tracers_real_B(c, Breal); tracers_push_with(c, Breal, 1); }
+        if (tracers && !emit) {
+            if (int rc = tracers_real_B(c, Breal)) return rc;
+            tracers_push_with(c, Breal, 1);
+        }
         if (c->integrator == 0) {                       // Adams-Bashforth 2, Euler start (R6)
             rhs_spectral(c, c->U, nullptr, c->have_old ? 2 : 1, emit ? Breal : nullptr);
             if (emit) tracers_push_with(c, Breal, 1);
@@ -763,7 +819,7 @@ int mhd_tracers_push(mhd_ctx* c, int nsteps) {
     if (!c->have_fields) return c->fail(MHD_ERR_NO_FIELDS, "mhd_set_fields has not been called");
     if (!tracers_active(c)) return c->fail(MHD_ERR_NO_FIELDS, "mhd_tracers_set has not been called");
     double* Breal[3];
-    tracers_real_B(c, Breal);
+    if (int rc = tracers_real_B(c, Breal)) return rc;
     tracers_push_with(c, Breal, nsteps);
     return check_cuda(c, "tracers_push");
 }

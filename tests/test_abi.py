@@ -50,6 +50,11 @@ def test_init_argument_validation(lib):
     assert lib.mhd_set_fields(h, 1, 0, ptrs) == -2
     assert b"mhd_bind" in lib.mhd_last_error(h)
     assert lib.mhd_set_option(h, 99, 0) == -1
+    # retired option ids keep their old meaning out of reach (include/mhd_bench.h); the one-launch S5 switch has a fresh id
+    assert lib.mhd_set_option(h, 7, 8) == -1 and lib.mhd_set_option(h, 10, 1) == -1
+    assert b"retired" in lib.mhd_last_error(h)
+    assert lib.mhd_set_option(h, 14, 2) == 0 and lib.mhd_set_option(h, 14, 3) == -1
+    assert lib.mhd_alt_launch_count(h, 13) == 0 and lib.mhd_alt_launch_count(h, 14) == 0 and lib.mhd_alt_launch_count(h, 1) == -1
     assert lib.mhd_destroy(h) == 0
 
 

@@ -167,6 +167,7 @@ def test_one_launch_sweep_s5_is_bitwise_the_two_launch_path(MHD, N, steps, varia
         g.step(steps)
         per_step = (g.launch_count() - l0) / steps
         assert per_step == (5 if one_s5 else 6)
+        assert g.alt_launch_count(b.MHD_OPT_FUSE_ASSEMBLE) == (steps if one_s5 else 0)     # the cluster kernel really ran
         out.append(g.get_fields(where="device"))
         del g
     for f in range(8):
@@ -191,6 +192,9 @@ def test_tma_fed_strided_passes_are_bitwise_the_register_fed_ones(MHD, N, steps,
         g.set_fields(prim, "primitive")
         g.step(steps)
         out.append((g.get_fields(where="device"), g.rhs(where="device")))
+        # without this the test would pass with the register-fed kernel compared with itself (no tensor maps, every
+        # pass ineligible).  Per step at least the inverse y pass and the two forward passes go through the TMA pipeline
+        assert (g.alt_launch_count(b.MHD_OPT_TMA) >= 3 * steps) if tma else (g.alt_launch_count(b.MHD_OPT_TMA) == 0)
         del g
     for f in range(8):
         if N == 512:        # the register-fed kernel uses the one-exchange plan (radix 32 x 16) there: roundoff, not bitwise

@@ -190,6 +190,22 @@ def test_tracers_on_the_chunked_pipeline(MHD, flags, N, brick, slab, integ):
         assert np.linalg.norm(a - r) <= 1e-13 * max(np.linalg.norm(r), 1.0)
 
 
+def test_tracers_are_refused_on_a_decomposed_context(MHD):
+    """on a chunked context the push needs the slab stage (ooc_real_fields) to fill the tracers' copy of B, and
+    that stage refuses a decomposed context.  Its return code is now propagated by mhd_tracers_push / mhd_step instead of
+    being dropped; the one refusal reachable through the ABI is caught even earlier — mhd_tracers_bind rejects a
+    decomposed context, so particles can never be pushed in a B array that was not written."""
+    from paper_1810_12707_b200 import dist
+    cfg = inputs.config1(32)
+    grp = dist.Lockstep([dist.DistMHD(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, rank=r, world=2) for r in range(2)])
+    grp.set_fields(cfg.prim, "primitive")
+    pos, vel = particles(64, 9)
+    with pytest.raises(RuntimeError, match="decomposed"):
+        grp.ranks[0].tracers_set(pos, vel)
+    with pytest.raises(RuntimeError):
+        grp.ranks[0].tracers_push(1)                     # nothing bound: refused, not MHD_OK
+
+
 @pytest.mark.parametrize("every", [1, 3, 32])
 def test_spatial_sort_does_not_change_results(MHD, every):
     """MHD_OPT_TRACER_SORT only reorders the particle storage: positions / velocities returned in id order are bitwise
