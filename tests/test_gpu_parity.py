@@ -225,6 +225,102 @@ def test_rhs_configs(orc, MHD, cfgname, N):
     print(cfgname, N, rep)
 
 
+def test_rhs_256_every_point_against_the_oracle(orc, MHD):
+    """The smaller of the two sizes the bench quotes, compared with the oracle AT THAT SIZE at every grid point (VERDICT r2
+    1(a)): BASELINE config 4 (256^3 ABC dynamo).  Per field: the backward-error bar beta <= 2e-15 always; north_star's literal
+    rel. L2 <= 1e-12 where it holds; where the literal bar is at the fp64 noise floor (R_rho cancels exactly, the momentum and
+    energy right-hand sides are differences of O(100) fluxes), SURVEY.md 8(c)-T criterion 3: against the oracle evaluated in
+    long double, the GPU's error is at most twice the fp64 oracle's own."""
+    N = 256
+    cfg = inputs.by_name("4", N)
+    o, g = both(orc, MHD, cfg)
+    Ro, phi, dsc = o.rhs_scales()
+    del o
+    Rg = g.rhs()
+    del g
+    kc = N // 3
+    need_ld = []
+    report = {}
+    for f in range(8):
+        err = float(np.linalg.norm(Rg[f] - Ro[f]))
+        scale = kc * phi[f] + kc * kc * dsc[f]
+        beta = err / max(scale, 1e-300)
+        nrm = float(np.linalg.norm(Ro[f]))
+        rho = err / max(nrm, 1e-300)
+        report[NAMES[f]] = [rho, beta]
+        assert beta <= 2e-15, (NAMES[f], "beta", beta, report)
+        if nrm <= 1e-9 * max(scale, 1e-300) or rho > 1e-12:
+            need_ld.append(f)
+    if need_ld:
+        ld = orc.Oracle(cfg.N, cfg.L, cfg.gamma, cfg.mu, cfg.eta, cfg.dt, long_double=True)
+        ld.set_fields(cfg.prim, "primitive")
+        Rl = ld.rhs()
+        del ld
+        for f in need_ld:
+            e_gpu = float(np.linalg.norm(Rg[f] - Rl[f]))
+            e_o64 = float(np.linalg.norm(Ro[f] - Rl[f]))
+            floor = 1e-17 * max(kc * phi[f] + kc * kc * dsc[f], 1e-300)     # both exactly zero (R_rho of config 4)
+            report[NAMES[f]] += ["criterion 3", e_gpu, e_o64]
+            assert e_gpu <= 2.0 * e_o64 + floor, (NAMES[f], "criterion 3", e_gpu, e_o64, report)
+    print("MEASURED rhs 256^3 config 4 [rho_f, beta_f(, criterion 3: |gpu - ld|, |oracle64 - ld|)]:", report)
+
+
+def _golden_lines():
+    import json
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "rhs_lines.txt")
+    if not os.path.exists(path):
+        return []
+    return [json.loads(l) for l in open(path) if l.strip() and not l.startswith("#")]
+
+
+@pytest.mark.parametrize("kind,N", [("abc", 64), ("random", 64), ("abc", 512), ("random", 512)])
+def test_rhs_on_dense_lines_against_stored_oracle(MHD, kind, N):
+    """512^3 (the size the metric is quoted on) against the ORACLE AT 512^3: tests/golden/rhs_lines.txt holds
+    the oracle's right-hand side of BASELINE config 5 and of a random smooth state on three full grid lines along each of
+    x, y and z per field (written by tests/golden/make_golden_lines.py from oracle/ only).  A line is dense along a
+    transformed axis: every butterfly stage, twiddle and pruning decision of that axis's passes contributes to it.
+    Bars: backward error beta <= 4e-15 per field over the sampled lines (scales phi, dsc of the whole grid, reduced to the
+    sample count; lines are a small sample, hence twice the whole-grid bar) and rel. L2 <= 1e-12 where the field is not an
+    exact cancellation (5e-12 on m and E at 512^3: the oracle's own fp64 noise floor, see below)."""
+    import torch
+    recs = [r for r in _golden_lines() if r["kind"] == kind and r["N"] == N]
+    assert recs, "tests/golden/rhs_lines.txt has no record for %s %d: run tests/golden/make_golden_lines.py" % (kind, N)
+    rec = recs[0]
+    # the recipe of the state is the generator's (make_golden_lines.state: seeded inputs only)
+    prim, L, gamma, mu, eta = (inputs.config45(N).prim, rec["L"], rec["gamma"], rec["mu"], rec["eta"]) if kind == "abc" else \
+        (inputs.random_smooth_state(N, 512, kmax=6), rec["L"], rec["gamma"], rec["mu"], rec["eta"])
+    g = MHD(N, L, gamma, mu, eta, 1e-3)
+    g.set_fields([torch.from_numpy(p).cuda() for p in prim], "primitive")
+    del prim
+    R = g.rhs(where="device")
+    kc = N // 3
+    pts = rec["anchors"]
+    nsamp = 3 * len(pts) * N
+    for f in range(8):
+        got = []
+        for (z, y, x) in pts:
+            got.append(R[f][z, y, :])
+        for (z, y, x) in pts:
+            got.append(R[f][z, :, x])
+        for (z, y, x) in pts:
+            got.append(R[f][:, y, x])
+        got = torch.stack(got).cpu().numpy().ravel()
+        want = np.array(rec["lines"][f], dtype=np.float64).ravel()      # [axis][line][N] in the same order
+        err = float(np.linalg.norm(got - want))
+        scale = (kc * rec["phi"][f] + kc * kc * rec["dsc"][f]) * math.sqrt(nsamp / float(N) ** 3)
+        beta = err / max(scale, 1e-300)
+        assert beta <= 4e-15, (kind, N, NAMES[f], "beta", beta)
+        if rec["norms"][f] > 1e-9 * (kc * rec["phi"][f] + kc * kc * rec["dsc"][f]):
+            rho = err / max(float(np.linalg.norm(want)), 1e-300)
+            # literal bar of north_star; at 512^3 the momentum and energy right-hand sides are differences of nearly uniform
+            # O(100) fluxes and the fp64 ORACLE itself sits 0.9-1.7e-12 from its long-double evaluation (measured at 256^3,
+            # test_rhs_256_every_point_against_the_oracle; no long-double oracle is affordable at 512^3), so two fp64
+            # evaluations cannot be asked to agree to 1e-12 there: 5e-12 (measured 1.35e-12 on m_x of config 5)
+            bar = 5e-12 if (N >= 512 and 1 <= f <= 4) else 1e-12
+            assert rho <= bar, (kind, N, NAMES[f], "rho", rho)
+
+
 def test_rhs_non_2pi_box(orc, MHD):
     N = 32
     prim = inputs.random_smooth_state(N, 11, kmax=3)
@@ -578,6 +674,14 @@ def test_full_size_rhs_against_oracle_subsampled(orc, MHD, N):
     assert abs(d0["ke"] - 1.5) <= 1e-12 and abs(d0["ie"] - 90.0) <= 1e-10 and abs(d0["me"] - 5e-9) <= 1e-20
 
 
+# All-point closed forms: max abs error <= EPS * kc * |flux|.  The bars are the errors MEASURED on a B200 (printed by the tests,
+# `pytest -s`) times a safety factor of 3.5-4: ABC 7.9e-16 (256^3) / 1.14e-15 (512^3) of kc * 5, Orszag-Tang
+# 4.4-5.2e-16 of kc * 10 on every axis pair.  Round 2 allowed 2e-14: a 1e-14-level twiddle or rounding defect
+# now fails.
+ABC_TOL_EPS = 4e-15
+OT_TOL_EPS = 2e-15
+
+
 @pytest.mark.parametrize("N", [256, 512])
 def test_full_size_abc_closed_form(MHD, N):
     U0, P0, mu = 0.7, 2.0, 0.013
@@ -594,12 +698,12 @@ def test_full_size_abc_closed_form(MHD, N):
     q = U0 ** 2 * (1.5 + sz * cy + sx * cz + sy * cx)
     kc = N // 3
     # absolute error bound: kc * |flux| * eps  with |flux| ~ P0 + E ~ 5
-    tol = 2e-15 * kc * 5.0 * 10
-    assert np.max(np.abs(R[0])) <= tol
-    for i in range(3):
-        assert np.max(np.abs(R[1 + i] - (-gq[i] - mu * u[i]))) <= tol
+    tol = ABC_TOL_EPS * kc * 5.0
     RE = -(u[0] * gq[0] + u[1] * gq[1] + u[2] * gq[2]) - 2 * mu * (q - 1.5 * U0 ** 2)
-    assert np.max(np.abs(R[4] - RE)) <= tol
+    errs = [np.max(np.abs(R[0]))] + [np.max(np.abs(R[1 + i] - (-gq[i] - mu * u[i]))) for i in range(3)] + [np.max(np.abs(R[4] - RE))]
+    print("MEASURED abc closed form N=%d: max abs error / (kc * 5) = %.3e (bar %.1e)" % (N, max(errs) / (kc * 5.0), ABC_TOL_EPS))
+    for e in errs:
+        assert e <= tol, errs
     for i in range(3):
         assert np.max(np.abs(R[5 + i])) == 0.0
 
@@ -726,14 +830,17 @@ def test_full_size_orszag_tang_closed_form(MHD, N, perm):
     RE = (sy * Hx - sx * Hy - sy * (cx * s2x + 2 * sx * c2x) + 2 * s2x * sy * cy
           + eta * (Jz * Jz - 4 * s2x ** 2 - sy ** 2) + mu * (c2x + c2y))
     kc = N // 3
-    tol = 2e-15 * kc * 10.0 * 10       # absolute: kc * |flux| * eps with |flux| <= (E + Pt)|u| ~ 10, one decade of margin
-    assert np.max(np.abs(R[0])) <= tol
+    tol = OT_TOL_EPS * kc * 10.0       # absolute: kc * |flux| * eps with |flux| <= (E + Pt)|u| ~ 10
+    errs = [np.max(np.abs(R[0]))]
     for i in range(3):
         exp_m = 0.0 if Rm[i] is None else Rm[i]
         exp_b = 0.0 if RB[i] is None else RB[i]
-        assert np.max(np.abs(R[1 + i] - exp_m)) <= tol, ("m", i)
-        assert np.max(np.abs(R[5 + i] - exp_b)) <= tol, ("B", i)
-    assert np.max(np.abs(R[4] - RE)) <= tol
+        errs += [np.max(np.abs(R[1 + i] - exp_m)), np.max(np.abs(R[5 + i] - exp_b))]
+    errs.append(np.max(np.abs(R[4] - RE)))
+    print("MEASURED orszag-tang closed form N=%d perm=%s: max abs error / (kc * 10) = %.3e (bar %.1e)"
+          % (N, perm, max(errs) / (kc * 10.0), OT_TOL_EPS))
+    for e in errs:
+        assert e <= tol, errs
 
 
 # ---------------------------------------------------------------------------------------------------------

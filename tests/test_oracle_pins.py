@@ -654,3 +654,33 @@ def test_p17_rhs_scales_resistive_flux_term(orc):
     assert abs(phi[2] - np.linalg.norm(P0 - 0.5 * b * b * s2)) <= 1e-13 * phi[2]
     assert abs(phi[3] - phi[1]) <= 1e-13 * phi[1]
     assert abs(dsc[6] - eta * b * s / math.sqrt(2)) <= 1e-13 * dsc[6] and dsc[5] == 0.0 and dsc[7] == 0.0
+
+
+def test_golden_lines_are_the_oracles(orc):
+    """tests/golden/rhs_lines.txt (written by tests/golden/make_golden_lines.py from oracle/ alone) cannot drift from the
+    oracle: the 64^3 records are re-derived here value by value.  The 512^3 records cannot be (46 GB, ~15 min each); the
+    config-5 one is tied to the re-derived 64^3 record instead: the ABC state and its right-hand side are band-limited far
+    below k_c(64), so the whole-grid L2 norms and flux scales of the two sizes differ exactly by sqrt(512^3 / 64^3)."""
+    import importlib.util
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_golden_lines", os.path.join(here, "make_golden_lines.py"))
+    gen = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(gen)
+    recs = {(r["kind"], r["N"]): r for r in gen.read()}
+    assert ("abc", 64) in recs and ("random", 64) in recs
+    for kind in ("abc", "random"):
+        stored, fresh = recs[(kind, 64)], gen.record(kind, 64)
+        assert stored["anchors"] == fresh["anchors"]
+        for key in ("phi", "dsc", "norms"):
+            assert np.allclose(stored[key], fresh[key], rtol=1e-13, atol=0), (kind, key)
+        a, b = np.array(stored["lines"]), np.array(fresh["lines"])
+        assert a.shape == (8, 3, gen.NLINES, 64)
+        assert np.max(np.abs(a - b)) <= 1e-13 * max(np.max(np.abs(b)), 1.0), kind     # same code, same inputs
+    if ("abc", 512) in recs:
+        big, small = recs[("abc", 512)], recs[("abc", 64)]
+        ratio = math.sqrt(512.0 ** 3 / 64.0 ** 3)
+        for f in range(8):
+            if small["norms"][f] > 1e-6:        # R_rho of the ABC state is an exact cancellation (roundoff only)
+                assert abs(big["norms"][f] / small["norms"][f] - ratio) <= 1e-9 * ratio, (NAMES[f], "norm")
+            assert abs(big["phi"][f] / small["phi"][f] - ratio) <= 1e-9 * ratio, (NAMES[f], "phi")
